@@ -1,0 +1,171 @@
+/*
+ * melt.h -- C ABI of the B200-native (sm_100a) MelT / MFCCT hot path (arxiv/paper_2606_01009).
+ *
+ * The library computes, for framed audio, the Direct Mel Projection of PAPER.md section III-A:
+ *
+ *   Eq. (1)-(2) PAPER.md:126-136  M analysis frequencies f_m at the HTK-Mel filterbank centres
+ *   Eq. (3)     PAPER.md:140-145  R_tm = sum_n w[n] x_t[n] cos(2 pi f_m n / fs),  I_tm with sin
+ *   Eq. (4)/(7) PAPER.md:147-171  S = R^2 + I^2
+ *   Eq. (5)-(6) PAPER.md:155-173  window folded into fixed basis matrices; R, I as one dense GEMM
+ *   Eq. (8)     PAPER.md:179-183  MelT = log(S + eps)   -- contract form: log10(max(S, 1e-10))
+ *   Eq. (9)     PAPER.md:187-191  MFCCT = MelT . D^T, D the K x M orthonormal DCT-II
+ *
+ * Every step runs in hand-written CUDA kernels (tcgen05 tensor-core MMAs accumulating in tensor memory,
+ * fused power / log / DCT epilogue).  Frames are never materialised: the overlapping frames are formed
+ * on chip from the raw signal (implicit im2col).  There is no CPU fallback: on a device that is not
+ * sm_100 every entry point that needs the GPU fails with MELT_ERR_UNSUPPORTED.
+ *
+ * Conventions
+ *   - "device" pointers are CUDA device memory of the device that was current at melt_plan_create;
+ *     "host" pointers are ordinary host memory.  The library never takes ownership of caller buffers.
+ *   - All forward calls are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = the
+ *     legacy default stream).  Caller buffers must stay valid until the stream reaches the call.
+ *   - No allocation and no host synchronisation happens inside a forward call.
+ *   - Errors are detected on the host before any launch and returned as melt_status; the message is
+ *     available from melt_last_error() (thread-local).  Kernel-side faults are not reported asynchronously.
+ *   - Inputs must be finite; in MELT_PREC_COMPENSATED mode |x| must stay below 8 * 2^(12 - s) where s is
+ *     MELT_OPT_INPUT_SCALE_LOG2 (default 12, i.e. |x| < 8: audio normalised to [-1, 1] has 8x headroom).
+ */
+#ifndef MELT_H_
+#define MELT_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct melt_plan melt_plan; /* opaque, library-owned */
+
+typedef enum {
+    MELT_OK = 0,
+    MELT_ERR_INVALID_ARG = 1, /* bad scalar, NULL pointer where data is needed, option out of range */
+    MELT_ERR_UNSUPPORTED = 2, /* valid request the sm_100a kernels do not cover, or non-sm_100 device */
+    MELT_ERR_ALIGNMENT = 3,   /* x / out not 4-byte aligned */
+    MELT_ERR_CUDA = 4,        /* a CUDA runtime call failed; melt_last_error() has the CUDA string */
+    MELT_ERR_ALLOC = 5        /* host or device allocation failed (plan creation only) */
+} melt_status;
+
+typedef enum {
+    MELT_WINDOW_HANN_PERIODIC = 0, /* 0.5 - 0.5 cos(2 pi n / N): BASELINE.json configs[0] */
+    MELT_WINDOW_HANN_SYMMETRIC = 1, /* 0.5 - 0.5 cos(2 pi n / (N-1)): PAPER.md:138 */
+    MELT_WINDOW_RECT = 2
+} melt_window;
+
+typedef enum {
+    MELT_MEL_HTK = 0,   /* Eq. (1)-(2) */
+    MELT_MEL_SLANEY = 1 /* not defined by the paper: melt_plan_create returns NULL (UNSUPPORTED) */
+} melt_mel_scale;
+
+typedef enum {
+    MELT_OPT_LAYOUT = 0,           /* melt_layout; default FRAME_MAJOR */
+    MELT_OPT_PRECISION = 1,        /* melt_precision; default COMPENSATED */
+    MELT_OPT_DROP_LAST = 2,        /* 0/1: drop the last frame of every clip (configs[1], [2]); default 0 */
+    MELT_OPT_PAD = 3,              /* melt_pad; default NONE */
+    MELT_OPT_INPUT_SCALE_LOG2 = 4, /* s in [-24, 24]: samples are multiplied by 2^s before the fp16 split of the
+                                      COMPENSATED mode (exact; undone in the epilogue); default 12 */
+    MELT_OPT_OUTPUT = 5            /* melt_output; default LOG */
+} melt_option;
+
+typedef enum {
+    MELT_LAYOUT_FRAME_MAJOR = 0,  /* out[b][t][c]  (configs[0], [3]) */
+    MELT_LAYOUT_FEATURE_MAJOR = 1 /* out[b][c][t]  (configs[1], [2], [4]); dense batches only */
+} melt_layout;
+
+typedef enum {
+    MELT_PREC_COMPENSATED = 0, /* fp16 hi/lo split of both operands, 3 tensor-core products per term, fp32
+                                  accumulate: meets every north-star tolerance */
+    MELT_PREC_TF32 = 1,        /* single kind::tf32 pass (operands rounded to nearest-away tf32) */
+    MELT_PREC_BF16 = 2         /* single kind::f16 pass on bf16 operands */
+} melt_precision;
+
+typedef enum {
+    MELT_PAD_NONE = 0,   /* T = floor((len - n_fft)/hop) + 1 frames per clip; tail samples ignored */
+    MELT_PAD_REFLECT = 1 /* the clip is virtually reflect-padded by n_fft/2 per side (edge sample not repeated);
+                            T = floor(len/hop) + 1 for even n_fft; needs len > n_fft/2 */
+} melt_pad;
+
+typedef enum {
+    MELT_OUTPUT_LOG = 0,  /* log10(max(S, 1e-10)), then the DCT when n_mfcc > 0 */
+    MELT_OUTPUT_POWER = 1 /* S itself (Eq. 4); only with n_mfcc == 0 */
+} melt_output;
+
+/*
+ * melt_plan_create -- builds the analysis frequencies (Eq. 1-2), the window, the window-folded cos/sin basis
+ * (Eq. 5) and, when n_mfcc > 0, the DCT matrix (Eq. 9) in double precision on the host, converts them once to
+ * the tensor-core operand format and uploads them to the current CUDA device.  Synchronous.
+ *   fs > 0 sampling rate (Hz); n_fft >= 2 frame length N; hop >= 1; window: melt_window;
+ *   n_mels >= 1 number of analysis frequencies M; 0 <= fmin < fmax <= fs/2 (Hz); mel_scale: melt_mel_scale;
+ *   0 <= n_mfcc <= min(n_mels, 64): 0 -> log-Mel output with C = n_mels channels, > 0 -> MFCCT with C = n_mfcc.
+ * Returns NULL on error (melt_last_error() says why).  The plan owns its device buffers until melt_plan_destroy.
+ */
+melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window, int n_mels,
+                            double fmin, double fmax, int mel_scale, int n_mfcc);
+
+/* Frees the plan and its device buffers.  NULL is ignored.  Do not destroy a plan with work in flight. */
+void melt_plan_destroy(melt_plan *plan);
+
+/*
+ * melt_plan_set_option -- sets one melt_option.  Allowed until the first forward call on the plan; afterwards the
+ * plan is immutable (so concurrent forwards on different streams are safe) and MELT_ERR_INVALID_ARG is returned.
+ * Changing MELT_OPT_PRECISION rebuilds and re-uploads the operand images (synchronous).
+ */
+int melt_plan_set_option(melt_plan *plan, int key, int value);
+
+/* Frames per clip for a clip of `len` samples under the plan's pad / drop_last options (0 if too short). */
+long long melt_num_frames(const melt_plan *plan, long long len);
+
+/* Output channels per frame: n_mfcc if n_mfcc > 0 else n_mels. */
+int melt_num_channels(const melt_plan *plan);
+
+/* Test hook: copies the n_mels analysis frequencies (Hz) to host memory f_hz[n_mels]. */
+int melt_plan_get_centres(const melt_plan *plan, double *f_hz);
+
+/*
+ * melt_forward -- the whole hot path on a dense batch.
+ *   x    device, fp32, [batch, len] contiguous, 4-byte aligned (16-byte alignment of every clip start, i.e. of x
+ *        and of len*4, enables the vectorised loader);
+ *   out  device, fp32, batch * C * T floats, T = melt_num_frames(plan, len), layout per MELT_OPT_LAYOUT.
+ * batch == 0 or T == 0 is a successful no-op.  Returns a melt_status.
+ */
+int melt_forward(const melt_plan *plan, const float *x, int batch, long long len, float *out, void *stream);
+
+/*
+ * melt_forward_ragged -- the whole hot path on clips packed back to back (configs[3]).
+ *   x                  device, fp32, packed samples;
+ *   offsets            device, int64, n_clips + 1 ascending sample offsets into x (clip i = [offsets[i], offsets[i+1]));
+ *   out                device, fp32, packed frame-major [sum_i T_i, C]; the caller sizes it from the clip lengths
+ *                      (an upper bound is sum_i melt_num_frames(len_i));
+ *   out_frame_offsets  device, int64, n_clips + 1: written by the library, frame offset of every clip in `out`
+ *                      (out_frame_offsets[n_clips] = total frames).  Must not be NULL.
+ * n_clips <= 2^20.  Frame-major layout only.  No host synchronisation: tiles are assigned on the device.
+ */
+int melt_forward_ragged(const melt_plan *plan, const float *x, const long long *offsets, int n_clips,
+                        float *out, long long *out_frame_offsets, void *stream);
+
+/*
+ * melt_forward_tap -- as melt_forward / melt_forward_ragged (offsets == NULL selects the dense form, in which
+ * n_clips is the batch and len the clip length; otherwise len is ignored), and additionally writes the log-Mel
+ * matrix that feeds the DCT to `logmel` (device, fp32, same frame order and layout as `out`, n_mels channels).
+ * Only meaningful for MFCCT plans (n_mfcc > 0); used for two-stage parity checks.  logmel may be NULL.
+ */
+int melt_forward_tap(const melt_plan *plan, const float *x, const long long *offsets, int n_clips, long long len,
+                     float *out, float *logmel, long long *out_frame_offsets, void *stream);
+
+/* Thread-local message of the last error returned on this thread ("" if none). */
+const char *melt_last_error(void);
+
+/* Library / kernel configuration as a short human-readable string for logs (static storage per plan). */
+const char *melt_plan_describe(const melt_plan *plan);
+
+/*
+ * Self-test of the tensor-core building block used by the forward kernels: D[128, n] = A[128, k] . B[n, k]^T
+ * with A written to tensor memory by threads and B read from shared memory (tcgen05.mma, A-from-TMEM form).
+ *   kind: 0 = fp16, 1 = bf16, 2 = tf32;  a, b host fp32 row-major (values are rounded to `kind` inside);
+ *   d host fp32 [128, n] result.  n % 16 == 0, 16 <= n <= 256; k % 16 == 0 (fp16/bf16) or k % 8 == 0 (tf32), k <= 256.
+ * Synchronous.  Returns a melt_status.
+ */
+int melt_selftest_umma(int kind, int n, int k, const float *a, const float *b, float *d);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MELT_H_ */

@@ -1,0 +1,146 @@
+"""Thin ctypes binding over libmelt_b200.so -- same names as the C calls in include/melt.h.
+
+Argument marshalling only: every step of the path (framing, projection, power, log, DCT, store) runs in the
+CUDA kernels behind the C ABI.  PyTorch is used by callers for device memory and streams only; this module
+takes raw device pointers (ints) or torch tensors (``.data_ptr()``).  There is no CPU fallback: if the library
+cannot be loaded the import of a symbol raises.
+"""
+import ctypes as C
+import os
+
+from . import build as _build
+
+MELT_OK, MELT_ERR_INVALID_ARG, MELT_ERR_UNSUPPORTED, MELT_ERR_ALIGNMENT, MELT_ERR_CUDA, MELT_ERR_ALLOC = range(6)
+MELT_WINDOW_HANN_PERIODIC, MELT_WINDOW_HANN_SYMMETRIC, MELT_WINDOW_RECT = 0, 1, 2
+MELT_MEL_HTK, MELT_MEL_SLANEY = 0, 1
+MELT_OPT_LAYOUT, MELT_OPT_PRECISION, MELT_OPT_DROP_LAST, MELT_OPT_PAD, MELT_OPT_INPUT_SCALE_LOG2, MELT_OPT_OUTPUT = range(6)
+MELT_LAYOUT_FRAME_MAJOR, MELT_LAYOUT_FEATURE_MAJOR = 0, 1
+MELT_PREC_COMPENSATED, MELT_PREC_TF32, MELT_PREC_BF16 = 0, 1, 2
+MELT_PAD_NONE, MELT_PAD_REFLECT = 0, 1
+MELT_OUTPUT_LOG, MELT_OUTPUT_POWER = 0, 1
+
+# every symbol include/melt.h declares (tests/test_abi.py checks the header against this list and the .so)
+SYMBOLS = [
+    "melt_plan_create", "melt_plan_destroy", "melt_plan_set_option", "melt_num_frames", "melt_num_channels",
+    "melt_plan_get_centres", "melt_forward", "melt_forward_ragged", "melt_forward_tap", "melt_last_error",
+    "melt_plan_describe", "melt_selftest_umma",
+]
+
+_lib = None
+
+
+class MeltError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("melt status %d: %s" % (status, msg))
+        self.status = status
+
+
+def library_path():
+    return _build.LIB
+
+
+def lib():
+    """Load (building first if the sources are newer) libmelt_b200.so.  Raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if not os.path.exists(path) or _build._stale():
+        path = _build.build()
+    L = C.CDLL(path)
+    vp, ip, ll, dbl = C.c_void_p, C.c_int, C.c_longlong, C.c_double
+    L.melt_plan_create.restype = vp
+    L.melt_plan_create.argtypes = [dbl, ip, ip, ip, ip, dbl, dbl, ip, ip]
+    L.melt_plan_destroy.restype = None
+    L.melt_plan_destroy.argtypes = [vp]
+    L.melt_plan_set_option.argtypes = [vp, ip, ip]
+    L.melt_num_frames.restype = ll
+    L.melt_num_frames.argtypes = [vp, ll]
+    L.melt_num_channels.argtypes = [vp]
+    L.melt_plan_get_centres.argtypes = [vp, C.POINTER(dbl)]
+    L.melt_forward.argtypes = [vp, vp, ip, ll, vp, vp]
+    L.melt_forward_ragged.argtypes = [vp, vp, vp, ip, vp, vp, vp]
+    L.melt_forward_tap.argtypes = [vp, vp, vp, ip, ll, vp, vp, vp, vp]
+    L.melt_last_error.restype = C.c_char_p
+    L.melt_plan_describe.restype = C.c_char_p
+    L.melt_plan_describe.argtypes = [vp]
+    L.melt_selftest_umma.argtypes = [ip, ip, ip, vp, vp, vp]
+    _lib = L
+    return L
+
+
+def _ptr(t):
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    return int(t.data_ptr())
+
+
+def _check(rc):
+    if rc != MELT_OK:
+        raise MeltError(rc, melt_last_error())
+
+
+def melt_last_error():
+    return lib().melt_last_error().decode()
+
+
+def melt_plan_create(fs, n_fft, hop, window, n_mels, fmin, fmax, mel_scale=MELT_MEL_HTK, n_mfcc=0):
+    h = lib().melt_plan_create(float(fs), int(n_fft), int(hop), int(window), int(n_mels), float(fmin), float(fmax),
+                               int(mel_scale), int(n_mfcc))
+    if not h:
+        raise MeltError(-1, melt_last_error())
+    return h
+
+
+def melt_plan_destroy(plan):
+    lib().melt_plan_destroy(plan)
+
+
+def melt_plan_set_option(plan, key, value):
+    _check(lib().melt_plan_set_option(plan, int(key), int(value)))
+
+
+def melt_num_frames(plan, length):
+    return int(lib().melt_num_frames(plan, int(length)))
+
+
+def melt_num_channels(plan):
+    return int(lib().melt_num_channels(plan))
+
+
+def melt_plan_get_centres(plan, n_mels):
+    buf = (C.c_double * n_mels)()
+    _check(lib().melt_plan_get_centres(plan, buf))
+    return list(buf)
+
+
+def melt_plan_describe(plan):
+    return lib().melt_plan_describe(plan).decode()
+
+
+def melt_forward(plan, x, batch, length, out, stream=0):
+    _check(lib().melt_forward(plan, _ptr(x), int(batch), int(length), _ptr(out), stream or None))
+
+
+def melt_forward_ragged(plan, x, offsets, n_clips, out, out_frame_offsets, stream=0):
+    _check(lib().melt_forward_ragged(plan, _ptr(x), _ptr(offsets), int(n_clips), _ptr(out), _ptr(out_frame_offsets),
+                                     stream or None))
+
+
+def melt_forward_tap(plan, x, offsets, n_clips, length, out, logmel, out_frame_offsets, stream=0):
+    _check(lib().melt_forward_tap(plan, _ptr(x), _ptr(offsets), int(n_clips), int(length), _ptr(out), _ptr(logmel),
+                                  _ptr(out_frame_offsets), stream or None))
+
+
+def melt_selftest_umma(kind, a, b):
+    """a [128, k], b [n, k] numpy float32 (host) -> d [128, n] numpy float32."""
+    import numpy as np
+    a = np.ascontiguousarray(a, np.float32)
+    b = np.ascontiguousarray(b, np.float32)
+    n, k = b.shape
+    assert a.shape == (128, k)
+    d = np.empty((128, n), np.float32)
+    _check(lib().melt_selftest_umma(int(kind), n, k, a.ctypes.data, b.ctypes.data, d.ctypes.data))
+    return d

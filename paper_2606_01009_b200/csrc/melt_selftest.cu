@@ -1,0 +1,139 @@
+// melt_selftest.cu -- self-test of the tensor-core building block of the forward kernels:
+// D[128, n] = A[128, k] . B[n, k]^T with A written to tensor memory by threads (thread = row, tcgen05.st),
+// B brought to shared memory by the bulk-copy engine in the no-swizzle canonical layout, one tcgen05.mma
+// (A-from-TMEM form) per K-step issued by a single thread, completion through tcgen05.commit -> mbarrier,
+// and the accumulator read back with tcgen05.ld.  Exactly the mechanisms melt_fwd_kernel relies on.
+#include "melt_internal.h"
+#include "sm100_ptx.cuh"
+
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+namespace melt {
+
+struct SelftestParams {
+    int kind, n, k;
+    const float *a;      // device [128, k] fp32
+    const uint8_t *bimg; // device, K-step slabs of n*32 bytes
+    float *d;            // device [128, n]
+};
+
+__global__ void __launch_bounds__(128, 1) selftest_umma_kernel(const SelftestParams p) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    __shared__ __align__(8) uint64_t bar_b, bar_mma;
+    __shared__ uint32_t tmem_base_s;
+
+    const int tid = threadIdx.x, warp = tid >> 5;
+    const int kstep = p.kind == OP_TF32 ? 8 : 16;
+    const int nsteps = p.k / kstep;
+    const uint32_t slab = (uint32_t)p.n * 32u;
+
+    if (tid == 0) {
+        mbar_init(smem_u32(&bar_b), 1);
+        mbar_init(smem_u32(&bar_mma), 1);
+        fence_barrier_init();
+    }
+    if (warp == 0) {
+        tmem_alloc(smem_u32(&tmem_base_s), 512);
+        tmem_relinquish();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = tmem_base_s;
+
+    if (tid == 0) {
+        mbar_arrive_expect_tx(smem_u32(&bar_b), slab * (uint32_t)nsteps);
+        for (int s = 0; s < nsteps; ++s)
+            bulk_g2s(smem_u32(smem) + (uint32_t)s * slab, p.bimg + (size_t)s * slab, slab, smem_u32(&bar_b));
+    }
+
+    // A: row `tid` -> TMEM lane `tid`, columns [256, ...): 16-bit kinds pack two K elements per column (even k low).
+    const uint32_t a_col0 = 256;
+    const uint32_t lane_addr = tmem_base + ((uint32_t)(warp * 32) << 16);
+    const float *arow = p.a + (size_t)tid * p.k;
+    for (int s = 0; s < nsteps; ++s) {
+        uint32_t v[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+            if (p.kind == OP_TF32) {
+                v[c] = cvt_tf32_rna(arow[s * 8 + c]);
+            } else if (p.kind == OP_F16) {
+                __half2 h = __floats2half2_rn(arow[s * 16 + 2 * c], arow[s * 16 + 2 * c + 1]);
+                v[c] = *reinterpret_cast<uint32_t *>(&h);
+            } else {
+                __nv_bfloat162 h = __floats2bfloat162_rn(arow[s * 16 + 2 * c], arow[s * 16 + 2 * c + 1]);
+                v[c] = *reinterpret_cast<uint32_t *>(&h);
+            }
+        }
+        tmem_st8(lane_addr + a_col0 + (uint32_t)s * 8u, v);
+    }
+    tmem_wait_st();
+    tc_fence_before();
+    __syncthreads();
+
+    if (tid == 0) {
+        tc_fence_after();
+        mbar_wait(smem_u32(&bar_b), 0);
+        const uint32_t idesc = umma_idesc(p.kind == OP_F16 ? UMMA_F16 : (p.kind == OP_BF16 ? UMMA_BF16 : UMMA_TF32), (uint32_t)p.n);
+        for (int s = 0; s < nsteps; ++s) {
+            uint64_t bdesc = umma_smem_desc_kmajor_noswz(smem_u32(smem) + (uint32_t)s * slab, 128, 256);
+            if (p.kind == OP_TF32) umma_ts_tf32(tmem_base, tmem_base + a_col0 + (uint32_t)s * 8u, bdesc, idesc, s > 0);
+            else umma_ts_f16(tmem_base, tmem_base + a_col0 + (uint32_t)s * 8u, bdesc, idesc, s > 0);
+        }
+        tc_commit(smem_u32(&bar_mma));
+    }
+    mbar_wait(smem_u32(&bar_mma), 0);
+    tc_fence_after();
+
+    for (int c0 = 0; c0 < p.n; c0 += 16) {
+        uint32_t v[16];
+        tmem_ld16(lane_addr + (uint32_t)c0, v);
+        tmem_wait_ld();
+#pragma unroll
+        for (int c = 0; c < 16; ++c) p.d[(size_t)tid * p.n + c0 + c] = __uint_as_float(v[c]);
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tmem_base, 512);
+}
+
+}  // namespace melt
+
+extern "C" int melt_selftest_umma(int kind, int n, int k, const float *a, const float *b, float *d) {
+    using namespace melt;
+    if (kind < 0 || kind > 2 || !a || !b || !d) return fail(MELT_ERR_INVALID_ARG, "melt_selftest_umma: bad argument");
+    const int kstep = operand_kstep(kind);
+    if (n < 16 || n > 256 || n % 16 || k < kstep || k > 256 || k % kstep)
+        return fail(MELT_ERR_INVALID_ARG, "melt_selftest_umma: n=%d k=%d out of range", n, k);
+    int dev = 0;
+    cudaDeviceProp prop;
+    MELT_CUDA(cudaGetDevice(&dev));
+    MELT_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) return fail(MELT_ERR_UNSUPPORTED, "device is sm_%d%d, need sm_100", prop.major, prop.minor);
+
+    const int nsteps = k / kstep;
+    const size_t slab = (size_t)n * 32, img_bytes = slab * nsteps;
+    if (img_bytes > 200 * 1024) return fail(MELT_ERR_INVALID_ARG, "melt_selftest_umma: B image too large");
+    std::vector<uint8_t> img(img_bytes);
+    for (int s = 0; s < nsteps; ++s)
+        pack_b_slab(kind, n, [&](int r, int kk) { return (double)b[(size_t)r * k + s * kstep + kk]; }, img.data() + s * slab);
+
+    float *da = nullptr, *dd = nullptr;
+    uint8_t *dimg = nullptr;
+    MELT_CUDA(cudaMalloc(&da, sizeof(float) * 128 * k));
+    MELT_CUDA(cudaMalloc(&dd, sizeof(float) * 128 * n));
+    MELT_CUDA(cudaMalloc(&dimg, img_bytes));
+    MELT_CUDA(cudaMemcpy(da, a, sizeof(float) * 128 * k, cudaMemcpyHostToDevice));
+    MELT_CUDA(cudaMemcpy(dimg, img.data(), img_bytes, cudaMemcpyHostToDevice));
+    MELT_CUDA(cudaFuncSetAttribute(selftest_umma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)img_bytes));
+    SelftestParams p{kind, n, k, da, dimg, dd};
+    selftest_umma_kernel<<<1, 128, img_bytes>>>(p);
+    MELT_CUDA(cudaGetLastError());
+    MELT_CUDA(cudaDeviceSynchronize());
+    MELT_CUDA(cudaMemcpy(d, dd, sizeof(float) * 128 * n, cudaMemcpyDeviceToHost));
+    cudaFree(da);
+    cudaFree(dd);
+    cudaFree(dimg);
+    return MELT_OK;
+}
