@@ -1,0 +1,361 @@
+// melt_plan.cu -- host side of the C ABI: plan construction (Eq. 1, 2, 5, 9 in double precision, conversion to
+// tensor-core operand images), options, validation and the forward entry points.
+//
+// What the plan precomputes:
+//   * f_m.
+//   * The window w[n] and its symmetry centre c = (a0 + b0)/2.  Both Hann flavours and the
+//     rectangular window satisfy w[a0 + j] = w[b0 - j]; P = R^2 + I^2 does not depend on the phase origin, so with
+//     the phase referred to c the cos rows are even and the sin rows odd about c, and Eq. (3) folds to
+//         R' = sum_j wc[m][j] (x[a0+j] + x[b0-j]),   I' = sum_j ws[m][j] (x[a0+j] - x[b0-j]),   j = 0..kf-1
+//     with wc[m][j] = g_j w[a0+j] cos(w_m (a0 + j - c)), ws[m][j] = w[a0+j] sin(w_m (a0 + j - c)), g_j = 1/2 for
+//     the self-paired centre sample, 1 otherwise.  R'^2 + I'^2 = R^2 + I^2 exactly; half the MMA work of Eq. (6).
+//   * The basis images: for every pass over the Mel bins and every K-step, one contiguous slab per operand kind in
+//     the no-swizzle canonical UMMA layout, so that the kernel moves a K-step of the basis with ONE bulk copy.
+#include "melt_plan.h"
+
+#include <algorithm>
+
+namespace melt {
+
+static const double kPi = 3.14159265358979323846264338327950288;
+static const int kBasisScaleLog2 = 14;  // COMPENSATED: basis stored as 2^14 * value (keeps the fp16 lo part normal)
+
+static double hz_to_mel(double f) { return 2595.0 * std::log10(1.0 + f / 700.0); }    // Eq. (1)
+static double mel_to_hz(double m) { return 700.0 * (std::pow(10.0, m / 2595.0) - 1.0); }  // Eq. (2)
+
+static long long frames_for(const melt_plan *p, long long len) {
+    if (len < 0) return 0;
+    long long padded = len;
+    if (p->pad == MELT_PAD_REFLECT) {
+        if (len < (long long)(p->n_fft / 2) + 1) return 0;
+        padded += 2LL * (p->n_fft / 2);
+    }
+    if (padded < p->n_fft) return 0;
+    long long T = (padded - p->n_fft) / p->hop + 1 - (p->drop_last ? 1 : 0);
+    return T < 0 ? 0 : T;
+}
+
+static void free_device(melt_plan *p) {
+    cudaFree(p->d_bimg);
+    cudaFree(p->d_tab);
+    cudaFree(p->d_dct);
+    p->d_bimg = nullptr;
+    p->d_tab = nullptr;
+    p->d_dct = nullptr;
+}
+
+static int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+int plan_build_device(melt_plan *p) {
+    KParams &k = p->kp;
+    const int N = p->n_fft, H = p->hop, M = p->n_mels;
+    const int kind = p->precision == MELT_PREC_COMPENSATED ? OP_F16 : (p->precision == MELT_PREC_BF16 ? OP_BF16 : OP_TF32);
+    const bool comp = p->precision == MELT_PREC_COMPENSATED;
+
+    // ---- fold geometry
+    const int c2 = (p->window == MELT_WINDOW_HANN_PERIODIC) ? N : N - 1;  // w[n] = w[c2 - n]
+    k.a0 = (c2 + 1) / 2;
+    k.b0 = c2 / 2;
+    k.kf = N - k.a0;
+    if (k.kf < 1) return fail(MELT_ERR_UNSUPPORTED, "n_fft=%d too short for the folded projection", N);
+    for (int j = 0; j < k.kf; ++j) {
+        int na = k.a0 + j, nb = k.b0 - j;
+        double wb = nb >= 0 ? p->win[nb] : 0.0;
+        if (nb < 0 && std::fabs(p->win[na]) > 1e-14) return fail(MELT_ERR_UNSUPPORTED, "window is not symmetric");
+        if (nb >= 0 && std::fabs(p->win[na] - wb) > 1e-13) return fail(MELT_ERR_UNSUPPORTED, "window is not symmetric");
+    }
+    const double centre = 0.5 * (double)c2;
+
+    // ---- tiling of the contraction and of the Mel bins
+    k.n_fft = N; k.hop = H; k.n_mels = M; k.n_mfcc = p->n_mfcc; k.n_ch = p->n_mfcc > 0 ? p->n_mfcc : M;
+    k.kstep = operand_kstep(kind);
+    k.units = (k.kf + k.kstep - 1) / k.kstep;
+    k.nk = comp ? 4 : 2;
+    k.passes = (M + 127) / 128;
+    k.nb = round_up((M + k.passes - 1) / k.passes, 16);
+    k.acc_cols = 2 * k.nb;
+    k.unit_cols = k.nk * 8;
+    k.acc_stages = (2 * k.acc_cols + 4 * k.unit_cols <= 512) ? 2 : 1;
+    k.a_col0 = k.acc_stages * k.acc_cols;
+    k.a_slots = std::min(MAX_A_SLOTS, (512 - k.a_col0) / k.unit_cols);
+    if (k.a_slots < 2) return fail(MELT_ERR_UNSUPPORTED, "tensor-memory budget exceeded (nb=%d)", k.nb);
+    k.unit_b_bytes = (uint32_t)(k.nk * k.nb * 32);
+    k.dct_pitch = round_up(std::max(p->n_mfcc, 1), 4);
+
+    // ---- shared-memory plan
+    const uint32_t tab_bytes = (uint32_t)(k.units * k.kstep * 4);
+    const uint32_t dct_bytes = p->n_mfcc > 0 ? (uint32_t)(M * k.dct_pitch * 4) : 0;
+    const uint32_t bar_bytes = 1024;
+    const uint32_t fixed = round_up((int)(tab_bytes + dct_bytes + bar_bytes), 128) + 128;
+    const int rows_whole = TILE_M + (N - 1) / H;          // hop-rows touched by one tile
+    const int pitch_whole = rows_whole | 1;               // odd: conflict-free transposed stores
+    const long long whole_words = (long long)H * pitch_whole + TILE_M;
+    const long long whole_bytes = whole_words * 4;
+    k.hop_inv40 = ((1ull << 40) + (unsigned long long)H - 1) / (unsigned long long)H;
+    const bool whole_ok = whole_words < 65536 && (long long)TILE_M * H + N < (1 << 24) && H < 65536 &&
+                          whole_bytes + 2LL * k.unit_b_bytes + fixed <= SMEM_BUDGET;
+    uint32_t stg_bytes;
+    if (whole_ok) {
+        k.stg_comb = 0; k.stg_slots = 1; k.chunk_units = k.units;
+        k.stg_pitch = pitch_whole; k.stg_slot_words = (int)whole_words;
+        stg_bytes = (uint32_t)whole_bytes;
+    } else {
+        k.stg_comb = 1; k.chunk_units = 64 / k.kstep;  // 64 folded samples per chunk
+        k.stg_pitch = TILE_M + 1;
+        k.stg_slot_words = 2 * 64 * k.stg_pitch + TILE_M;
+        k.stg_slots = 3;
+        stg_bytes = (uint32_t)(k.stg_slots * k.stg_slot_words * 4);
+    }
+    const long long b_room = (long long)SMEM_BUDGET - stg_bytes - fixed;
+    int fit = (int)std::min<long long>(b_room / k.unit_b_bytes, MAX_B_SLOTS);
+    if (fit < 2) return fail(MELT_ERR_UNSUPPORTED, "shared-memory budget exceeded (n_fft=%d hop=%d n_mels=%d)", N, H, M);
+    k.b_resident = (k.passes == 1 && k.units <= fit) ? 1 : 0;
+    k.b_slots = k.b_resident ? k.units : std::min(fit, 8);
+    k.off_b = 0;
+    k.off_stg = (uint32_t)round_up((int)(k.b_slots * k.unit_b_bytes), 128);
+    k.off_tab = k.off_stg + (uint32_t)round_up((int)stg_bytes, 128);
+    k.off_dct = k.off_tab + (uint32_t)round_up((int)tab_bytes, 16);
+    k.off_bar = (uint32_t)round_up((int)(k.off_dct + dct_bytes), 16);
+    k.smem_bytes = k.off_bar + bar_bytes;
+    if (k.smem_bytes > (uint32_t)SMEM_BUDGET) return fail(MELT_ERR_UNSUPPORTED, "shared-memory budget exceeded");
+
+    // ---- numerics
+    const int s_in = comp ? p->in_scale_log2 : 0, s_b = comp ? kBasisScaleLog2 : 0;
+    k.in_scale = (float)std::ldexp(1.0, s_in);
+    k.out_scale = (float)std::ldexp(1.0, -2 * (s_in + s_b));
+    k.out_log10_offset = (float)(-2.0 * (s_in + s_b) * std::log10(2.0));
+    k.output_power = p->output == MELT_OUTPUT_POWER;
+    k.pad = p->pad; k.drop_last = p->drop_last; k.feature_major = p->layout == MELT_LAYOUT_FEATURE_MAJOR;
+
+    // ---- staging offset table: for folded index j, where samples a0 + j and b0 - j of a frame live in a staging slot
+    //      (word offset of row 0; the converter adds its row).  j >= kf (K padding) points at the zero row.
+    std::vector<uint32_t> tab((size_t)k.units * k.kstep);
+    const uint32_t zero_off = (uint32_t)(k.stg_slot_words - TILE_M);
+    for (int j = 0; j < k.units * k.kstep; ++j) {
+        uint32_t oa = zero_off, ob = zero_off;
+        if (j < k.kf) {
+            if (!k.stg_comb) {
+                int na = k.a0 + j, nb = k.b0 - j;
+                oa = (uint32_t)((na % H) * k.stg_pitch + na / H);
+                ob = nb >= 0 ? (uint32_t)((nb % H) * k.stg_pitch + nb / H) : zero_off;
+            } else {
+                int jc = j % 64;
+                oa = (uint32_t)(jc * k.stg_pitch);
+                ob = (k.b0 - j >= 0) ? (uint32_t)((64 + jc) * k.stg_pitch) : zero_off;
+            }
+        }
+        tab[j] = oa | (ob << 16);
+    }
+
+    // ---- basis images (Eq. 5 folded), double -> operand format in one rounding
+    const double bscale = std::ldexp(1.0, s_b);
+    const size_t img_bytes = (size_t)k.passes * k.units * k.unit_b_bytes;
+    std::vector<uint8_t> img(img_bytes, 0);
+    auto coef = [&](int m, int j, bool sine) -> double {
+        if (m >= M || j >= k.kf) return 0.0;
+        const int na = k.a0 + j;
+        const double g = (na == k.b0 - j) ? 0.5 : 1.0;
+        const double arg = 2.0 * kPi * p->centres[m] * ((double)na - centre) / p->fs;
+        return bscale * p->win[na] * (sine ? std::sin(arg) : g * std::cos(arg));
+    };
+    auto hi_of = [&](double v) -> double {
+        if (kind == OP_F16) return f16_bits_to_f64(f64_to_f16_bits(v));
+        if (kind == OP_BF16) return bf16_bits_to_f64(f64_to_bf16_bits(v));
+        return tf32_bits_to_f64(f64_to_tf32_bits(v));
+    };
+    for (int ps = 0; ps < k.passes; ++ps)
+        for (int u = 0; u < k.units; ++u) {
+            uint8_t *slab = img.data() + ((size_t)ps * k.units + u) * k.unit_b_bytes;
+            for (int kk = 0; kk < k.nk; ++kk) {
+                // kinds: COMPENSATED [wc_hi, wc_lo, ws_hi, ws_lo]; single pass [wc, ws]
+                const bool sine = comp ? (kk >= 2) : (kk == 1);
+                const bool lo = comp && (kk & 1);
+                pack_b_slab(kind, k.nb, [&](int r, int kq) {
+                    double v = coef(ps * k.nb + r, u * k.kstep + kq, sine);
+                    return lo ? v - hi_of(v) : v;
+                }, slab + (size_t)kk * k.nb * 32);
+            }
+        }
+
+    // ---- DCT table (Eq. 9), [m][k] so a thread reads all k of one bin as float4s
+    std::vector<float> dct;
+    if (p->n_mfcc > 0) {
+        dct.assign((size_t)M * k.dct_pitch, 0.f);
+        for (int m = 0; m < M; ++m)
+            for (int q = 0; q < p->n_mfcc; ++q) {
+                double d = q == 0 ? std::sqrt(1.0 / M) : std::sqrt(2.0 / M) * std::cos(kPi * q * (2 * m + 1) / (2.0 * M));
+                dct[(size_t)m * k.dct_pitch + q] = (float)d;
+            }
+    }
+
+    // ---- upload
+    free_device(p);
+    MELT_CUDA(cudaMalloc(&p->d_bimg, img_bytes));
+    MELT_CUDA(cudaMemcpy(p->d_bimg, img.data(), img_bytes, cudaMemcpyHostToDevice));
+    MELT_CUDA(cudaMalloc(&p->d_tab, tab.size() * 4));
+    MELT_CUDA(cudaMemcpy(p->d_tab, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice));
+    if (!dct.empty()) {
+        MELT_CUDA(cudaMalloc(&p->d_dct, dct.size() * 4));
+        MELT_CUDA(cudaMemcpy(p->d_dct, dct.data(), dct.size() * 4, cudaMemcpyHostToDevice));
+    }
+    k.b_img = p->d_bimg; k.tab = p->d_tab; k.dct = p->d_dct;
+
+    char buf[512];
+    snprintf(buf, sizeof(buf),
+             "melt_b200 prec=%s fold(a0=%d,b0=%d,kf=%d) kstep=%d units=%d nb=%d passes=%d tmem(acc=%dx%d,a_slots=%d) "
+             "basis=%s(%d x %u B) staging=%s(%d x %d words) smem=%u B",
+             comp ? "fp16x3" : (kind == OP_BF16 ? "bf16" : "tf32"), k.a0, k.b0, k.kf, k.kstep, k.units, k.nb, k.passes,
+             k.acc_stages, k.acc_cols, k.a_slots, k.b_resident ? "resident" : "ring", k.b_slots, k.unit_b_bytes,
+             k.stg_comb ? "comb" : "whole", k.stg_slots, k.stg_slot_words, k.smem_bytes);
+    p->desc = buf;
+    return MELT_OK;
+}
+
+static int validate_common(const melt_plan *p, const float *x, float *out) {
+    if (!p) return fail(MELT_ERR_INVALID_ARG, "plan is NULL");
+    if (!x || !out) return fail(MELT_ERR_INVALID_ARG, "x / out is NULL");
+    if (((uintptr_t)x & 3) || ((uintptr_t)out & 3)) return fail(MELT_ERR_ALIGNMENT, "x / out must be 4-byte aligned");
+    int dev = -1;
+    MELT_CUDA(cudaGetDevice(&dev));
+    if (dev != p->device) return fail(MELT_ERR_INVALID_ARG, "plan was created on device %d, current device is %d", p->device, dev);
+    return MELT_OK;
+}
+
+static int forward_impl(const melt_plan *p, const float *x, const long long *offsets, int n_clips, long long len,
+                        float *out, float *tap, long long *out_frame_offsets, void *stream) {
+    int rc = validate_common(p, x, out);
+    if (rc) return rc;
+    if (n_clips < 0) return fail(MELT_ERR_INVALID_ARG, "negative clip count");
+    if (tap && ((uintptr_t)tap & 3)) return fail(MELT_ERR_ALIGNMENT, "logmel must be 4-byte aligned");
+    const_cast<melt_plan *>(p)->used = true;
+    if (n_clips == 0) return MELT_OK;
+    KParams kp = p->kp;
+    kp.x = x; kp.out = out; kp.tap = tap; kp.n_clips = n_clips;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (offsets) {
+        if (n_clips > MAX_CLIPS) return fail(MELT_ERR_UNSUPPORTED, "n_clips=%d exceeds %d", n_clips, MAX_CLIPS);
+        if (!out_frame_offsets) return fail(MELT_ERR_INVALID_ARG, "out_frame_offsets is NULL");
+        if (kp.feature_major) return fail(MELT_ERR_UNSUPPORTED, "ragged batches are frame-major only");
+        rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, st);
+        if (rc) return rc;
+        kp.offsets = offsets; kp.frame_offsets = out_frame_offsets; kp.tile_prefix = p->d_tile_prefix;
+        kp.len = 0; kp.frames_per_clip = 0; kp.tiles_per_clip = 0; kp.n_tiles = -1;
+    } else {
+        if (len < 0) return fail(MELT_ERR_INVALID_ARG, "negative len");
+        const long long T = frames_for(p, len);
+        if (T == 0) return MELT_OK;
+        const long long tpc = (T + TILE_M - 1) / TILE_M;
+        if (tpc * n_clips > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
+        kp.offsets = nullptr; kp.frame_offsets = nullptr; kp.tile_prefix = nullptr;
+        kp.len = len; kp.frames_per_clip = T; kp.tiles_per_clip = (int)tpc; kp.n_tiles = (int)(tpc * n_clips);
+    }
+    return launch_forward(p, kp, st);
+}
+
+}  // namespace melt
+
+using namespace melt;
+
+extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window, int n_mels, double fmin, double fmax,
+                                       int mel_scale, int n_mfcc) {
+    if (!(fs > 0.0) || !std::isfinite(fs)) { set_error("fs must be positive"); return nullptr; }
+    if (n_fft < 2 || n_fft > 65536) { set_error("n_fft=%d out of range [2, 65536]", n_fft); return nullptr; }
+    if (hop < 1 || hop > 65535) { set_error("hop=%d out of range [1, 65535]", hop); return nullptr; }
+    if (window < 0 || window > 2) { set_error("unknown window %d", window); return nullptr; }
+    if (n_mels < 1 || n_mels > 1024) { set_error("n_mels=%d out of range [1, 1024]", n_mels); return nullptr; }
+    if (!(fmin >= 0.0) || !(fmax > fmin) || !(fmax <= fs / 2.0 * (1.0 + 1e-12))) {
+        set_error("need 0 <= fmin < fmax <= fs/2 (got %g, %g, fs=%g)", fmin, fmax, fs);
+        return nullptr;
+    }
+    if (mel_scale != MELT_MEL_HTK) { set_error("mel_scale %d unsupported: the paper defines the HTK scale only", mel_scale); return nullptr; }
+    if (n_mfcc < 0 || n_mfcc > n_mels || n_mfcc > MAX_MFCC) { set_error("n_mfcc=%d out of range [0, min(n_mels, %d)]", n_mfcc, MAX_MFCC); return nullptr; }
+    int dev = 0;
+    cudaDeviceProp prop;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
+    if (e != cudaSuccess) { cuda_fail(e, "cudaGetDeviceProperties"); return nullptr; }
+    if (prop.major != 10) { set_error("device is sm_%d%d: this library is sm_100a only and has no fallback", prop.major, prop.minor); return nullptr; }
+
+    melt_plan *p = new (std::nothrow) melt_plan();
+    if (!p) { set_error("out of host memory"); return nullptr; }
+    p->fs = fs; p->fmin = fmin; p->fmax = fmax; p->n_fft = n_fft; p->hop = hop; p->window = window; p->n_mels = n_mels;
+    p->mel_scale = mel_scale; p->n_mfcc = n_mfcc;
+    p->layout = MELT_LAYOUT_FRAME_MAJOR; p->precision = MELT_PREC_COMPENSATED; p->drop_last = 0; p->pad = MELT_PAD_NONE;
+    p->in_scale_log2 = 12; p->output = MELT_OUTPUT_LOG; p->used = false; p->device = dev; p->sm_count = prop.multiProcessorCount;
+    p->d_bimg = nullptr; p->d_tab = nullptr; p->d_dct = nullptr; p->d_tile_prefix = nullptr; p->d_frame_offsets_scratch = nullptr;
+    memset(&p->kp, 0, sizeof(p->kp));
+    // Eq. (1)-(2): M centres uniformly spaced in mel between fmin and fmax, endpoints excluded
+    p->centres.resize(n_mels);
+    const double mlo = hz_to_mel(fmin), mhi = hz_to_mel(fmax);
+    for (int m = 0; m < n_mels; ++m) p->centres[m] = mel_to_hz(mlo + (double)(m + 1) * (mhi - mlo) / (double)(n_mels + 1));
+    p->win.resize(n_fft);
+    for (int n = 0; n < n_fft; ++n) {
+        if (window == MELT_WINDOW_HANN_PERIODIC) p->win[n] = 0.5 - 0.5 * std::cos(2.0 * kPi * n / n_fft);
+        else if (window == MELT_WINDOW_HANN_SYMMETRIC) p->win[n] = 0.5 - 0.5 * std::cos(2.0 * kPi * n / (n_fft - 1));
+        else p->win[n] = 1.0;
+    }
+    e = cudaMalloc(&p->d_tile_prefix, sizeof(int) * (size_t)(MAX_CLIPS + 1));
+    if (e != cudaSuccess) { cuda_fail(e, "cudaMalloc(tile_prefix)"); melt_plan_destroy(p); return nullptr; }
+    if (plan_build_device(p) != MELT_OK) { melt_plan_destroy(p); return nullptr; }
+    return p;
+}
+
+extern "C" void melt_plan_destroy(melt_plan *p) {
+    if (!p) return;
+    free_device(p);
+    cudaFree(p->d_tile_prefix);
+    delete p;
+}
+
+extern "C" int melt_plan_set_option(melt_plan *p, int key, int value) {
+    if (!p) return fail(MELT_ERR_INVALID_ARG, "plan is NULL");
+    if (p->used) return fail(MELT_ERR_INVALID_ARG, "plan is immutable after its first forward call");
+    switch (key) {
+        case MELT_OPT_LAYOUT:
+            if (value < 0 || value > 1) return fail(MELT_ERR_INVALID_ARG, "bad layout %d", value);
+            p->layout = value; break;
+        case MELT_OPT_PRECISION:
+            if (value < 0 || value > 2) return fail(MELT_ERR_INVALID_ARG, "bad precision %d", value);
+            p->precision = value; break;
+        case MELT_OPT_DROP_LAST:
+            if (value < 0 || value > 1) return fail(MELT_ERR_INVALID_ARG, "bad drop_last %d", value);
+            p->drop_last = value; break;
+        case MELT_OPT_PAD:
+            if (value < 0 || value > 1) return fail(MELT_ERR_INVALID_ARG, "bad pad %d", value);
+            p->pad = value; break;
+        case MELT_OPT_INPUT_SCALE_LOG2:
+            if (value < -24 || value > 24) return fail(MELT_ERR_INVALID_ARG, "bad input scale %d", value);
+            p->in_scale_log2 = value; break;
+        case MELT_OPT_OUTPUT:
+            if (value < 0 || value > 1) return fail(MELT_ERR_INVALID_ARG, "bad output %d", value);
+            if (value == MELT_OUTPUT_POWER && p->n_mfcc > 0) return fail(MELT_ERR_INVALID_ARG, "power output needs n_mfcc == 0");
+            p->output = value; break;
+        default:
+            return fail(MELT_ERR_INVALID_ARG, "unknown option %d", key);
+    }
+    return plan_build_device(p);
+}
+
+extern "C" long long melt_num_frames(const melt_plan *p, long long len) { return p ? frames_for(p, len) : 0; }
+extern "C" int melt_num_channels(const melt_plan *p) { return p ? p->kp.n_ch : 0; }
+
+extern "C" int melt_plan_get_centres(const melt_plan *p, double *f_hz) {
+    if (!p || !f_hz) return fail(MELT_ERR_INVALID_ARG, "NULL argument");
+    std::copy(p->centres.begin(), p->centres.end(), f_hz);
+    return MELT_OK;
+}
+
+extern "C" const char *melt_plan_describe(const melt_plan *p) { return p ? p->desc.c_str() : ""; }
+
+extern "C" int melt_forward(const melt_plan *p, const float *x, int batch, long long len, float *out, void *stream) {
+    return forward_impl(p, x, nullptr, batch, len, out, nullptr, nullptr, stream);
+}
+extern "C" int melt_forward_ragged(const melt_plan *p, const float *x, const long long *offsets, int n_clips, float *out,
+                                   long long *out_frame_offsets, void *stream) {
+    if (!offsets) return fail(MELT_ERR_INVALID_ARG, "offsets is NULL");
+    return forward_impl(p, x, offsets, n_clips, 0, out, nullptr, out_frame_offsets, stream);
+}
+extern "C" int melt_forward_tap(const melt_plan *p, const float *x, const long long *offsets, int n_clips, long long len,
+                                float *out, float *logmel, long long *out_frame_offsets, void *stream) {
+    return forward_impl(p, x, offsets, n_clips, len, out, logmel, out_frame_offsets, stream);
+}

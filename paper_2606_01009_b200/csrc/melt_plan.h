@@ -1,0 +1,78 @@
+// melt_plan.h -- the plan object and the kernel parameter block (host + device view).
+#pragma once
+#include "melt_internal.h"
+
+namespace melt {
+
+constexpr int TILE_M = 128;         // frames per tile = UMMA M
+constexpr int MAX_B_SLOTS = 32;     // shared-memory slots (K-step slabs) of the basis ring / resident basis
+constexpr int MAX_A_SLOTS = 8;      // tensor-memory slots (K-steps) of the A-operand ring
+constexpr int MAX_STG_SLOTS = 4;    // signal staging slots
+constexpr int MAX_CLIPS = 1 << 20;  // ragged batches: clips per call
+constexpr int MAX_MFCC = 64;
+constexpr int SMEM_BUDGET = 232448; // 227 KB: max dynamic shared memory per CTA on sm_100
+
+// Warp roles of melt_fwd_kernel (20 warps).
+constexpr int WARP_BPROD = 0, WARP_MMA = 1, WARP_TMEM = 2, WARP_EPI0 = 4, WARP_CONV0 = 8, WARP_LOAD0 = 16;
+constexpr int NUM_WARPS = 20, NUM_THREADS = NUM_WARPS * 32;
+constexpr int NUM_EPI_THREADS = 128, NUM_CONV_THREADS = 256, NUM_LOAD_THREADS = 128;
+
+struct KParams {
+    // ---- analysis geometry
+    int n_fft, hop, n_mels, n_mfcc, n_ch;  // n_ch = output channels per frame
+    int a0, b0, kf;                        // folded pairs: (a0 + j, b0 - j), j = 0..kf-1
+    int kstep, units;                      // K elements per MMA, K-steps per pass (ceil(kf / kstep))
+    int nb, passes;                        // Mel bins per pass (multiple of 16), number of passes over the bins
+    int nk;                                // operand kinds per term: 4 (hi/lo x sum/diff) or 2
+    // ---- tensor memory map (columns)
+    int acc_cols, acc_stages, unit_cols, a_slots, a_col0;
+    // ---- shared memory map (bytes from the dynamic smem base)
+    int b_resident, b_slots;
+    uint32_t unit_b_bytes;
+    int stg_comb, stg_slots, chunk_units, stg_pitch, stg_slot_words;
+    unsigned long long hop_inv40;          // ceil(2^40 / hop): exact division of sample indices < 2^24
+    uint32_t off_b, off_stg, off_tab, off_dct, off_bar, smem_bytes;
+    int dct_pitch;                         // floats per Mel bin in the DCT table (n_mfcc rounded up to 4)
+    // ---- numerics
+    float in_scale, out_scale, out_log10_offset;
+    int output_power;
+    // ---- batch
+    const float *x;
+    float *out, *tap;
+    const long long *offsets;       // ragged: device sample offsets (n_clips + 1), else NULL
+    const long long *frame_offsets; // ragged: device frame offsets written by the scan kernel
+    const int *tile_prefix;         // ragged: device exclusive prefix of tiles per clip (n_clips + 1)
+    int n_clips;
+    long long len;                  // dense: samples per clip
+    long long frames_per_clip;      // dense: T
+    int tiles_per_clip, n_tiles;    // dense
+    int pad, drop_last, feature_major;
+    // ---- plan-owned device data
+    const uint8_t *b_img;  // [passes][units] slabs of unit_b_bytes
+    const uint32_t *tab;   // [units * kstep] packed staging offsets (lo16: a0 + j sample, hi16: b0 - j sample)
+    const float *dct;      // [n_mels][dct_pitch]
+};
+
+}  // namespace melt
+
+struct melt_plan {
+    double fs, fmin, fmax;
+    int n_fft, hop, window, n_mels, mel_scale, n_mfcc;
+    int layout, precision, drop_last, pad, in_scale_log2, output;
+    bool used;
+    int device, sm_count;
+    std::vector<double> centres, win;
+    melt::KParams kp;  // geometry + plan-owned device pointers (batch fields filled per call)
+    uint8_t *d_bimg;
+    uint32_t *d_tab;
+    float *d_dct;
+    int *d_tile_prefix;
+    long long *d_frame_offsets_scratch;
+    std::string desc;
+};
+
+namespace melt {
+int plan_build_device(melt_plan *p);  // (re)builds geometry + operand images for the current options
+int launch_forward(const melt_plan *p, const KParams &kp, cudaStream_t stream);
+int launch_ragged_scan(const melt_plan *p, const long long *offsets, int n_clips, long long *frame_offsets, cudaStream_t stream);
+}  // namespace melt
