@@ -1,0 +1,331 @@
+#!/usr/bin/env python
+"""bench.py -- measures the MelT hot path on B200 (contract: see the task statement / DESIGN.md "Measurement").
+
+    python bench.py --gpus 1 --steps 50 --warmup 10                 # the CUDA path (default workload: cfg1)
+    python bench.py --impl reference --steps 3 --warmup 1           # the fp64 CPU oracle on a bounded sample
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W                      # N independent shards, no collective (weak scaling)
+
+One "step" = one pass of the whole hot path (framing -> projection -> power -> log [-> DCT] -> store) over one
+synthetic batch of the named workload.  Prints ONE JSON line on rank 0.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2606_01009_b200 import workloads as wl  # noqa: E402
+
+METRIC = "log-Mel frames/s"
+PEAKS_FALLBACK = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+PREC_NAMES = {"compensated": 0, "tf32": 1, "bf16": 2}
+PREC_DTYPE = {"compensated": "f16", "tf32": "tf32", "bf16": "bf16"}
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            d = json.load(fh)
+        d["_source"] = "measured"
+        return d
+    d = dict(PEAKS_FALLBACK)
+    d["_source"] = "fallback"
+    return d
+
+
+def workload_numbers(cfg, n_clips):
+    """Algorithmic work of one step: frames, audio seconds, flops, bytes."""
+    c = wl.CONFIGS[cfg]
+    N, H, M, K = c["n_fft"], c["hop"], c["n_mels"], c["n_mfcc"]
+    if cfg == "cfg3":
+        raise ValueError("ragged workload numbers come from the generated lengths")
+    L = c["clip_len"]
+    padded = L + (2 * (N // 2) if c["pad_reflect"] else 0)
+    T = (padded - N) // H + 1 - (1 if c["drop_last"] else 0)
+    frames = n_clips * T
+    C = K if K else M
+    return dict(frames=frames, audio_s=n_clips * L / c["fs"], T=T, C=C,
+                flops=2.0 * frames * 2 * M * N + 2.0 * frames * M * K,
+                bytes_in=4.0 * n_clips * L, bytes_out=4.0 * frames * C)
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc, self.thr = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thr = threading.Thread(target=self._read, daemon=True)
+        self.thr.start()
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.rows.append([t.strip() for t in ln.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for nm, val in zip(names, r[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def time_oracle(cfg, n_clips_sample, reps):
+    """The fp64 oracle as it stands on the host cores, on a bounded sample of the workload (frames/s)."""
+    from oracle import melt_oracle as orc
+    c = wl.CONFIGS[cfg]
+    d = wl.make_inputs(cfg, n_clips_sample)
+    kw = dict(fs=c["fs"], n_fft=c["n_fft"], hop=c["hop"], window_kind=c["window"], n_mels=c["n_mels"], fmin=c["fmin"],
+              fmax=c["fmax"], n_mfcc=c["n_mfcc"], drop_last=c["drop_last"], want=("L", "C"))
+    frames = 0
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        for b in range(d["x"].shape[0]):
+            frames += next(iter(orc.forward(d["x"][b], **kw).values())).shape[0]
+    dt = time.perf_counter() - t0
+    return frames / dt, dt, orc.num_threads(), frames
+
+
+def run_reference(args):
+    """--impl reference: the oracle IS the reference arm for this tier (bounded sample per step)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = args.workload
+    c = wl.CONFIGS[cfg]
+    sample_clips = args.cpu_clips
+    for _ in range(args.warmup):
+        time_oracle(cfg, 1, 1)
+    fps, dt, cores, frames = time_oracle(cfg, sample_clips, args.steps)
+    nums = workload_numbers(cfg, sample_clips)
+    sample = "%d of %d clips of %s per step (%d frames), fp64 direct sums, OpenMP over frames" % (
+        sample_clips, c["n_clips"], cfg, nums["frames"])
+    line = {
+        "impl": "reference", "metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "audio_s_per_s": fps * c["hop"] / c["fs"],
+        "config": {"workload": cfg, "sample": sample, "n_fft": c["n_fft"], "hop": c["hop"], "n_mels": c["n_mels"]},
+        "cpu_baseline": {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": fps, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=50)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="cfg1", choices=[k for k in wl.CONFIGS if k != "cfg3"])
+    ap.add_argument("--precision", default="compensated", choices=list(PREC_NAMES))
+    ap.add_argument("--clips", type=int, default=0, help="clips per GPU (default: the config's)")
+    ap.add_argument("--buffer-sets", type=int, default=0, help="rotating input/output sets (default: enough to exceed 2x L2)")
+    ap.add_argument("--cpu-clips", type=int, default=4, help="clips in the oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "cuda":
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2606_01009_b200 import binding as mb
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --impl cuda needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist_mod.init_process_group("nccl", device_id=torch.device("cuda", local))
+        dist = dist_mod
+
+    cfg = args.workload
+    c = wl.CONFIGS[cfg]
+    n_clips = args.clips or c["n_clips"]
+    nums = workload_numbers(cfg, n_clips)
+    peaks = load_peaks()
+
+    # ---- plan
+    plan = mb.melt_plan_create(*wl.plan_args(c))
+    mb.melt_plan_set_option(plan, mb.MELT_OPT_PRECISION, PREC_NAMES[args.precision])
+    mb.melt_plan_set_option(plan, mb.MELT_OPT_DROP_LAST, int(c["drop_last"]))
+    mb.melt_plan_set_option(plan, mb.MELT_OPT_LAYOUT, int(c["layout"] == "feature_major"))
+    desc = mb.melt_plan_describe(plan)
+
+    # ---- inputs: same per-clip streams on every rank but rank-shifted seed (weak scaling: every rank owns a full batch)
+    data = wl.make_inputs(cfg, n_clips, seed=c["seed"] + 7919 * rank)
+    x_host = torch.from_numpy(data["x"])
+    B, L = x_host.shape
+    T, C = mb.melt_num_frames(plan, L), mb.melt_num_channels(plan)
+    assert B * T == nums["frames"] and C == nums["C"], (B, T, C, nums)
+    set_bytes = x_host.numel() * 4 + B * C * T * 4
+    l2_bytes = torch.cuda.get_device_properties(local).L2_cache_size
+    nsets = args.buffer_sets or max(2, int(np.ceil(2.2 * l2_bytes / set_bytes)) + 1)
+    xs = [x_host.cuda() if i == 0 else None for i in range(nsets)]
+    for i in range(1, nsets):
+        xs[i] = torch.roll(xs[0], shifts=i, dims=0).contiguous()   # same clips, different addresses and order
+    outs = [torch.empty((B, C, T) if c["layout"] == "feature_major" else (B, T, C), device="cuda") for _ in range(nsets)]
+    stream = torch.cuda.current_stream()
+
+    def step(i):
+        mb.melt_forward(plan, xs[i % nsets], B, L, outs[i % nsets], stream.cuda_stream)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing
+    for i in range(args.warmup):
+        step(i)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    evs[0].record()
+    for i in range(args.steps):
+        step(i)
+        evs[i + 1].record()
+    barrier()
+    total_ms = evs[0].elapsed_time(evs[-1])
+    per_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(args.steps)]
+    clocks = sampler.stop() if rank == 0 else None
+    if dist is not None:
+        t = torch.tensor([total_ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    frames_all = nums["frames"] * world
+    value = frames_all / (ms_per_step * 1e-3)
+
+    # ---- end to end through the C ABI with HOST buffers (pinned): H2D + kernel + D2H inside the timed region
+    x_pin = x_host.pin_memory()
+    out_pin = torch.empty(outs[0].shape, dtype=torch.float32).pin_memory()
+    e2e_steps = max(3, min(args.steps, 20))
+
+    def e2e_step(i):
+        xs[i % nsets].copy_(x_pin, non_blocking=True)
+        mb.melt_forward(plan, xs[i % nsets], B, L, outs[i % nsets], stream.cuda_stream)
+        out_pin.copy_(outs[i % nsets], non_blocking=True)
+
+    for i in range(3):
+        e2e_step(i)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(e2e_steps):
+        e2e_step(i)
+    e1.record()
+    barrier()
+    e2e_ms = e0.elapsed_time(e1) / e2e_steps
+    if dist is not None:
+        t = torch.tensor([e2e_ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_value = frames_all / (e2e_ms * 1e-3)
+
+    if rank != 0:
+        mb.melt_plan_destroy(plan)
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the one kernel of the step
+    kernel_ms = statistics.mean(per_ms)
+    kernel_ms_median = statistics.median(per_ms)
+    dtype = PREC_DTYPE[args.precision]
+    tensor_peak = peaks["bf16_tflops"] * (0.5 if dtype == "tf32" else 1.0)      # burst: the kernel is timed alone
+    t_hbm = (nums["bytes_in"] + nums["bytes_out"]) / (peaks["hbm_gbs"] * 1e9)
+    t_tensor = nums["flops"] / (tensor_peak * 1e12)
+    if t_hbm >= t_tensor:
+        achieved = (nums["bytes_in"] + nums["bytes_out"]) / (kernel_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
+    else:
+        achieved = nums["flops"] / (kernel_ms * 1e-3) / 1e12
+        roof = {"bound": "tensor", "achieved": achieved, "peak": tensor_peak, "unit": "TFLOP/s"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"] = None
+    roof.update({"peaks": peaks["_source"], "kernel_ms": kernel_ms, "kernel_ms_median": kernel_ms_median,
+                 "kernel_ms_min": min(per_ms), "t_hbm_us": t_hbm * 1e6, "t_tensor_us": t_tensor * 1e6,
+                 "tensor_peak_dtype": dtype, "algorithmic_bytes": nums["bytes_in"] + nums["bytes_out"],
+                 "algorithmic_flops": nums["flops"],
+                 "frac_vs_tf32_roofline": max(t_hbm, nums["flops"] / (peaks["bf16_tflops"] * 0.5e12)) / (kernel_ms * 1e-3)})
+    prof = os.path.join(ROOT, "profiles", "traffic_%s_%s.json" % (cfg, args.precision))
+    if os.path.exists(prof):
+        with open(prof) as fh:
+            roof["traffic"] = json.load(fh).get("dram_bytes_per_launch")
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        fps, dt, cores, frames = time_oracle(cfg, args.cpu_clips, 1)
+        cpu = {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle",
+               "sample": "%d of %d clips of %s (%d frames, %.1f s of CPU wall time)" % (args.cpu_clips, c["n_clips"], cfg, frames, dt)}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": "frames/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": dtype,
+        "data": "synthetic", "audio_s_per_s": value * c["hop"] / c["fs"],
+        "config": {"workload": cfg, "clips_per_gpu": B, "clip_samples": int(L), "frames_per_step_per_gpu": nums["frames"],
+                   "n_fft": c["n_fft"], "hop": c["hop"], "n_mels": c["n_mels"], "n_mfcc": c["n_mfcc"], "layout": c["layout"],
+                   "precision": args.precision, "parallelism": "dp%d (independent shards, no collective)" % world,
+                   "l2_policy": "rotating %d input/output buffer sets, %.0f MB total > 2x L2 (%.0f MB)" % (
+                       nsets, nsets * set_bytes / 1e6, l2_bytes / 1e6),
+                   "kernel": desc},
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": "frames/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(x_pin.numel() * 4),
+                "d2h_bytes_per_step": int(out_pin.numel() * 4)},
+        "gpu_launches": args.steps,
+        "roofline": roof,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    mb.melt_plan_destroy(plan)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -155,10 +155,12 @@ def hires_batch(n_clips, seed, fs, clip_len, sigma=0.01, amp=0.3):
     return out
 
 
-def make_inputs(cfg, n_clips=None):
-    """Inputs of a named config (optionally with fewer clips, same per-clip streams).
+def make_inputs(cfg, n_clips=None, seed=None):
+    """Inputs of a named config (optionally with fewer clips, same per-clip streams; optionally another seed).
     Returns dict(x=..., offsets=None|int64[n+1], x_unpadded=... for the reflect-padded configs)."""
     c = dict(CONFIGS[cfg])
+    if seed is not None:
+        c["seed"] = int(seed)
     n = c["n_clips"] if n_clips is None else int(n_clips)
     if cfg == "cfg0":
         return dict(x=single_clip(c["seed"], c["clip_len"], c["fs"])[None, :], offsets=None)
