@@ -1,0 +1,342 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on the same seeded
+inputs -- BASELINE.json's five configs at full size (the launch configuration bench.py times) plus small cases
+that span several tiles and a ragged tail.  Bars: BASELINE.json north_star (see tests/parity_util.py).
+
+Which precision mode must meet which bar:
+  compensated  P bar 1e-3 (in fact < 1e-5) AND log bar 5e-3 everywhere         -- asserted
+  tf32, bf16   single tensor-core pass: P bar asserted where the arithmetic allows it, log bar reported only
+               (operand rounding puts ~2^-11 / 2^-8 white noise in every bin; SURVEY.md section 7 hard part 1)
+"""
+import numpy as np
+import pytest
+
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+
+# compensated mode: asserted 5x below the north-star TF32 bar (1e-3); measured values are 1e-6 .. 5e-5
+COMP_P_BAR = 2e-4
+
+
+def _wl():
+    from paper_2606_01009_b200 import workloads
+    return workloads
+
+
+def _orc():
+    from oracle import melt_oracle
+    return melt_oracle
+
+
+def _check_dense(c, x, precision, n_expect_frames=None, pad=None, layout=None, p_bar=None, log_bar=pu.LOG_BAR,
+                 chunk=32):
+    """Runs log and power outputs on the GPU for the whole batch, the oracle clip-chunk by clip-chunk."""
+    orc = _orc()
+    L_gpu = pu.gpu_dense(c, x, precision, layout=layout, pad=pad)
+    P_gpu = pu.gpu_dense(c, x, precision, layout=layout, pad=pad, output="power", n_mfcc=0) if c["n_mfcc"] == 0 else None
+    assert np.isfinite(L_gpu).all()
+    if n_expect_frames is not None:
+        assert L_gpu.shape[1] == n_expect_frames
+    perr = lerr = 0.0
+    for b0 in range(0, x.shape[0], chunk):
+        ref = orc.forward_batch(x[b0:b0 + chunk], want=("P", "L"), **pu.oracle_kwargs(c, pad=pad))
+        assert ref["L"].shape == L_gpu[b0:b0 + chunk].shape
+        lerr = max(lerr, pu.log_error(L_gpu[b0:b0 + chunk], ref["L"], ref["P"]))
+        if P_gpu is not None:
+            perr = max(perr, pu.power_error(P_gpu[b0:b0 + chunk], ref["P"]))
+    print("\n[parity] %s prec=%s frames=%d  max|dP|/Pmax=%.3e  max|dlog10|(masked)=%.3e" % (
+        c.get("name", "?"), precision, L_gpu.shape[0] * L_gpu.shape[1], perr, lerr))
+    if p_bar is not None:
+        assert perr <= p_bar
+    if log_bar is not None:
+        assert lerr <= log_bar
+    return perr, lerr
+
+
+def _cfg(name):
+    c = dict(_wl().CONFIGS[name])
+    c["name"] = name
+    return c
+
+
+# ------------------------------------------------------------------------------------------- configs[0]
+@pytest.mark.parametrize("precision", ["compensated", "tf32", "bf16"])
+def test_cfg0_single_clip(precision):
+    c = _cfg("cfg0")
+    x = _wl().make_inputs("cfg0")["x"]
+    comp = precision == "compensated"
+    _check_dense(c, x, precision, n_expect_frames=98, p_bar=COMP_P_BAR if comp else pu.P_BAR[precision],
+                 log_bar=pu.LOG_BAR if comp else None)
+
+
+# ------------------------------------------------------------------------------------------- configs[1]
+@pytest.mark.parametrize("layout", ["feature_major", "frame_major"])
+def test_cfg1_three_clips_both_layouts(layout):
+    c = _cfg("cfg1")
+    x = _wl().make_inputs("cfg1", 3)["x"]
+    _check_dense(c, x, "compensated", n_expect_frames=3000, layout=layout, p_bar=COMP_P_BAR)
+
+
+def test_cfg1_library_side_reflect_padding_equals_prepadded():
+    """DESIGN.md reading R4: PAD_REFLECT on the raw [B, 480000] clip == framing the harness-padded [B, 480400] clip."""
+    c = _cfg("cfg1")
+    d = _wl().make_inputs("cfg1", 2)
+    a = pu.gpu_dense(c, d["x"], "compensated")
+    b = pu.gpu_dense(c, d["x_unpadded"], "compensated", pad=True)
+    assert a.shape == b.shape == (2, 3000, 80)
+    np.testing.assert_allclose(a, b, atol=2e-4)       # same samples, different loader path / tile alignment
+    _check_dense(c, d["x_unpadded"], "compensated", n_expect_frames=3000, pad=True, p_bar=COMP_P_BAR)
+
+
+def test_cfg1_full_size_bench_configuration():
+    c = _cfg("cfg1")
+    x = _wl().make_inputs("cfg1")["x"]
+    assert x.shape == (32, 480400)
+    _check_dense(c, x, "compensated", n_expect_frames=3000, p_bar=COMP_P_BAR)
+
+
+@pytest.mark.parametrize("precision", ["tf32", "bf16"])
+def test_cfg1_single_pass_modes(precision):
+    c = _cfg("cfg1")
+    x = _wl().make_inputs("cfg1", 4)["x"]
+    _check_dense(c, x, precision, p_bar=pu.P_BAR[precision] if precision == "bf16" else None, log_bar=None)
+
+
+# ------------------------------------------------------------------------------------------- configs[2]
+@pytest.mark.parametrize("precision", ["compensated", "tf32", "bf16"])
+def test_cfg2_eight_clips_all_modes(precision):
+    c = _cfg("cfg2")
+    x = _wl().make_inputs("cfg2", 8)["x"]
+    comp = precision == "compensated"
+    _check_dense(c, x, precision, n_expect_frames=3000, p_bar=COMP_P_BAR if comp else (pu.P_BAR[precision] if precision == "bf16" else None),
+                 log_bar=pu.LOG_BAR if comp else None)
+
+
+def test_cfg2_full_size():
+    c = _cfg("cfg2")
+    x = _wl().make_inputs("cfg2")["x"]
+    assert x.shape == (256, 480400)
+    _check_dense(c, x, "compensated", n_expect_frames=3000, p_bar=COMP_P_BAR, chunk=16)
+
+
+# ------------------------------------------------------------------------------------------- configs[3]
+def _check_ragged(c, x, off, precision="compensated"):
+    orc = _orc()
+    C_gpu, fo, L_gpu = pu.gpu_ragged(c, x, off, precision, tap=True)
+    ref = orc.forward_ragged(x, off, want=("P", "L", "C"), **pu.oracle_kwargs(c))
+    np.testing.assert_array_equal(fo, ref["frame_offsets"])                      # integer work: bit exact
+    assert C_gpu.shape == ref["C"].shape and np.isfinite(C_gpu).all() and np.isfinite(L_gpu).all()
+    lerr = pu.log_error(L_gpu, ref["L"], ref["P"])                              # stage 1: log-Mel that feeds the DCT
+    stage2 = float(np.abs(C_gpu - orc.dct_apply(L_gpu, c["n_mfcc"])).max())     # stage 2: DCT of the GPU's own log-Mel
+    e2e = float(np.abs(C_gpu - ref["C"]).max())
+    print("\n[parity] %s ragged clips=%d frames=%d  log-Mel err=%.3e  DCT-stage err=%.3e  end-to-end |dC|=%.3e" % (
+        c["name"], len(off) - 1, C_gpu.shape[0], lerr, stage2, e2e))
+    assert lerr <= pu.LOG_BAR
+    assert stage2 <= 1e-4                                                        # DESIGN.md reading R9
+    # end to end: |dC_k| <= sum_m |D_km| * |dL_m|; below the mask floor dL is unbounded by the contract, so only report
+    return lerr, stage2, e2e
+
+
+def test_cfg3_ragged_small():
+    c = _cfg("cfg3")
+    x, off = _wl().speaker_ragged(24, c["seed"], c["fs"], c["min_len"], c["max_len"])
+    _check_ragged(c, x, off)
+
+
+def test_cfg3_ragged_full_size():
+    c = _cfg("cfg3")
+    d = _wl().make_inputs("cfg3")
+    assert len(d["offsets"]) == 1025
+    _check_ragged(c, d["x"], d["offsets"])
+
+
+def test_ragged_degenerate_clips():
+    """zero-length clips, clips shorter than one frame, exactly one frame, a tile boundary (128, 129 frames)."""
+    c = _cfg("cfg3")
+    rng = np.random.default_rng(77)
+    lens = [0, 399, 400, 559, 560, 400 + 127 * 160, 400 + 128 * 160, 0, 5000, 1, 401, 400 + 255 * 160 + 3]
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    x = rng.normal(0, 0.1, int(off[-1])).astype(np.float32)
+    _, fo, _ = pu.gpu_ragged(c, x, off, tap=True)
+    np.testing.assert_array_equal(np.diff(fo), [0, 0, 1, 1, 2, 128, 129, 0, 29, 0, 1, 256])
+    _check_ragged(c, x, off)
+
+
+def test_mfcct_dense_two_stage():
+    c = _cfg("cfg3")
+    rng = np.random.default_rng(78)
+    x = rng.normal(0, 0.1, (3, 400 + 300 * 160)).astype(np.float32)
+    orc = _orc()
+    C_gpu, L_gpu = pu.gpu_dense(c, x, "compensated", layout="frame_major", tap=True)
+    ref = orc.forward_batch(x, want=("P", "L", "C"), **pu.oracle_kwargs(c))
+    assert pu.log_error(L_gpu, ref["L"], ref["P"]) <= pu.LOG_BAR
+    for b in range(3):
+        assert np.abs(C_gpu[b] - orc.dct_apply(L_gpu[b], 13)).max() <= 1e-4
+
+
+# ------------------------------------------------------------------------------------------- configs[4]
+@pytest.mark.parametrize("name", ["cfg4a", "cfg4b", "cfg4c", "cfg4d"])
+def test_cfg4_full_size(name):
+    c = _cfg(name)
+    x = _wl().make_inputs(name)["x"]
+    assert x.shape[0] == 64
+    _check_dense(c, x, "compensated", n_expect_frames={"cfg4a": 858, "cfg4b": 427, "cfg4c": 858, "cfg4d": 427}[name],
+                 p_bar=COMP_P_BAR, chunk=16)
+
+
+@pytest.mark.parametrize("precision", ["tf32", "bf16"])
+def test_cfg4a_single_pass_modes(precision):
+    c = _cfg("cfg4a")
+    x = _wl().make_inputs("cfg4a", 4)["x"]
+    _check_dense(c, x, precision, p_bar=None, log_bar=None)
+
+
+# ------------------------------------------------------------------------------------------- shapes the fast paths do not cover
+@pytest.mark.parametrize("n_fft,hop,n_mels,window", [
+    (400, 160, 80, 1),      # symmetric Hann
+    (400, 160, 80, 2),      # rectangular
+    (401, 160, 23, 0),      # odd frame length, Mel count not a multiple of 16
+    (37, 7, 5, 1),          # tiny odd everything, hop not a multiple of 4
+    (64, 16, 1, 0),         # one analysis frequency
+    (512, 128, 200, 0),     # more than 128 Mel bins -> two passes over the bins
+    (1200, 160, 128, 0),    # the paper's cepstral framing: n_fft = 7.5 hops
+])
+def test_odd_geometries(n_fft, hop, n_mels, window):
+    rng = np.random.default_rng(n_fft + hop + n_mels)
+    fs = 16000.0
+    c = dict(name="odd(%d,%d,%d,w%d)" % (n_fft, hop, n_mels, window), fs=fs, n_fft=n_fft, hop=hop, window=window,
+             n_mels=n_mels, fmin=30.0, fmax=7900.0, n_mfcc=0, layout="frame_major")
+    L = n_fft + 300 * hop + 3
+    t = np.arange(L) / fs
+    x = np.stack([(0.3 * np.sin(2 * np.pi * rng.uniform(100, 7000) * t + rng.uniform(0, 6)) + rng.normal(0, 0.01, L))
+                  for _ in range(2)]).astype(np.float32)
+    _check_dense(c, x, "compensated", n_expect_frames=301, p_bar=COMP_P_BAR)
+
+
+def test_unaligned_input_pointer_and_length():
+    """x only 4-byte aligned, len not a multiple of 4: the generic loader path must give the same numbers."""
+    import torch
+    from paper_2606_01009_b200 import binding as mb
+    c = _cfg("cfg0")
+    rng = np.random.default_rng(5)
+    L = 16000 + 2
+    xh = rng.normal(0, 0.1, (3, L)).astype(np.float32)
+    plan = pu.plan_for(c)
+    try:
+        buf = torch.zeros(3 * L + 8, device="cuda")
+        T = mb.melt_num_frames(plan, L)
+        outs = []
+        for shift in (0, 1, 3):
+            xd = buf[shift:shift + 3 * L]
+            xd.copy_(torch.from_numpy(xh.reshape(-1)))
+            out = torch.empty((3, T, 80), device="cuda")
+            mb.melt_forward(plan, xd, 3, L, out, torch.cuda.current_stream().cuda_stream)
+            torch.cuda.synchronize()
+            outs.append(out.cpu().numpy().astype(np.float64))
+    finally:
+        mb.melt_plan_destroy(plan)
+    ref = _orc().forward_batch(xh, want=("P", "L"), **pu.oracle_kwargs(c))
+    for o in outs:
+        assert pu.log_error(o, ref["L"], ref["P"]) <= pu.LOG_BAR
+
+
+def test_all_zero_input_hits_the_clamp_exactly():
+    c = _cfg("cfg1")
+    x = np.zeros((2, 480400), np.float32)
+    out = pu.gpu_dense(c, x, "compensated")
+    assert out.shape == (2, 3000, 80) and np.all(out == -10.0)
+    c3 = _cfg("cfg3")
+    Cg = pu.gpu_dense(c3, np.zeros((1, 8000), np.float32), "compensated", layout="frame_major")
+    np.testing.assert_allclose(Cg[..., 0], -10.0 * np.sqrt(40.0), rtol=1e-6)
+    np.testing.assert_allclose(Cg[..., 1:], 0.0, atol=2e-5)
+
+
+def test_silent_spans_give_minus_ten():
+    """DESIGN.md reading R11: spans set to exactly 0.0 -> P = 0 -> exactly -10 on both sides."""
+    c = _cfg("cfg1")
+    d = _wl().make_inputs("cfg1", 6)
+    out = pu.gpu_dense(c, d["x"], "compensated")
+    ref = _orc().forward_batch(d["x"], want=("L",), **pu.oracle_kwargs(c))["L"]
+    silent = ref == -10.0
+    assert silent.any()
+    assert np.all(out[silent] == -10.0)
+
+
+def test_scale_invariance_of_the_compensated_split():
+    """Quiet and loud inputs: the fp16 split is scaled internally, so relative accuracy must not depend on level
+    (|x| < 8 is the documented range of the default input scale)."""
+    c = _cfg("cfg0")
+    x = _wl().make_inputs("cfg0")["x"]
+    for g in (1e-3, 1.0, 6.0):
+        _check_dense(c, (x * g).astype(np.float32), "compensated", p_bar=COMP_P_BAR)
+
+
+# ------------------------------------------------------------------------------------------- boundary behaviour
+def test_empty_and_too_short_inputs_are_successful_noops():
+    import torch
+    from paper_2606_01009_b200 import binding as mb
+    c = _cfg("cfg0")
+    plan = pu.plan_for(c)
+    try:
+        x = torch.zeros(1000, device="cuda")
+        out = torch.full((10,), 7.0, device="cuda")
+        mb.melt_forward(plan, x, 0, 1000, out)            # batch 0
+        mb.melt_forward(plan, x, 2, 399, out)             # len < n_fft -> T = 0
+        torch.cuda.synchronize()
+        assert mb.melt_num_frames(plan, 399) == 0 and mb.melt_num_frames(plan, 400) == 1
+        assert torch.all(out == 7.0)
+    finally:
+        mb.melt_plan_destroy(plan)
+
+
+def test_argument_validation():
+    import torch
+    from paper_2606_01009_b200 import binding as mb
+    with pytest.raises(mb.MeltError):
+        mb.melt_plan_create(16000.0, 400, 160, 0, 80, 0.0, 9000.0)          # fmax > fs/2
+    with pytest.raises(mb.MeltError):
+        mb.melt_plan_create(16000.0, 1, 160, 0, 80, 0.0, 8000.0)            # n_fft < 2
+    with pytest.raises(mb.MeltError):
+        mb.melt_plan_create(16000.0, 400, 160, 0, 80, 0.0, 8000.0, mb.MELT_MEL_SLANEY)   # not defined by the paper
+    with pytest.raises(mb.MeltError):
+        mb.melt_plan_create(16000.0, 400, 160, 0, 40, 20.0, 7600.0, 0, 41)  # n_mfcc > n_mels
+    plan = mb.melt_plan_create(16000.0, 400, 160, 0, 80, 0.0, 8000.0)
+    try:
+        x = torch.zeros(16000, device="cuda")
+        out = torch.zeros(98 * 80, device="cuda")
+        with pytest.raises(mb.MeltError) as ei:
+            mb.melt_forward(plan, None, 1, 16000, out)
+        assert ei.value.status == mb.MELT_ERR_INVALID_ARG
+        with pytest.raises(mb.MeltError) as ei:
+            mb.melt_forward(plan, x.data_ptr() + 2, 1, 15000, out)
+        assert ei.value.status == mb.MELT_ERR_ALIGNMENT
+        with pytest.raises(mb.MeltError):
+            mb.melt_forward(plan, x, -1, 16000, out)
+        mb.melt_forward(plan, x, 1, 16000, out)
+        torch.cuda.synchronize()
+        with pytest.raises(mb.MeltError):                                    # immutable after the first forward
+            mb.melt_plan_set_option(plan, mb.MELT_OPT_LAYOUT, 1)
+        f = mb.melt_plan_get_centres(plan, 80)
+        np.testing.assert_allclose(f, _orc().centres(0.0, 8000.0, 80), rtol=1e-12)
+    finally:
+        mb.melt_plan_destroy(plan)
+
+
+def test_forward_is_asynchronous_on_the_given_stream():
+    import torch
+    from paper_2606_01009_b200 import binding as mb
+    c = _cfg("cfg1")
+    x_host = _wl().make_inputs("cfg1", 2)["x"]
+    plan = pu.plan_for(c)
+    try:
+        s = torch.cuda.Stream()
+        x = torch.from_numpy(x_host).cuda()
+        outs = [torch.empty((2, 80, 3000), device="cuda") for _ in range(2)]
+        torch.cuda.synchronize()
+        with torch.cuda.stream(s):
+            mb.melt_forward(plan, x, 2, x.shape[1], outs[0], s.cuda_stream)
+            mb.melt_forward(plan, x, 2, x.shape[1], outs[1], s.cuda_stream)
+        s.synchronize()
+        assert torch.equal(outs[0], outs[1])                                  # deterministic
+    finally:
+        mb.melt_plan_destroy(plan)
