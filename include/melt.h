@@ -165,6 +165,14 @@ const char *melt_plan_describe(const melt_plan *plan);
  */
 int melt_selftest_umma(int kind, int n, int k, const float *a, const float *b, float *d);
 
+/*
+ * Self-test of the CTA-pair form of the same building block (tcgen05.mma.cta_group::2 on a cluster of two CTAs):
+ * D[256, n] = A[256, k] . B[n, k]^T, CTA r of the pair holding rows [128 r, 128 r + 128) of A in its tensor memory
+ * and rows [r n/2, (r+1) n/2) of B in its shared memory.  a host fp32 [256, k]; b host fp32 [n, k]; d host fp32
+ * [256, n].  n % 16 == 0, 32 <= n <= 256; k as for melt_selftest_umma.  Synchronous.  Returns a melt_status.
+ */
+int melt_selftest_umma2(int kind, int n, int k, const float *a, const float *b, float *d);
+
 #ifdef __cplusplus
 }
 #endif

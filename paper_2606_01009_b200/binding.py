@@ -23,7 +23,7 @@ MELT_OUTPUT_LOG, MELT_OUTPUT_POWER = 0, 1
 SYMBOLS = [
     "melt_plan_create", "melt_plan_destroy", "melt_plan_set_option", "melt_num_frames", "melt_num_channels",
     "melt_plan_get_centres", "melt_forward", "melt_forward_ragged", "melt_forward_tap", "melt_last_error",
-    "melt_plan_describe", "melt_selftest_umma",
+    "melt_plan_describe", "melt_selftest_umma", "melt_selftest_umma2",
 ]
 
 _lib = None
@@ -65,6 +65,7 @@ def lib():
     L.melt_plan_describe.restype = C.c_char_p
     L.melt_plan_describe.argtypes = [vp]
     L.melt_selftest_umma.argtypes = [ip, ip, ip, vp, vp, vp]
+    L.melt_selftest_umma2.argtypes = [ip, ip, ip, vp, vp, vp]
     _lib = L
     return L
 
@@ -143,4 +144,16 @@ def melt_selftest_umma(kind, a, b):
     assert a.shape == (128, k)
     d = np.empty((128, n), np.float32)
     _check(lib().melt_selftest_umma(int(kind), n, k, a.ctypes.data, b.ctypes.data, d.ctypes.data))
+    return d
+
+
+def melt_selftest_umma2(kind, a, b):
+    """CTA-pair form: a [256, k], b [n, k] numpy float32 (host) -> d [256, n] numpy float32."""
+    import numpy as np
+    a = np.ascontiguousarray(a, np.float32)
+    b = np.ascontiguousarray(b, np.float32)
+    n, k = b.shape
+    assert a.shape == (256, k)
+    d = np.empty((256, n), np.float32)
+    _check(lib().melt_selftest_umma2(int(kind), n, k, a.ctypes.data, b.ctypes.data, d.ctypes.data))
     return d

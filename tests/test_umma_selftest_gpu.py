@@ -41,3 +41,18 @@ def test_umma_ts_random_fp16():
     d = mb.melt_selftest_umma(0, a, b)
     ref = _round(a, 0) @ _round(b, 0).T
     np.testing.assert_allclose(d, ref, rtol=0, atol=2e-5 * np.abs(ref).max())
+
+
+@pytest.mark.parametrize("kind", [0, 1, 2])
+@pytest.mark.parametrize("n,k", [(32, 16), (80, 48), (128, 208), (256, 64), (48, 256)])
+def test_umma2_cta_pair_matches_float64(kind, n, k):
+    """tcgen05.mma.cta_group::2: 256 rows over a CTA pair, B split by rows between the two CTAs' shared memories."""
+    from paper_2606_01009_b200 import binding as mb
+    rng = np.random.default_rng(1000 + 100 * kind + n + k)
+    if kind == 2:
+        k = max(8, k // 2)
+    a = rng.integers(-32, 33, (256, k)).astype(np.float32) / 16.0
+    b = rng.integers(-32, 33, (n, k)).astype(np.float32) / 16.0
+    d = mb.melt_selftest_umma2(kind, a, b)
+    ref = _round(a, kind) @ _round(b, kind).T
+    np.testing.assert_array_equal(d.astype(np.float64), ref)
