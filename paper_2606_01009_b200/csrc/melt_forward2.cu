@@ -1,0 +1,525 @@
+// melt_forward2.cu -- the hot path (steps S1-S6 of SURVEY.md 8(a)) as ONE persistent, warp-specialised kernel on CTA
+// PAIRS (thread-block clusters of two SMs, tcgen05.mma.cta_group::2).  A tile is 256 consecutive frames of one clip:
+// CTA r of the pair owns frames [128 r, 128 r + 128) of it (its 128 tensor-memory lanes).
+//
+//   loader warp       raw fp32 signal (global) -> shared-memory staging ring with the bulk-copy engine (cp.async.bulk), one
+//                     copy per hop-row (`hop` samples) at a padded pitch, in chunks of 32 frames (= one tensor-memory
+//                     lane quarter).  Implicit im2col: a sample is fetched from HBM/L2 once per chunk and the 2.5x frame
+//                     overlap is served from shared memory; nothing is staged through registers.
+//   converter warps   thread = frame.  128-bit conflict-free shared loads (row pitch = 4 * odd words), fold of the frame
+//                     about the window centre (x[c+j] +- x[c-j]), split into tensor-core operands (fp16 hi + lo, or
+//                     bf16, or tf32) and ONE tcgen05.st per K-step straight into TENSOR MEMORY: the A operand never
+//                     exists in shared or global memory.
+//   basis             each CTA keeps HALF of the folded cos/sin basis (nb/2 Mel rows per operand kind) resident in shared
+//                     memory; the pair's tensor cores read both halves (cta_group::2), which halves the per-SM shared
+//                     bandwidth and footprint of the B operand and leaves room for a deep staging ring.
+//   MMA issuer        one thread of the leader CTA: tcgen05.mma.cta_group::2 kind::f16 / kind::tf32, M = 256 over the
+//                     pair, A from tensor memory, B from shared memory, fp32 accumulators in tensor memory
+//                     (R in columns [0, nb), I in [nb, 2 nb)), double-buffered when they fit.
+//   epilogue warps    tcgen05.ld -> R^2 + I^2 -> log10(max(., 1e-10)) -> optional DCT-II (fp32 FMA) -> coalesced stores.
+//
+// Hand-offs are mbarriers; cross-CTA ones are remote arrivals (mapa) and multicast tcgen05.commit.
+#include "melt_plan.h"
+#include "sm100_ptx.cuh"
+
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include <algorithm>
+
+namespace melt {
+
+enum { P2_COMP = 0, P2_TF32 = 1, P2_BF16 = 2 };
+// barrier indices (8 bytes each)
+enum {
+    V_STG_FULL = 0, V_STG_EMPTY = V2_MAX_STG, V_A_FULL = 2 * V2_MAX_STG, V_A_EMPTY = V_A_FULL + 16, V_ACC_FULL = V_A_EMPTY + 16,
+    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + 1, V_NBARS = V_B_PEER + 1
+};
+constexpr int V2_MAX_A_SLOTS = 16;
+constexpr int W_LOAD = 0, W_MMA = 1, W_BASIS = 2, W_EPI0 = 4, W_CONV0 = 8;
+
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float lds32(uint32_t addr) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+template <int KQ>
+__device__ __forceinline__ void dct_acc2(float (&cacc)[MAX_MFCC], const float *drow, float v) {
+#pragma unroll
+    for (int q = 0; q < KQ; ++q) {
+        const float4 d = *reinterpret_cast<const float4 *>(drow + 4 * q);
+        cacc[4 * q + 0] = fmaf(d.x, v, cacc[4 * q + 0]);
+        cacc[4 * q + 1] = fmaf(d.y, v, cacc[4 * q + 1]);
+        cacc[4 * q + 2] = fmaf(d.z, v, cacc[4 * q + 2]);
+        cacc[4 * q + 3] = fmaf(d.w, v, cacc[4 * q + 3]);
+    }
+}
+
+template <int PREC, int SIGMA>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    constexpr int KS = (PREC == P2_TF32) ? 8 : 16;  // folded pairs per K-step
+    constexpr int NQ = KS / 4;                      // 128-bit loads per direction per K-step
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t bar0 = sbase + p.off_bar;
+    auto BAR = [&](int idx) -> uint32_t { return bar0 + (uint32_t)idx * 8u; };
+    uint32_t *tmem_ptr_s = reinterpret_cast<uint32_t *>(smem + p.off_bar + V_NBARS * 8);
+    float *dct_s = reinterpret_cast<float *>(smem + p.off_dct);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t rank = cluster_ctarank();
+    const int S = p.stg_slots;
+
+    // ------------------------------------------------------------------ one-time setup
+    if (tid == 0) {
+        for (int i = 0; i < V2_MAX_STG; ++i) { mbar_init(BAR(V_STG_FULL + i), 1); mbar_init(BAR(V_STG_EMPTY + i), 2); }
+        for (int i = 0; i < V2_MAX_A_SLOTS; ++i) { mbar_init(BAR(V_A_FULL + i), 8); mbar_init(BAR(V_A_EMPTY + i), 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 1); mbar_init(BAR(V_ACC_EMPTY + i), 8); }
+        mbar_init(BAR(V_B_FULL), 1);
+        mbar_init(BAR(V_B_PEER), 1);
+        fence_barrier_init();
+    }
+    if (warp == W_BASIS) {
+        tmem_alloc2(smem_u32(tmem_ptr_s), 512);
+        tmem_relinquish2();
+    }
+    {   // staging ring (and its guard bands) starts finite: stale rows are multiplied by zero basis entries or belong to
+        // frames that are never stored, but must never be NaN / Inf bit patterns
+        float4 *z = reinterpret_cast<float4 *>(smem + p.off_stg - 128);
+        const int n16 = (S * p.slot_bytes + 256) / 16;
+        for (int i = tid; i < n16; i += V2_THREADS) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    if (p.n_mfcc > 0)
+        for (int i = tid; i < p.n_mels * p.dct_pitch; i += V2_THREADS) dct_s[i] = __ldg(p.dct + i);
+    fence_proxy_async_smem();  // the zero fill (generic proxy) is ordered before the bulk copies (async proxy) that follow
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr_s;
+
+    const int first_tile = (int)cluster_id_x(), tile_step = (int)cluster_nid_x();
+    const int n_tiles = p.n_tiles;
+
+    if (warp == W_LOAD) {
+        // ============================================================== signal loader (bulk-copy engine)
+        int slot = 0;
+        uint32_t ph = 0;
+        const long long len = p.len;
+        for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+            const int b = tile / p.tiles_per_clip;
+            const int t0 = (tile - b * p.tiles_per_clip) * 256 + (int)rank * 128;
+            const float *xb = p.x + (long long)b * len;
+            for (int q = 0; q < 4; ++q) {
+                mbar_wait(BAR(V_STG_EMPTY + slot), ph ^ 1u);
+                const long long row0 = (long long)(t0 + 32 * q);
+                uint32_t bytes[2];
+                uint32_t mine = 0;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int i = lane + 32 * h;
+                    const long long start = (row0 + i) * p.hop;
+                    long long rem = len - start;
+                    rem = rem < 0 ? 0 : (rem > p.hop ? p.hop : rem);
+                    bytes[h] = (i < p.rows_per_chunk && row0 < p.frames_per_clip) ? (uint32_t)rem * 4u : 0u;
+                    mine += bytes[h];
+                }
+                const uint32_t total = __reduce_add_sync(0xffffffffu, mine);
+                if (lane == 0) {
+                    if (total) mbar_arrive_expect_tx(BAR(V_STG_FULL + slot), total);
+                    else mbar_arrive(BAR(V_STG_FULL + slot));
+                }
+                __syncwarp();
+                const uint32_t dst0 = sbase + p.off_stg + (uint32_t)slot * (uint32_t)p.slot_bytes;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const int i = lane + 32 * h;
+                    if (bytes[h])
+                        bulk_g2s(dst0 + (uint32_t)i * (uint32_t)p.pitch_bytes, xb + (row0 + i) * p.hop, bytes[h], BAR(V_STG_FULL + slot));
+                }
+                if (++slot == S) { slot = 0; ph ^= 1u; }
+            }
+        }
+    } else if (warp == W_BASIS) {
+        // ============================================================== basis: this CTA's half, resident
+        if (lane == 0 && first_tile < n_tiles) {
+            mbar_arrive_expect_tx(BAR(V_B_FULL), (uint32_t)p.units * p.unit_b_bytes);
+            const uint8_t *src = p.b_img + (size_t)rank * p.units * p.unit_b_bytes;
+            for (int u = 0; u < p.units; ++u)
+                bulk_g2s(sbase + p.off_b + (uint32_t)u * p.unit_b_bytes, src + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL));
+            if (rank == 1) {  // tell the leader that the peer half has landed
+                mbar_wait(BAR(V_B_FULL), 0);
+                mbar_arrive_cluster(mapa_cluster(BAR(V_B_PEER), 0));
+            }
+        }
+    } else if (warp == W_MMA) {
+        // ============================================================== MMA issuer (one thread of the leader CTA)
+        if (rank == 0 && lane == 0 && first_tile < n_tiles) {
+            const uint32_t idesc = umma_idesc(PREC == P2_COMP ? UMMA_F16 : (PREC == P2_BF16 ? UMMA_BF16 : UMMA_TF32), (uint32_t)p.nb, 256u);
+            mbar_wait(BAR(V_B_FULL), 0);
+            mbar_wait_cluster(BAR(V_B_PEER), 0);
+            int aslot = 0, stage = 0;
+            uint32_t aph = 0, sph = 0;
+            for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+                mbar_wait_cluster(BAR(V_ACC_EMPTY + stage), sph ^ 1u);
+                tc_fence_after();
+                const uint32_t d_r = tmem_base + (uint32_t)stage * (uint32_t)p.acc_cols, d_i = d_r + (uint32_t)p.nb;
+                for (int u = 0; u < p.units; ++u) {
+                    mbar_wait_cluster(BAR(V_A_FULL + aslot), aph);
+                    tc_fence_after();
+                    const uint32_t a = tmem_base + (uint32_t)p.a_col0 + (uint32_t)aslot * (uint32_t)p.unit_cols;
+                    const uint32_t b = sbase + p.off_b + (uint32_t)u * p.unit_b_bytes;
+                    const uint32_t acc = u > 0;
+                    if (PREC == P2_COMP) {
+                        // A kinds: s_hi @0, s_lo @8, d_hi @16, d_lo @24;  B kinds: wc_hi, wc_lo, ws_hi, ws_lo
+                        const uint64_t wc_hi = umma_smem_desc_kmajor_noswz(b, 128, 256);
+                        const uint64_t wc_lo = umma_smem_desc_kmajor_noswz(b + p.kind_bytes, 128, 256);
+                        const uint64_t ws_hi = umma_smem_desc_kmajor_noswz(b + 2 * p.kind_bytes, 128, 256);
+                        const uint64_t ws_lo = umma_smem_desc_kmajor_noswz(b + 3 * p.kind_bytes, 128, 256);
+                        umma2_ts_f16(d_r, a + 0, wc_hi, idesc, acc);
+                        umma2_ts_f16(d_i, a + 16, ws_hi, idesc, acc);
+                        umma2_ts_f16(d_r, a + 8, wc_hi, idesc, 1);
+                        umma2_ts_f16(d_i, a + 24, ws_hi, idesc, 1);
+                        umma2_ts_f16(d_r, a + 0, wc_lo, idesc, 1);
+                        umma2_ts_f16(d_i, a + 16, ws_lo, idesc, 1);
+                    } else {
+                        const uint64_t wc = umma_smem_desc_kmajor_noswz(b, 128, 256);
+                        const uint64_t ws = umma_smem_desc_kmajor_noswz(b + p.kind_bytes, 128, 256);
+                        if (PREC == P2_TF32) { umma2_ts_tf32(d_r, a + 0, wc, idesc, acc); umma2_ts_tf32(d_i, a + 8, ws, idesc, acc); }
+                        else { umma2_ts_f16(d_r, a + 0, wc, idesc, acc); umma2_ts_f16(d_i, a + 8, ws, idesc, acc); }
+                    }
+                    tc_commit2(BAR(V_A_EMPTY + aslot), 3);
+                    if (++aslot == p.a_slots) { aslot = 0; aph ^= 1u; }
+                }
+                tc_commit2(BAR(V_ACC_FULL + stage), 3);
+                if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
+            }
+        }
+    } else if (warp >= W_EPI0 && warp < W_EPI0 + 4) {
+        // ============================================================== epilogue (thread = frame)
+        const int q = warp & 3;
+        const int row = q * 32 + lane;
+        const uint32_t lane_taddr = tmem_base + ((uint32_t)(q * 32) << 16);
+        const uint32_t acc_empty_remote = mapa_cluster(BAR(V_ACC_EMPTY), 0);
+        const float kLog10_2 = 0.30102999566398120f;
+        int stage = 0;
+        uint32_t sph = 0;
+        const long long T = p.frames_per_clip;
+        for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+            const int b = tile / p.tiles_per_clip;
+            const int t0 = (tile - b * p.tiles_per_clip) * 256 + (int)rank * 128;
+            const bool valid = (long long)(t0 + row) < T;
+            float cacc[MAX_MFCC];
+            if (p.n_mfcc > 0) {
+#pragma unroll
+                for (int k = 0; k < MAX_MFCC; ++k) cacc[k] = 0.f;
+            }
+            float *optr, *tptr;
+            long long cstride;
+            if (p.feature_major) {
+                optr = p.out + ((long long)b * p.n_ch) * T + t0 + row;
+                tptr = p.tap ? p.tap + ((long long)b * p.n_mels) * T + t0 + row : nullptr;
+                cstride = T;
+            } else {
+                optr = p.out + ((long long)b * T + t0 + row) * p.n_ch;
+                tptr = p.tap ? p.tap + ((long long)b * T + t0 + row) * p.n_mels : nullptr;
+                cstride = 1;
+            }
+            mbar_wait(BAR(V_ACC_FULL + stage), sph);
+            tc_fence_after();
+            const uint32_t t_r = lane_taddr + (uint32_t)stage * (uint32_t)p.acc_cols, t_i = t_r + (uint32_t)p.nb;
+            for (int c0 = 0; c0 < p.nb; c0 += 16) {
+                uint32_t vr[16], vi[16];
+                tmem_ld16(t_r + (uint32_t)c0, vr);
+                tmem_ld16(t_i + (uint32_t)c0, vi);
+                tmem_wait_ld();
+#pragma unroll
+                for (int c = 0; c < 16; ++c) {
+                    const int m = c0 + c;
+                    if (m < p.n_mels) {
+                        const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                        const float praw = fmaf(r, r, im * im);                                          // Eq. (4)
+                        float v;
+                        if (p.output_power) v = praw * p.out_scale;
+                        else v = fmaxf(fmaf(__log2f(praw), kLog10_2, p.out_log10_offset), -10.f);       // Eq. (8), contract form
+                        if (p.n_mfcc > 0) {
+                            const float *drow = dct_s + m * p.dct_pitch;
+                            if (p.dct_pitch <= 16) dct_acc2<4>(cacc, drow, v);
+                            else if (p.dct_pitch <= 40) dct_acc2<10>(cacc, drow, v);
+                            else dct_acc2<16>(cacc, drow, v);
+                            if (tptr && valid) tptr[m * cstride] = v;
+                        } else if (valid) {
+                            optr[m * cstride] = v;
+                        }
+                    }
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(acc_empty_remote + (uint32_t)stage * 8u);
+            if (p.n_mfcc > 0 && valid) {                                                                  // Eq. (9)
+#pragma unroll
+                for (int k = 0; k < MAX_MFCC; ++k)
+                    if (k < p.n_mfcc) optr[k * cstride] = cacc[k];
+            }
+            if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
+        }
+    } else if (warp >= W_CONV0) {
+        // ============================================================== converters (thread = frame; two groups alternate K-steps)
+        const int q = warp & 3, g = (warp - W_CONV0) >> 2;
+        const uint32_t lane_taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)p.a_col0;
+        const uint32_t a_full_remote = mapa_cluster(BAR(V_A_FULL), 0);
+        const uint32_t row_off = sbase + p.off_stg + (uint32_t)lane * (uint32_t)p.pitch_bytes;
+        const float S_in = p.in_scale;
+        int sslot = q;
+        uint32_t sph = 0;
+        int aslot = g % p.a_slots;               // ring position of unit counter ug = it * units + u, first u = g
+        uint32_t aph = (uint32_t)((g / p.a_slots) & 1);
+        for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+            mbar_wait(BAR(V_STG_FULL + sslot), sph);
+            const uint32_t fb = row_off + (uint32_t)sslot * (uint32_t)p.slot_bytes;
+            int u = g;
+            while (u < p.units) {
+                // ---- loads: NQ forward quads, NQ mirrored quads (+ one single when the mirrored run starts at 1 mod 4)
+                const short *tb = p.tab[u];
+                float fw[KS], bw[KS];
+#pragma unroll
+                for (int i = 0; i < NQ; ++i) {
+                    const float4 f = lds128(fb + (uint32_t)(int)tb[i]);
+                    fw[4 * i + 0] = f.x; fw[4 * i + 1] = f.y; fw[4 * i + 2] = f.z; fw[4 * i + 3] = f.w;
+                }
+                // mirrored partner of pair e is the sample at position KS-1-e of the descending run
+                if (SIGMA == 0) {
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i) {
+                        const float4 f = lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs+4i .. rs+4i+3
+                        bw[KS - 1 - (4 * i + 0)] = f.x; bw[KS - 1 - (4 * i + 1)] = f.y;
+                        bw[KS - 1 - (4 * i + 2)] = f.z; bw[KS - 1 - (4 * i + 3)] = f.w;
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i) {
+                        const float4 f = lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs-1+4i .. rs+2+4i
+                        if (i > 0) bw[KS - 1 - (4 * i - 1)] = f.x;                  // position 4i-1 of the run
+                        bw[KS - 1 - (4 * i + 0)] = f.y; bw[KS - 1 - (4 * i + 1)] = f.z; bw[KS - 1 - (4 * i + 2)] = f.w;
+                    }
+                    bw[0] = lds32(fb + (uint32_t)(int)tb[8]);                       // position KS-1 of the run
+                }
+                mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);
+                tc_fence_after();
+                const uint32_t dst = lane_taddr + (uint32_t)aslot * (uint32_t)p.unit_cols;
+                if (PREC == P2_COMP) {
+                    uint32_t v[32];
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        const float b0 = bw[2 * c] * S_in, b1 = bw[2 * c + 1] * S_in;
+                        const float s0 = fmaf(fw[2 * c], S_in, b0), s1 = fmaf(fw[2 * c + 1], S_in, b1);
+                        const float d0 = fmaf(fw[2 * c], S_in, -b0), d1 = fmaf(fw[2 * c + 1], S_in, -b1);
+                        const __half2 sh = __floats2half2_rn(s0, s1), dh = __floats2half2_rn(d0, d1);
+                        const float2 shf = __half22float2(sh), dhf = __half22float2(dh);
+                        const __half2 sl = __floats2half2_rn(s0 - shf.x, s1 - shf.y);
+                        const __half2 dl = __floats2half2_rn(d0 - dhf.x, d1 - dhf.y);
+                        v[c] = *reinterpret_cast<const uint32_t *>(&sh);
+                        v[8 + c] = *reinterpret_cast<const uint32_t *>(&sl);
+                        v[16 + c] = *reinterpret_cast<const uint32_t *>(&dh);
+                        v[24 + c] = *reinterpret_cast<const uint32_t *>(&dl);
+                    }
+                    tmem_st32(dst, v);
+                } else if (PREC == P2_BF16) {
+                    uint32_t v[16];
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        const __nv_bfloat162 sh = __floats2bfloat162_rn(fw[2 * c] + bw[2 * c], fw[2 * c + 1] + bw[2 * c + 1]);
+                        const __nv_bfloat162 dh = __floats2bfloat162_rn(fw[2 * c] - bw[2 * c], fw[2 * c + 1] - bw[2 * c + 1]);
+                        v[c] = *reinterpret_cast<const uint32_t *>(&sh);
+                        v[8 + c] = *reinterpret_cast<const uint32_t *>(&dh);
+                    }
+                    tmem_st16(dst, v);
+                } else {
+                    uint32_t v[16];
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        v[c] = cvt_tf32_rna(fw[c] + bw[c]);
+                        v[8 + c] = cvt_tf32_rna(fw[c] - bw[c]);
+                    }
+                    tmem_st16(dst, v);
+                }
+                tmem_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(a_full_remote + (uint32_t)aslot * 8u);
+                // advance to this group's next unit (the next tile's first one after the last)
+                int du = 2;
+                if (u + 2 >= p.units) du = p.units - u + g;   // ug(next tile, u = g) - ug(this tile, u)
+                u += 2;
+                aslot += du;
+                while (aslot >= p.a_slots) { aslot -= p.a_slots; aph ^= 1u; }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));
+            sslot += 4;
+            if (sslot >= S) { sslot -= S; sph ^= 1u; }
+        }
+    }
+
+    // ------------------------------------------------------------------ teardown
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == W_BASIS) tmem_dealloc2(tmem_base, 512);
+}
+
+// ---------------------------------------------------------------------------------------------- host side
+static int round_up2(int v, int m) { return (v + m - 1) / m * m; }
+
+int plan_build_v2(melt_plan *p) {
+    p->v2_ok = false;
+    K2Params &k = p->k2;
+    const KParams &k1 = p->kp;
+    memset(&k, 0, sizeof(k));
+    const int N = p->n_fft, H = p->hop, M = p->n_mels;
+    const bool comp = p->precision == MELT_PREC_COMPENSATED;
+    const int kind = comp ? OP_F16 : (p->precision == MELT_PREC_BF16 ? OP_BF16 : OP_TF32);
+    k.n_fft = N; k.hop = H; k.n_mels = M; k.n_mfcc = p->n_mfcc; k.n_ch = k1.n_ch;
+    k.kstep = operand_kstep(kind);
+    k.units = (k1.kf + k.kstep - 1) / k.kstep;
+    k.nk = comp ? 4 : 2;
+    k.unit_cols = k.nk * 8;
+    k.nb = round_up2(M, 16);
+    if (k.nb < 32) k.nb = 32;
+    // ---- what the kernel covers (everything else stays on the general v1 kernel)
+    if (M > 128 || k.units > V2_MAX_UNITS || (H & 3) || (k1.a0 & 3) || p->pad != MELT_PAD_NONE) return MELT_OK;
+    const int rs = k1.b0 - (k.kstep - 1);           // lowest sample of the mirrored run of unit 0
+    const int sigma = ((rs % 4) + 4) % 4;
+    if (sigma > 1) return MELT_OK;
+    p->v2_sigma = sigma;
+    k.acc_cols = 2 * k.nb;
+    k.acc_stages = (2 * k.acc_cols + 4 * k.unit_cols <= 512) ? 2 : 1;
+    k.a_col0 = k.acc_stages * k.acc_cols;
+    k.a_slots = std::min(V2_MAX_A_SLOTS, (512 - k.a_col0) / k.unit_cols);
+    if (k.a_slots < 2) return MELT_OK;
+    k.rows_per_chunk = 32 + (N - 1) / H;
+    if (k.rows_per_chunk > 64) return MELT_OK;
+    const int pitch_words = ((H / 4) & 1) ? H : H + 4;   // pitch / 4 odd: 8 consecutive rows hit 8 distinct 16-byte bank groups
+    k.pitch_bytes = pitch_words * 4;
+    k.slot_bytes = k.rows_per_chunk * k.pitch_bytes;
+    k.kind_bytes = (uint32_t)(k.nb / 2) * 32u;
+    k.unit_b_bytes = (uint32_t)k.nk * k.kind_bytes;
+    k.dct_pitch = k1.dct_pitch;
+    const uint32_t b_bytes = (uint32_t)k.units * k.unit_b_bytes;
+    const uint32_t dct_bytes = p->n_mfcc > 0 ? (uint32_t)(M * k.dct_pitch * 4) : 0;
+    const uint32_t bar_bytes = (uint32_t)round_up2(V_NBARS * 8 + 16, 128);
+    k.off_b = 0;
+    k.off_stg = (uint32_t)round_up2((int)b_bytes, 128) + 128;  // 128-byte zero guard in front of the ring
+    const long long room = (long long)SMEM_BUDGET - k.off_stg - 128 - dct_bytes - bar_bytes - 256;
+    k.stg_slots = (int)std::min<long long>(room / k.slot_bytes, V2_MAX_STG);
+    if (k.stg_slots < 5) return MELT_OK;
+    k.off_dct = (uint32_t)round_up2((int)(k.off_stg + (uint32_t)k.stg_slots * k.slot_bytes + 128), 128);
+    k.off_bar = (uint32_t)round_up2((int)(k.off_dct + dct_bytes), 128);
+    k.smem_bytes = k.off_bar + bar_bytes;
+    if (k.smem_bytes > (uint32_t)SMEM_BUDGET) return MELT_OK;
+    k.in_scale = k1.in_scale; k.out_scale = k1.out_scale; k.out_log10_offset = k1.out_log10_offset;
+    k.output_power = k1.output_power; k.feature_major = k1.feature_major;
+
+    // ---- per-unit load table: byte offset of sample n of a frame = ((n div H) * pitch + n mod H) * 4 (floor division)
+    auto off_of = [&](int n) -> int {
+        int row = n >= 0 ? n / H : -((-n + H - 1) / H);
+        return (row * pitch_words + (n - row * H)) * 4;
+    };
+    for (int u = 0; u < k.units; ++u) {
+        const int nq = k.kstep / 4;
+        for (int i = 0; i < nq; ++i) k.tab[u][i] = (short)off_of(k1.a0 + k.kstep * u + 4 * i);
+        const int run = k1.b0 - k.kstep * u - (k.kstep - 1);   // lowest sample of the mirrored run
+        for (int i = 0; i < nq; ++i) k.tab[u][4 + i] = (short)off_of(run - sigma + 4 * i);
+        k.tab[u][8] = (short)off_of(run + k.kstep - 1);
+        for (int i = 0; i < V2_TAB; ++i)
+            if (k.tab[u][i] < -128 || k.tab[u][i] + 16 > k.slot_bytes + 128) return MELT_OK;   // stays inside ring + guards
+    }
+
+    // ---- basis image: [rank][unit][kind][nb/2 rows] slabs (same folded coefficients as v1, split by Mel row)
+    const double kPi = 3.14159265358979323846264338327950288;
+    const int c2 = (p->window == MELT_WINDOW_HANN_PERIODIC) ? N : N - 1;
+    const double centre = 0.5 * (double)c2;
+    const int s_b = comp ? 14 : 0;
+    const double bscale = std::ldexp(1.0, s_b);
+    auto coef = [&](int m, int j, bool sine) -> double {
+        if (m >= M || j >= k1.kf) return 0.0;
+        const int na = k1.a0 + j;
+        const double gsc = (na == k1.b0 - j) ? 0.5 : 1.0;
+        const double arg = 2.0 * kPi * p->centres[m] * ((double)na - centre) / p->fs;
+        return bscale * p->win[na] * (sine ? std::sin(arg) : gsc * std::cos(arg));
+    };
+    auto hi_of = [&](double v) -> double {
+        if (kind == OP_F16) return f16_bits_to_f64(f64_to_f16_bits(v));
+        if (kind == OP_BF16) return bf16_bits_to_f64(f64_to_bf16_bits(v));
+        return tf32_bits_to_f64(f64_to_tf32_bits(v));
+    };
+    const size_t img_bytes = (size_t)2 * b_bytes;
+    std::vector<uint8_t> img(img_bytes, 0);
+    const int nh = k.nb / 2;
+    for (int r = 0; r < 2; ++r)
+        for (int u = 0; u < k.units; ++u) {
+            uint8_t *slab = img.data() + ((size_t)r * k.units + u) * k.unit_b_bytes;
+            for (int kk = 0; kk < k.nk; ++kk) {
+                const bool sine = comp ? (kk >= 2) : (kk == 1);
+                const bool lo = comp && (kk & 1);
+                pack_b_slab(kind, nh, [&](int row, int kq) {
+                    double v = coef(r * nh + row, u * k.kstep + kq, sine);
+                    return lo ? v - hi_of(v) : v;
+                }, slab + (size_t)kk * k.kind_bytes);
+            }
+        }
+    cudaFree(p->d_bimg2);
+    p->d_bimg2 = nullptr;
+    MELT_CUDA(cudaMalloc(&p->d_bimg2, img_bytes));
+    MELT_CUDA(cudaMemcpy(p->d_bimg2, img.data(), img_bytes, cudaMemcpyHostToDevice));
+    k.b_img = p->d_bimg2;
+    k.dct = p->d_dct;
+    p->v2_ok = true;
+    char buf[512];
+    snprintf(buf, sizeof(buf),
+             "melt_b200 v2 (CTA pair, 256-frame tiles) prec=%s fold(a0=%d,b0=%d,kf=%d) kstep=%d units=%d nb=%d tmem(acc=%dx%d,"
+             "a_slots=%d) basis=resident half (%u B/CTA) staging=%d x %d B chunks of 32 frames (pitch %d B) smem=%u B",
+             comp ? "fp16x3" : (kind == OP_BF16 ? "bf16" : "tf32"), k1.a0, k1.b0, k1.kf, k.kstep, k.units, k.nb, k.acc_stages,
+             k.acc_cols, k.a_slots, b_bytes, k.stg_slots, k.slot_bytes, k.pitch_bytes, k.smem_bytes);
+    p->desc = std::string(buf) + " | general path: " + p->desc;
+    return MELT_OK;
+}
+
+bool v2_accepts(const melt_plan *p, const float *x, long long len) {
+    return p->v2_ok && (((uintptr_t)x & 15) == 0) && ((len & 3) == 0);
+}
+
+template <int PREC, int SIGMA>
+static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
+        attr_done = true;
+    }
+    melt_fwd2_kernel<PREC, SIGMA><<<grid, V2_THREADS, kp.smem_bytes, stream>>>(kp);
+    MELT_CUDA(cudaGetLastError());
+    return MELT_OK;
+}
+
+int launch_forward2(const melt_plan *pl, const K2Params &kp, cudaStream_t stream) {
+    int pairs = pl->sm_count / 2;
+    if (kp.n_tiles < pairs) pairs = kp.n_tiles;
+    if (pairs < 1) return MELT_OK;
+    const int grid = 2 * pairs;
+    const int sg = pl->v2_sigma;
+    switch (pl->precision) {
+        case MELT_PREC_COMPENSATED: return sg ? launch_one<P2_COMP, 1>(kp, grid, stream) : launch_one<P2_COMP, 0>(kp, grid, stream);
+        case MELT_PREC_TF32: return sg ? launch_one<P2_TF32, 1>(kp, grid, stream) : launch_one<P2_TF32, 0>(kp, grid, stream);
+        default: return sg ? launch_one<P2_BF16, 1>(kp, grid, stream) : launch_one<P2_BF16, 0>(kp, grid, stream);
+    }
+}
+
+}  // namespace melt

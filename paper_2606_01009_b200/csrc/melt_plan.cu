@@ -39,6 +39,9 @@ static void free_device(melt_plan *p) {
     cudaFree(p->d_bimg);
     cudaFree(p->d_tab);
     cudaFree(p->d_dct);
+    cudaFree(p->d_bimg2);
+    p->d_bimg2 = nullptr;
+    p->v2_ok = false;
     p->d_bimg = nullptr;
     p->d_tab = nullptr;
     p->d_dct = nullptr;
@@ -208,7 +211,7 @@ int plan_build_device(melt_plan *p) {
              k.acc_stages, k.acc_cols, k.a_slots, k.b_resident ? "resident" : "ring", k.b_slots, k.unit_b_bytes,
              k.stg_comb ? "comb" : "whole", k.stg_slots, k.stg_slot_words, k.smem_bytes);
     p->desc = buf;
-    return MELT_OK;
+    return plan_build_v2(p);   // the CTA-pair kernel takes the geometries it covers; this kernel stays the general path
 }
 
 static int validate_common(const melt_plan *p, const float *x, float *out) {
@@ -246,6 +249,14 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
         if (T == 0) return MELT_OK;
         const long long tpc = (T + TILE_M - 1) / TILE_M;
         if (tpc * n_clips > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
+        if (v2_accepts(p, x, len) && !(tap && ((uintptr_t)tap & 3))) {
+            K2Params k2 = p->k2;
+            const long long tpc2 = (T + 255) / 256;
+            if (tpc2 * n_clips > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
+            k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = len; k2.frames_per_clip = T;
+            k2.tiles_per_clip = (int)tpc2; k2.n_tiles = (int)(tpc2 * n_clips);
+            return launch_forward2(p, k2, st);
+        }
         kp.offsets = nullptr; kp.frame_offsets = nullptr; kp.tile_prefix = nullptr;
         kp.len = len; kp.frames_per_clip = T; kp.tiles_per_clip = (int)tpc; kp.n_tiles = (int)(tpc * n_clips);
     }
@@ -282,7 +293,7 @@ extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window
     p->mel_scale = mel_scale; p->n_mfcc = n_mfcc;
     p->layout = MELT_LAYOUT_FRAME_MAJOR; p->precision = MELT_PREC_COMPENSATED; p->drop_last = 0; p->pad = MELT_PAD_NONE;
     p->in_scale_log2 = 12; p->output = MELT_OUTPUT_LOG; p->used = false; p->device = dev; p->sm_count = prop.multiProcessorCount;
-    p->d_bimg = nullptr; p->d_tab = nullptr; p->d_dct = nullptr; p->d_tile_prefix = nullptr; p->d_frame_offsets_scratch = nullptr;
+    p->d_bimg = nullptr; p->d_bimg2 = nullptr; p->v2_ok = false; p->v2_sigma = 0; p->d_tab = nullptr; p->d_dct = nullptr; p->d_tile_prefix = nullptr; p->d_frame_offsets_scratch = nullptr;
     memset(&p->kp, 0, sizeof(p->kp));
     // Eq. (1)-(2): M centres uniformly spaced in mel between fmin and fmax, endpoints excluded
     p->centres.resize(n_mels);

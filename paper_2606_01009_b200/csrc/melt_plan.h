@@ -53,6 +53,38 @@ struct KParams {
     const float *dct;      // [n_mels][dct_pitch]
 };
 
+// ---------------------------------------------------------------------------------------------- v2 (CTA-pair kernel)
+constexpr int V2_THREADS = 512;       // 16 warps: loader, MMA issuer, basis/TMEM, spare, 4 epilogue, 8 converters
+constexpr int V2_MAX_UNITS = 32;      // K-steps per tile the per-unit load table covers
+constexpr int V2_MAX_STG = 12;        // staging ring slots (32-frame chunks)
+constexpr int V2_TAB = 12;            // int16 entries per unit: [0,4) forward quads, [4,8) backward quads, [8] single
+
+struct K2Params {
+    // ---- analysis geometry (as KParams)
+    int n_fft, hop, n_mels, n_mfcc, n_ch;
+    int kstep, units, nb, nk, unit_cols;
+    int acc_cols, acc_stages, a_slots, a_col0;
+    // ---- staging ring of 32-frame chunks: rows of `hop` samples at a padded pitch
+    int rows_per_chunk, pitch_bytes, slot_bytes, stg_slots;
+    // ---- basis (this CTA's half: nb/2 rows per kind)
+    uint32_t unit_b_bytes, kind_bytes;
+    uint32_t off_b, off_stg, off_dct, off_bar, smem_bytes;
+    int dct_pitch;
+    float in_scale, out_scale, out_log10_offset;
+    int output_power, feature_major;
+    // ---- batch (dense)
+    const float *x;
+    float *out, *tap;
+    int n_clips;
+    long long len, frames_per_clip;
+    int tiles_per_clip, n_tiles;  // 256-frame tiles
+    // ---- plan-owned device data
+    const uint8_t *b_img;  // [2 ranks][units] slabs of unit_b_bytes
+    const float *dct;      // [n_mels][dct_pitch]
+    // ---- per-unit shared-memory byte offsets (relative to the first sample of the thread's frame)
+    short tab[V2_MAX_UNITS][V2_TAB];
+};
+
 }  // namespace melt
 
 struct melt_plan {
@@ -63,6 +95,10 @@ struct melt_plan {
     int device, sm_count;
     std::vector<double> centres, win;
     melt::KParams kp;  // geometry + plan-owned device pointers (batch fields filled per call)
+    melt::K2Params k2; // the CTA-pair kernel's view of the same plan (valid when v2_ok)
+    bool v2_ok;        // the geometry is covered by melt_fwd2_kernel
+    int v2_sigma;      // alignment class of the mirrored sample run (0 or 1)
+    uint8_t *d_bimg2;
     uint8_t *d_bimg;
     uint32_t *d_tab;
     float *d_dct;
@@ -74,5 +110,8 @@ struct melt_plan {
 namespace melt {
 int plan_build_device(melt_plan *p);  // (re)builds geometry + operand images for the current options
 int launch_forward(const melt_plan *p, const KParams &kp, cudaStream_t stream);
+int plan_build_v2(melt_plan *p);   // fills p->k2 / p->v2_ok (never fails the plan: v1 remains the general path)
+bool v2_accepts(const melt_plan *p, const float *x, long long len);
+int launch_forward2(const melt_plan *p, const K2Params &kp, cudaStream_t stream);
 int launch_ragged_scan(const melt_plan *p, const long long *offsets, int n_clips, long long *frame_offsets, cudaStream_t stream);
 }  // namespace melt
