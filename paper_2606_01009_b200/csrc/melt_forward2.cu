@@ -156,7 +156,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 bulk_g2s(sbase + p.off_b + (uint32_t)u * p.unit_b_bytes, src + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL));
             if (rank == 1) {  // tell the leader that the peer half has landed
                 mbar_wait(BAR(V_B_FULL), 0);
-                mbar_arrive_cluster(mapa_cluster(BAR(V_B_PEER), 0));
+                mbar_arrive_cluster_release(mapa_cluster(BAR(V_B_PEER), 0));
             }
         }
     } else if (warp == W_MMA) {
@@ -168,11 +168,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             int aslot = 0, stage = 0;
             uint32_t aph = 0, sph = 0;
             for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
-                mbar_wait_cluster(BAR(V_ACC_EMPTY + stage), sph ^ 1u);
+                mbar_wait(BAR(V_ACC_EMPTY + stage), sph ^ 1u);
                 tc_fence_after();
                 const uint32_t d_r = tmem_base + (uint32_t)stage * (uint32_t)p.acc_cols, d_i = d_r + (uint32_t)p.nb;
                 for (int u = 0; u < p.units; ++u) {
-                    mbar_wait_cluster(BAR(V_A_FULL + aslot), aph);
+                    mbar_wait(BAR(V_A_FULL + aslot), aph);
                     tc_fence_after();
                     const uint32_t a = tmem_base + (uint32_t)p.a_col0 + (uint32_t)aslot * (uint32_t)p.unit_cols;
                     const uint32_t b = sbase + p.off_b + (uint32_t)u * p.unit_b_bytes;
@@ -212,6 +212,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         int stage = 0;
         uint32_t sph = 0;
         const long long T = p.frames_per_clip;
+        const bool fast_log = p.n_mfcc == 0 && !p.output_power && p.tap == nullptr;
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             const int b = tile / p.tiles_per_clip;
             const int t0 = (tile - b * p.tiles_per_clip) * 256 + (int)rank * 128;
@@ -235,6 +236,26 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             mbar_wait(BAR(V_ACC_FULL + stage), sph);
             tc_fence_after();
             const uint32_t t_r = lane_taddr + (uint32_t)stage * (uint32_t)p.acc_cols, t_i = t_r + (uint32_t)p.nb;
+            if (fast_log) {
+                // log-Mel, no DCT, no tap: the common case, kept to ~8 instructions per element
+                float *o = optr;
+                const float off = p.out_log10_offset;
+                for (int c0 = 0; c0 < p.nb; c0 += 16) {
+                    uint32_t vr[16], vi[16];
+                    tmem_ld16(t_r + (uint32_t)c0, vr);
+                    tmem_ld16(t_i + (uint32_t)c0, vi);
+                    tmem_wait_ld();
+                    const int nfull = p.n_mels - c0;   // columns of this group that are real Mel bins
+#pragma unroll
+                    for (int c = 0; c < 16; ++c) {
+                        const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                        const float praw = fmaf(r, r, im * im);                                              // Eq. (4)
+                        const float v = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, off), -10.f);                    // Eq. (8), contract form
+                        if (valid && c < nfull) *o = v;
+                        o += cstride;
+                    }
+                }
+            } else {
             for (int c0 = 0; c0 < p.nb; c0 += 16) {
                 uint32_t vr[16], vi[16];
                 tmem_ld16(t_r + (uint32_t)c0, vr);
@@ -248,7 +269,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         const float praw = fmaf(r, r, im * im);                                          // Eq. (4)
                         float v;
                         if (p.output_power) v = praw * p.out_scale;
-                        else v = fmaxf(fmaf(__log2f(praw), kLog10_2, p.out_log10_offset), -10.f);       // Eq. (8), contract form
+                        else v = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, p.out_log10_offset), -10.f);       // Eq. (8), contract form
                         if (p.n_mfcc > 0) {
                             const float *drow = dct_s + m * p.dct_pitch;
                             if (p.dct_pitch <= 16) dct_acc2<4>(cacc, drow, v);
@@ -261,9 +282,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     }
                 }
             }
+            }
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(acc_empty_remote + (uint32_t)stage * 8u);
+            if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
             if (p.n_mfcc > 0 && valid) {                                                                  // Eq. (9)
 #pragma unroll
                 for (int k = 0; k < MAX_MFCC; ++k)
@@ -312,8 +334,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     }
                     bw[0] = lds32(fb + (uint32_t)(int)tb[8]);                       // position KS-1 of the run
                 }
-                mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);
-                tc_fence_after();
                 const uint32_t dst = lane_taddr + (uint32_t)aslot * (uint32_t)p.unit_cols;
                 if (PREC == P2_COMP) {
                     uint32_t v[32];
@@ -331,6 +351,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         v[16 + c] = *reinterpret_cast<const uint32_t *>(&dh);
                         v[24 + c] = *reinterpret_cast<const uint32_t *>(&dl);
                     }
+                    mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    tc_fence_after();
                     tmem_st32(dst, v);
                 } else if (PREC == P2_BF16) {
                     uint32_t v[16];
@@ -341,6 +363,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         v[c] = *reinterpret_cast<const uint32_t *>(&sh);
                         v[8 + c] = *reinterpret_cast<const uint32_t *>(&dh);
                     }
+                    mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    tc_fence_after();
                     tmem_st16(dst, v);
                 } else {
                     uint32_t v[16];
@@ -349,12 +373,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         v[c] = cvt_tf32_rna(fw[c] + bw[c]);
                         v[8 + c] = cvt_tf32_rna(fw[c] - bw[c]);
                     }
+                    mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    tc_fence_after();
                     tmem_st16(dst, v);
                 }
                 tmem_wait_st();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive_cluster(a_full_remote + (uint32_t)aslot * 8u);
+                if (lane == 0) mbar_arrive_remote(a_full_remote + (uint32_t)aslot * 8u);
                 // advance to this group's next unit (the next tile's first one after the last)
                 int du = 2;
                 if (u + 2 >= p.units) du = p.units - u + g;   // ug(next tile, u = g) - ug(this tile, u)

@@ -107,6 +107,8 @@ int plan_build_device(melt_plan *p) {
         k.stg_pitch = TILE_M + 1;
         k.stg_slot_words = 2 * 64 * k.stg_pitch + TILE_M;
         k.stg_slots = 3;
+        while (k.stg_slots > 2 && (long long)SMEM_BUDGET - (long long)k.stg_slots * k.stg_slot_words * 4 - fixed < 4LL * k.unit_b_bytes)
+            --k.stg_slots;  // wide bases (M = 128 per pass, fp16x3): trade one staging slot for a deeper basis ring
         stg_bytes = (uint32_t)(k.stg_slots * k.stg_slot_words * 4);
     }
     const long long b_room = (long long)SMEM_BUDGET - stg_bytes - fixed;

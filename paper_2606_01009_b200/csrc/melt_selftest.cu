@@ -161,7 +161,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(128, 1) selftest_umm
     tc_fence_before();
     mbar_wait(smem_u32(&bar_b), 0);  // every thread: this CTA's half of B has landed
     __syncwarp();
-    if ((tid & 31) == 0) mbar_arrive_cluster(mapa_cluster(smem_u32(&bar_afull), 0));  // tell the leader: A rows + B half ready
+    if ((tid & 31) == 0) mbar_arrive_cluster_release(mapa_cluster(smem_u32(&bar_afull), 0));  // tell the leader: A rows + B half ready
 
     if (rank == 0 && tid == 0) {
         mbar_wait_cluster(smem_u32(&bar_afull), 0);

@@ -170,8 +170,15 @@ __device__ __forceinline__ uint32_t mapa_cluster(uint32_t smem_addr, uint32_t ra
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(rank));
     return r;
 }
-// arrive (release at cluster scope) on an mbarrier given by a shared::cluster address (own or peer CTA)
-__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+// arrive on an mbarrier given by a shared::cluster address (own or peer CTA).  Default semantics (release at CTA scope):
+// no MEMBAR.GPU is emitted.  This is the per-K-step hand-off form: what it publishes lives in TENSOR MEMORY and is
+// ordered by tcgen05.wait + tcgen05.fence::before_thread_sync, not by the generic-proxy memory model.
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+// the same with release semantics at cluster scope (a full memory barrier: hundreds of cycles).  Only for one-time
+// hand-offs of shared-memory contents between the CTAs of a pair.
+__device__ __forceinline__ void mbar_arrive_cluster_release(uint32_t cluster_addr) {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t parity) {  // acquire at cluster scope
@@ -264,6 +271,13 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t *v) {
 }
 
 // ---------------------------------------------------------------------------------------------- conversions
+// log2 on the special-function unit, flush-to-zero form: ONE MUFU.LG2 (the non-ftz form wraps it in a denormal
+// rescue sequence).  lg2(0) = -inf, which the callers clamp.
+__device__ __forceinline__ float lg2_ftz(float x) {
+    float r;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
 __device__ __forceinline__ uint32_t cvt_tf32_rna(float x) {
     uint32_t r;
     asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x));
