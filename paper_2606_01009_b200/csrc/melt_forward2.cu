@@ -73,7 +73,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     uint32_t *tmem_ptr_s = reinterpret_cast<uint32_t *>(smem + p.off_bar + V_NBARS * 8);
     float *dct_s = reinterpret_cast<float *>(smem + p.off_dct);
 
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // provably warp-uniform: role branches stay non-divergent
     const uint32_t rank = cluster_ctarank();
     const int S = p.stg_slots;
 
@@ -110,6 +111,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
 
     if (warp == W_LOAD) {
         // ============================================================== signal loader (bulk-copy engine)
+        // The whole warp runs the (uniform) loop; one elected lane issues the copies.
         int slot = 0;
         uint32_t ph = 0;
         const long long len = p.len;
@@ -120,48 +122,47 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             for (int q = 0; q < 4; ++q) {
                 mbar_wait(BAR(V_STG_EMPTY + slot), ph ^ 1u);
                 const long long row0 = (long long)(t0 + 32 * q);
-                uint32_t bytes[2];
-                uint32_t mine = 0;
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int i = lane + 32 * h;
-                    const long long start = (row0 + i) * p.hop;
-                    long long rem = len - start;
-                    rem = rem < 0 ? 0 : (rem > p.hop ? p.hop : rem);
-                    bytes[h] = (i < p.rows_per_chunk && row0 < p.frames_per_clip) ? (uint32_t)rem * 4u : 0u;
-                    mine += bytes[h];
-                }
-                const uint32_t total = __reduce_add_sync(0xffffffffu, mine);
-                if (lane == 0) {
-                    if (total) mbar_arrive_expect_tx(BAR(V_STG_FULL + slot), total);
-                    else mbar_arrive(BAR(V_STG_FULL + slot));
+                const int n_rows = row0 < p.frames_per_clip ? p.rows_per_chunk : 0;
+                long long avail = len - row0 * p.hop;                      // samples of the clip from the chunk's first row on
+                avail = avail < 0 ? 0 : avail;
+                const long long want = (long long)n_rows * p.hop;
+                const uint32_t total = (uint32_t)(avail < want ? avail : want) * 4u;
+                if (elect_one()) {
+                    const uint32_t full = BAR(V_STG_FULL + slot);
+                    if (total) mbar_arrive_expect_tx(full, total);
+                    else mbar_arrive(full);
+                    uint32_t dst = sbase + p.off_stg + (uint32_t)slot * (uint32_t)p.slot_bytes;
+                    const float *src = xb + row0 * p.hop;
+                    uint32_t left = total;
+                    const uint32_t row_bytes = (uint32_t)p.hop * 4u;
+                    while (left) {
+                        const uint32_t nb = left < row_bytes ? left : row_bytes;
+                        bulk_g2s(dst, src, nb, full);
+                        dst += (uint32_t)p.pitch_bytes; src += p.hop; left -= nb;
+                    }
                 }
                 __syncwarp();
-                const uint32_t dst0 = sbase + p.off_stg + (uint32_t)slot * (uint32_t)p.slot_bytes;
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const int i = lane + 32 * h;
-                    if (bytes[h])
-                        bulk_g2s(dst0 + (uint32_t)i * (uint32_t)p.pitch_bytes, xb + (row0 + i) * p.hop, bytes[h], BAR(V_STG_FULL + slot));
-                }
                 if (++slot == S) { slot = 0; ph ^= 1u; }
             }
         }
     } else if (warp == W_BASIS) {
         // ============================================================== basis: this CTA's half, resident
-        if (lane == 0 && first_tile < n_tiles) {
-            mbar_arrive_expect_tx(BAR(V_B_FULL), (uint32_t)p.units * p.unit_b_bytes);
-            const uint8_t *src = p.b_img + (size_t)rank * p.units * p.unit_b_bytes;
-            for (int u = 0; u < p.units; ++u)
-                bulk_g2s(sbase + p.off_b + (uint32_t)u * p.unit_b_bytes, src + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL));
+        if (first_tile < n_tiles) {
+            if (elect_one()) {
+                mbar_arrive_expect_tx(BAR(V_B_FULL), (uint32_t)p.units * p.unit_b_bytes);
+                const uint8_t *src = p.b_img + (size_t)rank * p.units * p.unit_b_bytes;
+                for (int u = 0; u < p.units; ++u)
+                    bulk_g2s(sbase + p.off_b + (uint32_t)u * p.unit_b_bytes, src + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL));
+            }
+            __syncwarp();
             if (rank == 1) {  // tell the leader that the peer half has landed
                 mbar_wait(BAR(V_B_FULL), 0);
-                mbar_arrive_cluster_release(mapa_cluster(BAR(V_B_PEER), 0));
+                if (lane == 0) mbar_arrive_cluster_release(mapa_cluster(BAR(V_B_PEER), 0));
             }
         }
     } else if (warp == W_MMA) {
-        // ============================================================== MMA issuer (one thread of the leader CTA)
-        if (rank == 0 && lane == 0 && first_tile < n_tiles) {
+        // ============================================================== MMA issuer (leader CTA; one elected lane issues)
+        if (rank == 0 && first_tile < n_tiles) {
             const uint32_t idesc = umma_idesc(PREC == P2_COMP ? UMMA_F16 : (PREC == P2_BF16 ? UMMA_BF16 : UMMA_TF32), (uint32_t)p.nb, 256u);
             mbar_wait(BAR(V_B_FULL), 0);
             mbar_wait_cluster(BAR(V_B_PEER), 0);
@@ -169,36 +170,38 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             uint32_t aph = 0, sph = 0;
             for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
                 mbar_wait(BAR(V_ACC_EMPTY + stage), sph ^ 1u);
-                tc_fence_after();
                 const uint32_t d_r = tmem_base + (uint32_t)stage * (uint32_t)p.acc_cols, d_i = d_r + (uint32_t)p.nb;
                 for (int u = 0; u < p.units; ++u) {
                     mbar_wait(BAR(V_A_FULL + aslot), aph);
                     tc_fence_after();
-                    const uint32_t a = tmem_base + (uint32_t)p.a_col0 + (uint32_t)aslot * (uint32_t)p.unit_cols;
-                    const uint32_t b = sbase + p.off_b + (uint32_t)u * p.unit_b_bytes;
-                    const uint32_t acc = u > 0;
-                    if (PREC == P2_COMP) {
-                        // A kinds: s_hi @0, s_lo @8, d_hi @16, d_lo @24;  B kinds: wc_hi, wc_lo, ws_hi, ws_lo
-                        const uint64_t wc_hi = umma_smem_desc_kmajor_noswz(b, 128, 256);
-                        const uint64_t wc_lo = umma_smem_desc_kmajor_noswz(b + p.kind_bytes, 128, 256);
-                        const uint64_t ws_hi = umma_smem_desc_kmajor_noswz(b + 2 * p.kind_bytes, 128, 256);
-                        const uint64_t ws_lo = umma_smem_desc_kmajor_noswz(b + 3 * p.kind_bytes, 128, 256);
-                        umma2_ts_f16(d_r, a + 0, wc_hi, idesc, acc);
-                        umma2_ts_f16(d_i, a + 16, ws_hi, idesc, acc);
-                        umma2_ts_f16(d_r, a + 8, wc_hi, idesc, 1);
-                        umma2_ts_f16(d_i, a + 24, ws_hi, idesc, 1);
-                        umma2_ts_f16(d_r, a + 0, wc_lo, idesc, 1);
-                        umma2_ts_f16(d_i, a + 16, ws_lo, idesc, 1);
-                    } else {
-                        const uint64_t wc = umma_smem_desc_kmajor_noswz(b, 128, 256);
-                        const uint64_t ws = umma_smem_desc_kmajor_noswz(b + p.kind_bytes, 128, 256);
-                        if (PREC == P2_TF32) { umma2_ts_tf32(d_r, a + 0, wc, idesc, acc); umma2_ts_tf32(d_i, a + 8, ws, idesc, acc); }
-                        else { umma2_ts_f16(d_r, a + 0, wc, idesc, acc); umma2_ts_f16(d_i, a + 8, ws, idesc, acc); }
+                    if (elect_one()) {
+                        const uint32_t a = tmem_base + (uint32_t)p.a_col0 + (uint32_t)aslot * (uint32_t)p.unit_cols;
+                        const uint32_t b = sbase + p.off_b + (uint32_t)u * p.unit_b_bytes;
+                        const uint32_t acc = u > 0;
+                        if (PREC == P2_COMP) {
+                            // A kinds: s_hi @0, s_lo @8, d_hi @16, d_lo @24;  B kinds: wc_hi, wc_lo, ws_hi, ws_lo
+                            const uint64_t wc_hi = umma_smem_desc_kmajor_noswz(b, 128, 256);
+                            const uint64_t wc_lo = umma_smem_desc_kmajor_noswz(b + p.kind_bytes, 128, 256);
+                            const uint64_t ws_hi = umma_smem_desc_kmajor_noswz(b + 2 * p.kind_bytes, 128, 256);
+                            const uint64_t ws_lo = umma_smem_desc_kmajor_noswz(b + 3 * p.kind_bytes, 128, 256);
+                            umma2_ts_f16(d_r, a + 0, wc_hi, idesc, acc);
+                            umma2_ts_f16(d_i, a + 16, ws_hi, idesc, acc);
+                            umma2_ts_f16(d_r, a + 8, wc_hi, idesc, 1);
+                            umma2_ts_f16(d_i, a + 24, ws_hi, idesc, 1);
+                            umma2_ts_f16(d_r, a + 0, wc_lo, idesc, 1);
+                            umma2_ts_f16(d_i, a + 16, ws_lo, idesc, 1);
+                        } else {
+                            const uint64_t wc = umma_smem_desc_kmajor_noswz(b, 128, 256);
+                            const uint64_t ws = umma_smem_desc_kmajor_noswz(b + p.kind_bytes, 128, 256);
+                            if (PREC == P2_TF32) { umma2_ts_tf32(d_r, a + 0, wc, idesc, acc); umma2_ts_tf32(d_i, a + 8, ws, idesc, acc); }
+                            else { umma2_ts_f16(d_r, a + 0, wc, idesc, acc); umma2_ts_f16(d_i, a + 8, ws, idesc, acc); }
+                        }
+                        tc_commit2(BAR(V_A_EMPTY + aslot), 3);
+                        if (u == p.units - 1) tc_commit2(BAR(V_ACC_FULL + stage), 3);
                     }
-                    tc_commit2(BAR(V_A_EMPTY + aslot), 3);
+                    __syncwarp();
                     if (++aslot == p.a_slots) { aslot = 0; aph ^= 1u; }
                 }
-                tc_commit2(BAR(V_ACC_FULL + stage), 3);
                 if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
             }
         }

@@ -9,6 +9,16 @@ namespace melt {
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
+// ---------------------------------------------------------------------------------------------- single-lane issue
+// One lane of a fully converged warp.  Instructions that take uniform-register operands (tcgen05.mma, bulk copies)
+// must be issued from a warp-uniform region guarded by this predicate: inside `if (tid == 0)` the compiler cannot
+// prove uniformity and wraps every such instruction in a per-lane election loop (~100 cycles per tcgen05.mma).
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
+
 // ---------------------------------------------------------------------------------------------- mbarrier
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
