@@ -22,10 +22,12 @@
 #include "melt_plan.h"
 #include "sm100_ptx.cuh"
 
+#include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
 #include <algorithm>
+#include <cstdlib>
 
 namespace melt {
 
@@ -49,6 +51,16 @@ __device__ __forceinline__ float lds32(uint32_t addr) {
     return v;
 }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// Optional event trace (development builds only, -DMELT_TRACE): lane 0 of every warp of cluster 0 appends (tag, clock) pairs.
+#ifdef MELT_TRACE
+__device__ long long *g_melt_trace = nullptr;   // [2 ranks][16 warps][1024] events
+#define TRACE_DECL int tr_n = 0; long long *tr_buf = (g_melt_trace && cluster_id_x() == 0 && (threadIdx.x & 31) == 0) ? g_melt_trace + ((size_t)cluster_ctarank() * 16 + (threadIdx.x >> 5)) * 1024 : nullptr;
+#define TRACE(tag) do { if (tr_buf && tr_n < 1023) tr_buf[++tr_n] = ((long long)(tag) << 48) | (clock64() & 0xFFFFFFFFFFFFll); if (tr_buf) tr_buf[0] = tr_n; } while (0)
+#else
+#define TRACE_DECL
+#define TRACE(tag) do { } while (0)
+#endif
 
 template <int KQ>
 __device__ __forceinline__ void dct_acc2(float (&cacc)[MAX_MFCC], const float *drow, float v) {
@@ -108,6 +120,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
 
     const int first_tile = (int)cluster_id_x(), tile_step = (int)cluster_nid_x();
     const int n_tiles = p.n_tiles;
+    TRACE_DECL
+    TRACE(1);
 
     if (warp == W_LOAD) {
         // ============================================================== signal loader (bulk-copy engine)
@@ -115,33 +129,46 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         int slot = 0;
         uint32_t ph = 0;
         const long long len = p.len;
+        if (p.tma_rows > 0 && lane == 0) tma_prefetch_desc(p.tmap);
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             const int b = tile / p.tiles_per_clip;
             const int t0 = (tile - b * p.tiles_per_clip) * 256 + (int)rank * 128;
             const float *xb = p.x + (long long)b * len;
             for (int q = 0; q < 4; ++q) {
+                TRACE(10);
                 mbar_wait(BAR(V_STG_EMPTY + slot), ph ^ 1u);
+                TRACE(11);
                 const long long row0 = (long long)(t0 + 32 * q);
                 const int n_rows = row0 < p.frames_per_clip ? p.rows_per_chunk : 0;
                 long long avail = len - row0 * p.hop;                      // samples of the clip from the chunk's first row on
                 avail = avail < 0 ? 0 : avail;
                 const long long want = (long long)n_rows * p.hop;
                 const uint32_t total = (uint32_t)(avail < want ? avail : want) * 4u;
+                const uint32_t dst0 = sbase + p.off_stg + (uint32_t)slot * (uint32_t)p.slot_bytes;
+                const bool by_tma = n_rows > 0 && row0 + n_rows <= (long long)p.tma_rows;
                 if (elect_one()) {
                     const uint32_t full = BAR(V_STG_FULL + slot);
-                    if (total) mbar_arrive_expect_tx(full, total);
-                    else mbar_arrive(full);
-                    uint32_t dst = sbase + p.off_stg + (uint32_t)slot * (uint32_t)p.slot_bytes;
-                    const float *src = xb + row0 * p.hop;
-                    uint32_t left = total;
-                    const uint32_t row_bytes = (uint32_t)p.hop * 4u;
-                    while (left) {
-                        const uint32_t nb = left < row_bytes ? left : row_bytes;
-                        bulk_g2s(dst, src, nb, full);
-                        dst += (uint32_t)p.pitch_bytes; src += p.hop; left -= nb;
+                    if (by_tma) {
+                        // one tensor-map box = the whole chunk: rows_per_chunk hop-rows of pitch width (implicit im2col)
+                        mbar_arrive_expect_tx(full, (uint32_t)p.rows_per_chunk * (uint32_t)p.pitch_bytes);
+                        tma_load_3d(dst0, p.tmap, 0, (int)row0, b, full);
+                    } else {
+                        // clip tail (or no tensor map): one bulk copy per hop-row, clipped to the clip
+                        if (total) mbar_arrive_expect_tx(full, total);
+                        else mbar_arrive(full);
+                        uint32_t dst = dst0;
+                        const float *src = xb + row0 * p.hop;
+                        uint32_t left = total;
+                        const uint32_t row_bytes = (uint32_t)p.hop * 4u;
+                        while (left) {
+                            const uint32_t nb = left < row_bytes ? left : row_bytes;
+                            bulk_g2s(dst, src, nb, full);
+                            dst += (uint32_t)p.pitch_bytes; src += p.hop; left -= nb;
+                        }
                     }
                 }
                 __syncwarp();
+                TRACE(12);
                 if (++slot == S) { slot = 0; ph ^= 1u; }
             }
         }
@@ -169,10 +196,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             int aslot = 0, stage = 0;
             uint32_t aph = 0, sph = 0;
             for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+                TRACE(20);
                 mbar_wait(BAR(V_ACC_EMPTY + stage), sph ^ 1u);
+                TRACE(21);
                 const uint32_t d_r = tmem_base + (uint32_t)stage * (uint32_t)p.acc_cols, d_i = d_r + (uint32_t)p.nb;
                 for (int u = 0; u < p.units; ++u) {
                     mbar_wait(BAR(V_A_FULL + aslot), aph);
+                    TRACE(22);
                     tc_fence_after();
                     if (elect_one()) {
                         const uint32_t a = tmem_base + (uint32_t)p.a_col0 + (uint32_t)aslot * (uint32_t)p.unit_cols;
@@ -200,6 +230,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         if (u == p.units - 1) tc_commit2(BAR(V_ACC_FULL + stage), 3);
                     }
                     __syncwarp();
+                    TRACE(23);
                     if (++aslot == p.a_slots) { aslot = 0; aph ^= 1u; }
                 }
                 if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
@@ -236,7 +267,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 tptr = p.tap ? p.tap + ((long long)b * T + t0 + row) * p.n_mels : nullptr;
                 cstride = 1;
             }
+            TRACE(30);
             mbar_wait(BAR(V_ACC_FULL + stage), sph);
+            TRACE(31);
             tc_fence_after();
             const uint32_t t_r = lane_taddr + (uint32_t)stage * (uint32_t)p.acc_cols, t_i = t_r + (uint32_t)p.nb;
             if (fast_log) {
@@ -289,6 +322,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
+            TRACE(32);
             if (p.n_mfcc > 0 && valid) {                                                                  // Eq. (9)
 #pragma unroll
                 for (int k = 0; k < MAX_MFCC; ++k)
@@ -308,11 +342,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         int aslot = g % p.a_slots;               // ring position of unit counter ug = it * units + u, first u = g
         uint32_t aph = (uint32_t)((g / p.a_slots) & 1);
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+            TRACE(40);
             mbar_wait(BAR(V_STG_FULL + sslot), sph);
+            TRACE(41);
             const uint32_t fb = row_off + (uint32_t)sslot * (uint32_t)p.slot_bytes;
             int u = g;
             while (u < p.units) {
                 // ---- loads: NQ forward quads, NQ mirrored quads (+ one single when the mirrored run starts at 1 mod 4)
+                TRACE(42);
                 const short *tb = p.tab[u];
                 float fw[KS], bw[KS];
 #pragma unroll
@@ -354,7 +391,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         v[16 + c] = *reinterpret_cast<const uint32_t *>(&dh);
                         v[24 + c] = *reinterpret_cast<const uint32_t *>(&dl);
                     }
+                    TRACE(43);
                     mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    TRACE(44);
                     tc_fence_after();
                     tmem_st32(dst, v);
                 } else if (PREC == P2_BF16) {
@@ -366,7 +405,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         v[c] = *reinterpret_cast<const uint32_t *>(&sh);
                         v[8 + c] = *reinterpret_cast<const uint32_t *>(&dh);
                     }
+                    TRACE(43);
                     mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    TRACE(44);
                     tc_fence_after();
                     tmem_st16(dst, v);
                 } else {
@@ -376,7 +417,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         v[c] = cvt_tf32_rna(fw[c] + bw[c]);
                         v[8 + c] = cvt_tf32_rna(fw[c] - bw[c]);
                     }
+                    TRACE(43);
                     mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    TRACE(44);
                     tc_fence_after();
                     tmem_st16(dst, v);
                 }
@@ -384,6 +427,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_remote(a_full_remote + (uint32_t)aslot * 8u);
+                TRACE(45);
                 // advance to this group's next unit (the next tile's first one after the last)
                 int du = 2;
                 if (u + 2 >= p.units) du = p.units - u + g;   // ug(next tile, u = g) - ug(this tile, u)
@@ -438,7 +482,7 @@ int plan_build_v2(melt_plan *p) {
     if (k.rows_per_chunk > 64) return MELT_OK;
     const int pitch_words = ((H / 4) & 1) ? H : H + 4;   // pitch / 4 odd: 8 consecutive rows hit 8 distinct 16-byte bank groups
     k.pitch_bytes = pitch_words * 4;
-    k.slot_bytes = k.rows_per_chunk * k.pitch_bytes;
+    k.slot_bytes = round_up2(k.rows_per_chunk * k.pitch_bytes, 128);   // tensor-map boxes land on 128-byte boundaries
     k.kind_bytes = (uint32_t)(k.nb / 2) * 32u;
     k.unit_b_bytes = (uint32_t)k.nk * k.kind_bytes;
     k.dct_pitch = k1.dct_pitch;
@@ -522,6 +566,47 @@ int plan_build_v2(melt_plan *p) {
     return MELT_OK;
 }
 
+// The tensor map depends on the call's buffer (x, len, batch), so it is encoded per call on the host (a few hundred
+// nanoseconds of integer packing inside the driver; no allocation, no synchronisation) and travels as a kernel parameter.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = []() -> EncodeTiledFn {
+        void *f = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+            return nullptr;
+        return (EncodeTiledFn)f;
+    }();
+    return fn;
+}
+
+int v2_encode_tmap(K2Params &k) {
+    k.tma_rows = 0;
+    static const bool disabled = getenv("MELT_DISABLE_TMA") != nullptr;   // debug switch: per-row bulk copies everywhere
+    if (disabled) return MELT_OK;
+    EncodeTiledFn enc = encode_tiled_fn();
+    const long long W = k.pitch_bytes / 4;
+    if (!enc || W > 256 || k.rows_per_chunk > 256 || k.len < W) return MELT_OK;
+    const long long rows = (k.len - W) / k.hop + 1;   // rows whose W-wide extent stays inside a clip (hence inside the buffer)
+    if (rows < k.rows_per_chunk || rows > 0x7fffffffLL) return MELT_OK;
+    static_assert(sizeof(CUtensorMap) == 128, "CUtensorMap size");
+    CUtensorMap tm;
+    const cuuint64_t gdim[3] = {(cuuint64_t)W, (cuuint64_t)rows, (cuuint64_t)k.n_clips};
+    const cuuint64_t gstr[2] = {(cuuint64_t)k.hop * 4u, (cuuint64_t)k.len * 4u};   // overlapping rows: stride (hop) < extent (pitch)
+    const cuuint32_t box[3] = {(cuuint32_t)W, (cuuint32_t)k.rows_per_chunk, 1u};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    if ((gstr[1] & 15) || gstr[1] >= (1ull << 40)) return MELT_OK;
+    const CUresult r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float *>(k.x), gdim, gstr, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return MELT_OK;   // the per-row bulk-copy loader covers everything
+    memcpy(k.tmap, &tm, 128);
+    k.tma_rows = (int)rows;
+    return MELT_OK;
+}
+
 bool v2_accepts(const melt_plan *p, const float *x, long long len) {
     return p->v2_ok && (((uintptr_t)x & 15) == 0) && ((len & 3) == 0);
 }
@@ -552,3 +637,9 @@ int launch_forward2(const melt_plan *pl, const K2Params &kp, cudaStream_t stream
 }
 
 }  // namespace melt
+
+#ifdef MELT_TRACE
+extern "C" int melt_debug_set_trace(long long *buf) {
+    return (int)cudaMemcpyToSymbol(melt::g_melt_trace, &buf, sizeof(buf));
+}
+#endif

@@ -257,6 +257,7 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
             if (tpc2 * n_clips > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
             k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = len; k2.frames_per_clip = T;
             k2.tiles_per_clip = (int)tpc2; k2.n_tiles = (int)(tpc2 * n_clips);
+            v2_encode_tmap(k2);
             return launch_forward2(p, k2, st);
         }
         kp.offsets = nullptr; kp.frame_offsets = nullptr; kp.tile_prefix = nullptr;

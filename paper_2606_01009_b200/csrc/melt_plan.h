@@ -83,6 +83,11 @@ struct K2Params {
     const float *dct;      // [n_mels][dct_pitch]
     // ---- per-unit shared-memory byte offsets (relative to the first sample of the thread's frame)
     short tab[V2_MAX_UNITS][V2_TAB];
+    // ---- implicit im2col by the tensor-map engine: 3-D map over the raw signal, dims (sample-in-row: pitch words,
+    //      hop-row: stride = hop, clip: stride = len); one box = one 32-frame chunk.  tma_rows = hop-rows per clip whose
+    //      whole pitch-wide extent lies inside the clip (chunks reaching beyond take the per-row bulk-copy path); 0 = off.
+    int tma_rows;
+    alignas(64) unsigned char tmap[128];
 };
 
 }  // namespace melt
@@ -113,5 +118,6 @@ int launch_forward(const melt_plan *p, const KParams &kp, cudaStream_t stream);
 int plan_build_v2(melt_plan *p);   // fills p->k2 / p->v2_ok (never fails the plan: v1 remains the general path)
 bool v2_accepts(const melt_plan *p, const float *x, long long len);
 int launch_forward2(const melt_plan *p, const K2Params &kp, cudaStream_t stream);
+int v2_encode_tmap(K2Params &kp);   // fills kp.tmap / kp.tma_rows for this call's (x, len, batch); never fails the call
 int launch_ragged_scan(const melt_plan *p, const long long *offsets, int n_clips, long long *frame_offsets, cudaStream_t stream);
 }  // namespace melt
