@@ -35,10 +35,10 @@ enum { P2_COMP = 0, P2_TF32 = 1, P2_BF16 = 2 };
 // barrier indices (8 bytes each)
 enum {
     V_STG_FULL = 0, V_STG_EMPTY = V2_MAX_STG, V_A_FULL = 2 * V2_MAX_STG, V_A_EMPTY = V_A_FULL + 16, V_ACC_FULL = V_A_EMPTY + 16,
-    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + 1, V_NBARS = V_B_PEER + 1
+    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_NBARS = V_B_PEER + V2_MAX_UNITS
 };
 constexpr int V2_MAX_A_SLOTS = 16;
-constexpr int W_LOAD = 0, W_MMA = 1, W_BASIS = 2, W_EPI0 = 4, W_CONV0 = 8;
+constexpr int W_LOAD = 0, W_MMA = 1, W_BASIS = 2, W_MMA2 = 3, W_EPI0 = 4, W_CONV0 = 8;
 
 __device__ __forceinline__ float4 lds128(uint32_t addr) {
     float4 v;
@@ -50,6 +50,36 @@ __device__ __forceinline__ float lds32(uint32_t addr) {
     asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
     return v;
 }
+// packed fp32 pairs in one 64-bit register (sm_100 FADD2 / FMUL2: two lanes per issue slot)
+__device__ __forceinline__ uint64_t f2_pack(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ uint64_t f2_add(uint64_t a, uint64_t b) {
+    uint64_t r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ uint64_t f2_sub(uint64_t a, uint64_t b) {
+    uint64_t r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ uint64_t f2_mul(uint64_t a, uint64_t b) {
+    uint64_t r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ __half2 f2_to_half2(uint64_t a) {   // round to nearest even, lane 0 -> low half
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a));
+    return __floats2half2_rn(lo, hi);
+}
+__device__ __forceinline__ uint64_t half2_to_f2(__half2 h) {
+    const float2 f = __half22float2(h);
+    return f2_pack(f.x, f.y);
+}
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // Optional event trace (development builds only, -DMELT_TRACE): lane 0 of every warp of cluster 0 appends (tag, clock) pairs.
@@ -57,7 +87,9 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 __device__ long long *g_melt_trace = nullptr;   // [2 ranks][16 warps][1024] events
 #define TRACE_DECL int tr_n = 0; long long *tr_buf = (g_melt_trace && cluster_id_x() == 0 && (threadIdx.x & 31) == 0) ? g_melt_trace + ((size_t)cluster_ctarank() * 16 + (threadIdx.x >> 5)) * 1024 : nullptr;
 #define TRACE(tag) do { if (tr_buf && tr_n < 1023) tr_buf[++tr_n] = ((long long)(tag) << 48) | (clock64() & 0xFFFFFFFFFFFFll); if (tr_buf) tr_buf[0] = tr_n; } while (0)
+#define TRACE_CTA(which) do { if (g_melt_trace && threadIdx.x == 0) g_melt_trace[2 * 16 * 1024 + blockIdx.x * 2 + (which)] = (long long)globaltimer_ns(); } while (0)
 #else
+#define TRACE_CTA(which) do { } while (0)
 #define TRACE_DECL
 #define TRACE(tag) do { } while (0)
 #endif
@@ -77,6 +109,7 @@ __device__ __forceinline__ void dct_acc2(float (&cacc)[MAX_MFCC], const float *d
 template <int PREC, int SIGMA>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
     extern __shared__ __align__(128) uint8_t smem[];
+    TRACE_CTA(0);
     constexpr int KS = (PREC == P2_TF32) ? 8 : 16;  // folded pairs per K-step
     constexpr int NQ = KS / 4;                      // 128-bit loads per direction per K-step
     const uint32_t sbase = smem_u32(smem);
@@ -93,10 +126,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     // ------------------------------------------------------------------ one-time setup
     if (tid == 0) {
         for (int i = 0; i < V2_MAX_STG; ++i) { mbar_init(BAR(V_STG_FULL + i), 1); mbar_init(BAR(V_STG_EMPTY + i), 2); }
-        for (int i = 0; i < V2_MAX_A_SLOTS; ++i) { mbar_init(BAR(V_A_FULL + i), 8); mbar_init(BAR(V_A_EMPTY + i), 1); }
-        for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 1); mbar_init(BAR(V_ACC_EMPTY + i), 8); }
-        mbar_init(BAR(V_B_FULL), 1);
-        mbar_init(BAR(V_B_PEER), 1);
+        for (int i = 0; i < V2_MAX_A_SLOTS; ++i) { mbar_init(BAR(V_A_FULL + i), 8); mbar_init(BAR(V_A_EMPTY + i), 2); }   // both issuers commit
+        for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 2); mbar_init(BAR(V_ACC_EMPTY + i), 8); }
+        for (int i = 0; i < V2_MAX_UNITS; ++i) { mbar_init(BAR(V_B_FULL + i), 1); mbar_init(BAR(V_B_PEER + i), 1); }
         fence_barrier_init();
     }
     if (warp == W_BASIS) {
@@ -174,66 +206,104 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         }
     } else if (warp == W_BASIS) {
         // ============================================================== basis: this CTA's half, resident
+        // One barrier per K-step slab, so that the first tile's MMAs start as soon as the first slabs have landed.
         if (first_tile < n_tiles) {
             if (elect_one()) {
-                mbar_arrive_expect_tx(BAR(V_B_FULL), (uint32_t)p.units * p.unit_b_bytes);
-                const uint8_t *src = p.b_img + (size_t)rank * p.units * p.unit_b_bytes;
-                for (int u = 0; u < p.units; ++u)
-                    bulk_g2s(sbase + p.off_b + (uint32_t)u * p.unit_b_bytes, src + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL));
+                // the image is replicated in global memory: 74 clusters fetching the same lines at once serialise in L2
+                const uint8_t *src = p.b_img + ((size_t)(cluster_id_x() % (uint32_t)p.b_replicas) * 2 + rank) * p.units * p.unit_b_bytes;
+                for (int u = 0; u < p.units; ++u) {
+                    mbar_arrive_expect_tx(BAR(V_B_FULL + u), p.unit_b_bytes);
+                    bulk_g2s(sbase + p.off_b + (uint32_t)u * p.unit_b_bytes, src + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL + u));
+                }
             }
             __syncwarp();
-            if (rank == 1) {  // tell the leader that the peer half has landed
-                mbar_wait(BAR(V_B_FULL), 0);
-                if (lane == 0) mbar_arrive_cluster_release(mapa_cluster(BAR(V_B_PEER), 0));
+            if (rank == 1) {  // tell the leader, slab by slab, that the peer half has landed
+                for (int u = 0; u < p.units; ++u) {
+                    mbar_wait(BAR(V_B_FULL + u), 0);
+                    // complete_tx has made the slab visible in this CTA's shared memory; the tensor core of the pair reads
+                    // it through the async proxy, so a plain remote arrival (no cluster-scope fence, which costs ~1000 cycles
+                    // with bulk copies in flight) is the hand-off
+                    if (lane == 0) mbar_arrive_remote(mapa_cluster(BAR(V_B_PEER + u), 0));
+                }
             }
         }
-    } else if (warp == W_MMA) {
-        // ============================================================== MMA issuer (leader CTA; one elected lane issues)
+    } else if (warp == W_MMA || warp == W_MMA2) {
+        // ============================================================== MMA issuers (leader CTA)
+        // Two issuer warps on different schedulers: W_MMA accumulates R (A = folded sums, B = cos rows), W_MMA2 accumulates I
+        // (A = folded differences, B = sin rows).  Every accumulator has ONE issuing thread, so the summation order is fixed.
+        // An iteration covers two K-steps: the fixed cost of a hand-off (barrier probe, fence, election, operand set-up) is
+        // then paid once per ~480 cycles of tensor work instead of once per ~240, which a warp that shares its scheduler
+        // with three busy converter / epilogue warps could not keep up with.
         if (rank == 0 && first_tile < n_tiles) {
+            const int which = warp == W_MMA ? 0 : 1;
             const uint32_t idesc = umma_idesc(PREC == P2_COMP ? UMMA_F16 : (PREC == P2_BF16 ? UMMA_BF16 : UMMA_TF32), (uint32_t)p.nb, 256u);
-            mbar_wait(BAR(V_B_FULL), 0);
-            mbar_wait_cluster(BAR(V_B_PEER), 0);
+            // shared-memory descriptors of K-step 0; K-step u adds u * unit_b_bytes (in 16-byte units) to the address field
+            // B kinds: COMPENSATED [wc_hi, wc_lo, ws_hi, ws_lo]; single pass [wc, ws]
+            const uint32_t b0 = sbase + p.off_b + (uint32_t)which * (PREC == P2_COMP ? 2u : 1u) * p.kind_bytes;
+            const uint64_t dsc_hi = umma_smem_desc_kmajor_noswz(b0, 128, 256);
+            const uint64_t dsc_lo = umma_smem_desc_kmajor_noswz(b0 + p.kind_bytes, 128, 256);
+            const uint64_t dstep = (uint64_t)(p.unit_b_bytes >> 4);
+            const int units = p.units, a_slots = p.a_slots, acc_stages = p.acc_stages;
+            // A kinds: COMPENSATED s_hi @0, s_lo @8, d_hi @16, d_lo @24; single pass s @0, d @8
+            const uint32_t a_base = tmem_base + (uint32_t)p.a_col0 + (uint32_t)which * (PREC == P2_COMP ? 16u : 8u);
+            const uint32_t unit_cols = (uint32_t)p.unit_cols;
+            const uint32_t acc_cols = (uint32_t)p.acc_cols;
+            const uint32_t d_base = tmem_base + (uint32_t)which * (uint32_t)p.nb;
             int aslot = 0, stage = 0;
             uint32_t aph = 0, sph = 0;
+            bool basis_pending = true;
             for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
                 TRACE(20);
                 mbar_wait(BAR(V_ACC_EMPTY + stage), sph ^ 1u);
                 TRACE(21);
-                const uint32_t d_r = tmem_base + (uint32_t)stage * (uint32_t)p.acc_cols, d_i = d_r + (uint32_t)p.nb;
-                for (int u = 0; u < p.units; ++u) {
+                const uint32_t d = d_base + (uint32_t)stage * acc_cols;
+                uint64_t du = 0;
+                for (int u = 0; u < units; u += 2) {
+                    const bool two = u + 1 < units;
+                    int aslot1 = aslot + 1;
+                    uint32_t aph1 = aph;
+                    if (aslot1 == a_slots) { aslot1 = 0; aph1 ^= 1u; }
+                    if (basis_pending) {
+                        mbar_wait(BAR(V_B_FULL + u), 0); mbar_wait_cluster(BAR(V_B_PEER + u), 0);
+                        if (two) { mbar_wait(BAR(V_B_FULL + u + 1), 0); mbar_wait_cluster(BAR(V_B_PEER + u + 1), 0); }
+                    }
                     mbar_wait(BAR(V_A_FULL + aslot), aph);
+                    if (two) mbar_wait(BAR(V_A_FULL + aslot1), aph1);
                     TRACE(22);
                     tc_fence_after();
                     if (elect_one()) {
-                        const uint32_t a = tmem_base + (uint32_t)p.a_col0 + (uint32_t)aslot * (uint32_t)p.unit_cols;
-                        const uint32_t b = sbase + p.off_b + (uint32_t)u * p.unit_b_bytes;
+                        const uint32_t a0 = a_base + (uint32_t)aslot * unit_cols, a1 = a_base + (uint32_t)aslot1 * unit_cols;
                         const uint32_t acc = u > 0;
                         if (PREC == P2_COMP) {
-                            // A kinds: s_hi @0, s_lo @8, d_hi @16, d_lo @24;  B kinds: wc_hi, wc_lo, ws_hi, ws_lo
-                            const uint64_t wc_hi = umma_smem_desc_kmajor_noswz(b, 128, 256);
-                            const uint64_t wc_lo = umma_smem_desc_kmajor_noswz(b + p.kind_bytes, 128, 256);
-                            const uint64_t ws_hi = umma_smem_desc_kmajor_noswz(b + 2 * p.kind_bytes, 128, 256);
-                            const uint64_t ws_lo = umma_smem_desc_kmajor_noswz(b + 3 * p.kind_bytes, 128, 256);
-                            umma2_ts_f16(d_r, a + 0, wc_hi, idesc, acc);
-                            umma2_ts_f16(d_i, a + 16, ws_hi, idesc, acc);
-                            umma2_ts_f16(d_r, a + 8, wc_hi, idesc, 1);
-                            umma2_ts_f16(d_i, a + 24, ws_hi, idesc, 1);
-                            umma2_ts_f16(d_r, a + 0, wc_lo, idesc, 1);
-                            umma2_ts_f16(d_i, a + 16, ws_lo, idesc, 1);
+                            umma2_ts_f16(d, a0, dsc_hi + du, idesc, acc);          // hi . hi
+                            umma2_ts_f16(d, a0 + 8, dsc_hi + du, idesc, 1);        // lo . hi
+                            umma2_ts_f16(d, a0, dsc_lo + du, idesc, 1);            // hi . lo
+                            tc_commit2(BAR(V_A_EMPTY + aslot), 3);
+                            if (two) {
+                                umma2_ts_f16(d, a1, dsc_hi + du + dstep, idesc, 1);
+                                umma2_ts_f16(d, a1 + 8, dsc_hi + du + dstep, idesc, 1);
+                                umma2_ts_f16(d, a1, dsc_lo + du + dstep, idesc, 1);
+                                tc_commit2(BAR(V_A_EMPTY + aslot1), 3);
+                            }
+                        } else if (PREC == P2_TF32) {
+                            umma2_ts_tf32(d, a0, dsc_hi + du, idesc, acc);
+                            tc_commit2(BAR(V_A_EMPTY + aslot), 3);
+                            if (two) { umma2_ts_tf32(d, a1, dsc_hi + du + dstep, idesc, 1); tc_commit2(BAR(V_A_EMPTY + aslot1), 3); }
                         } else {
-                            const uint64_t wc = umma_smem_desc_kmajor_noswz(b, 128, 256);
-                            const uint64_t ws = umma_smem_desc_kmajor_noswz(b + p.kind_bytes, 128, 256);
-                            if (PREC == P2_TF32) { umma2_ts_tf32(d_r, a + 0, wc, idesc, acc); umma2_ts_tf32(d_i, a + 8, ws, idesc, acc); }
-                            else { umma2_ts_f16(d_r, a + 0, wc, idesc, acc); umma2_ts_f16(d_i, a + 8, ws, idesc, acc); }
+                            umma2_ts_f16(d, a0, dsc_hi + du, idesc, acc);
+                            tc_commit2(BAR(V_A_EMPTY + aslot), 3);
+                            if (two) { umma2_ts_f16(d, a1, dsc_hi + du + dstep, idesc, 1); tc_commit2(BAR(V_A_EMPTY + aslot1), 3); }
                         }
-                        tc_commit2(BAR(V_A_EMPTY + aslot), 3);
-                        if (u == p.units - 1) tc_commit2(BAR(V_ACC_FULL + stage), 3);
+                        if (u + 2 >= units) tc_commit2(BAR(V_ACC_FULL + stage), 3);
                     }
                     __syncwarp();
                     TRACE(23);
-                    if (++aslot == p.a_slots) { aslot = 0; aph ^= 1u; }
+                    du += 2 * dstep;
+                    if (two) { aslot = aslot1; aph = aph1; }
+                    if (++aslot == a_slots) { aslot = 0; aph ^= 1u; }
                 }
-                if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
+                basis_pending = false;
+                if (++stage == acc_stages) { stage = 0; sph ^= 1u; }
             }
         }
     } else if (warp >= W_EPI0 && warp < W_EPI0 + 4) {
@@ -376,26 +446,32 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 }
                 const uint32_t dst = lane_taddr + (uint32_t)aslot * (uint32_t)p.unit_cols;
                 if (PREC == P2_COMP) {
-                    uint32_t v[32];
+                    // packed fp32 arithmetic (FMUL2 / FADD2): two folded pairs per instruction.  The mirrored samples are
+                    // scaled one by one, which also puts them in pair order at no cost; scaling by 2^s is exact, so
+                    // t + b == fma(f, S, b).
+                    uint32_t vsh[8], vsl[8], vdh[8], vdl[8];
+                    const uint64_t S2 = f2_pack(S_in, S_in);
 #pragma unroll
                     for (int c = 0; c < 8; ++c) {
-                        const float b0 = bw[2 * c] * S_in, b1 = bw[2 * c + 1] * S_in;
-                        const float s0 = fmaf(fw[2 * c], S_in, b0), s1 = fmaf(fw[2 * c + 1], S_in, b1);
-                        const float d0 = fmaf(fw[2 * c], S_in, -b0), d1 = fmaf(fw[2 * c + 1], S_in, -b1);
-                        const __half2 sh = __floats2half2_rn(s0, s1), dh = __floats2half2_rn(d0, d1);
-                        const float2 shf = __half22float2(sh), dhf = __half22float2(dh);
-                        const __half2 sl = __floats2half2_rn(s0 - shf.x, s1 - shf.y);
-                        const __half2 dl = __floats2half2_rn(d0 - dhf.x, d1 - dhf.y);
-                        v[c] = *reinterpret_cast<const uint32_t *>(&sh);
-                        v[8 + c] = *reinterpret_cast<const uint32_t *>(&sl);
-                        v[16 + c] = *reinterpret_cast<const uint32_t *>(&dh);
-                        v[24 + c] = *reinterpret_cast<const uint32_t *>(&dl);
+                        const uint64_t t = f2_mul(f2_pack(fw[2 * c], fw[2 * c + 1]), S2);
+                        const uint64_t b = f2_pack(bw[2 * c] * S_in, bw[2 * c + 1] * S_in);
+                        const uint64_t s = f2_add(t, b), d = f2_sub(t, b);
+                        const __half2 sh = f2_to_half2(s), dh = f2_to_half2(d);
+                        const uint64_t sr = f2_sub(s, half2_to_f2(sh)), dr = f2_sub(d, half2_to_f2(dh));
+                        const __half2 sl = f2_to_half2(sr), dl = f2_to_half2(dr);
+                        vsh[c] = *reinterpret_cast<const uint32_t *>(&sh);
+                        vsl[c] = *reinterpret_cast<const uint32_t *>(&sl);
+                        vdh[c] = *reinterpret_cast<const uint32_t *>(&dh);
+                        vdl[c] = *reinterpret_cast<const uint32_t *>(&dl);
                     }
                     TRACE(43);
                     mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
                     TRACE(44);
                     tc_fence_after();
-                    tmem_st32(dst, v);
+                    tmem_st8(dst, vsh);
+                    tmem_st8(dst + 8, vsl);
+                    tmem_st8(dst + 16, vdh);
+                    tmem_st8(dst + 24, vdl);
                 } else if (PREC == P2_BF16) {
                     uint32_t v[16];
 #pragma unroll
@@ -447,6 +523,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     __syncthreads();
     cluster_sync_all();
     if (warp == W_BASIS) tmem_dealloc2(tmem_base, 512);
+    TRACE_CTA(1);
 }
 
 // ---------------------------------------------------------------------------------------------- host side
@@ -551,8 +628,14 @@ int plan_build_v2(melt_plan *p) {
         }
     cudaFree(p->d_bimg2);
     p->d_bimg2 = nullptr;
-    MELT_CUDA(cudaMalloc(&p->d_bimg2, img_bytes));
-    MELT_CUDA(cudaMemcpy(p->d_bimg2, img.data(), img_bytes, cudaMemcpyHostToDevice));
+    {   // replicas of the image spread the clusters' simultaneous first fetch over more L2 lines (tuning knob; default 1)
+        const char *e = getenv("MELT_BASIS_REPLICAS");
+        const int want = e ? atoi(e) : 1;
+        k.b_replicas = (int)std::max<size_t>(1, std::min<size_t>((size_t)std::max(want, 1), ((size_t)8 << 20) / img_bytes));
+    }
+    MELT_CUDA(cudaMalloc(&p->d_bimg2, img_bytes * k.b_replicas));
+    for (int r = 0; r < k.b_replicas; ++r)
+        MELT_CUDA(cudaMemcpy(p->d_bimg2 + (size_t)r * img_bytes, img.data(), img_bytes, cudaMemcpyHostToDevice));
     k.b_img = p->d_bimg2;
     k.dct = p->d_dct;
     p->v2_ok = true;

@@ -79,7 +79,8 @@ struct K2Params {
     long long len, frames_per_clip;
     int tiles_per_clip, n_tiles;  // 256-frame tiles
     // ---- plan-owned device data
-    const uint8_t *b_img;  // [2 ranks][units] slabs of unit_b_bytes
+    const uint8_t *b_img;  // [b_replicas][2 ranks][units] slabs of unit_b_bytes
+    int b_replicas;
     const float *dct;      // [n_mels][dct_pitch]
     // ---- per-unit shared-memory byte offsets (relative to the first sample of the thread's frame)
     short tab[V2_MAX_UNITS][V2_TAB];
