@@ -129,6 +129,16 @@ int melt_plan_get_centres(const melt_plan *plan, double *f_hz);
 int melt_forward(const melt_plan *plan, const float *x, int batch, long long len, float *out, void *stream);
 
 /*
+ * melt_forward_host -- melt_forward on HOST buffers: copies x_host [batch, len] to a plan-owned device workspace, runs the
+ * hot path and copies the result to out_host (batch * C * T floats, layout per MELT_OPT_LAYOUT), all asynchronously on
+ * `stream`.  The call returns without waiting: synchronise the stream before reading out_host or reusing x_host.  Pinned
+ * (page-locked) host buffers are needed for the copies to be asynchronous.  The workspace is allocated on the first call and
+ * re-allocated (after a stream synchronisation) only when a later call needs more room; because it belongs to the plan,
+ * calls of melt_forward_host on one plan must be issued on one stream at a time.
+ */
+int melt_forward_host(melt_plan *plan, const float *x_host, int batch, long long len, float *out_host, void *stream);
+
+/*
  * melt_forward_ragged -- the whole hot path on clips packed back to back (configs[3]).
  *   x                  device, fp32, packed samples;
  *   offsets            device, int64, n_clips + 1 ascending sample offsets into x (clip i = [offsets[i], offsets[i+1]));

@@ -22,7 +22,7 @@ MELT_OUTPUT_LOG, MELT_OUTPUT_POWER = 0, 1
 # every symbol include/melt.h declares (tests/test_abi.py checks the header against this list and the .so)
 SYMBOLS = [
     "melt_plan_create", "melt_plan_destroy", "melt_plan_set_option", "melt_num_frames", "melt_num_channels",
-    "melt_plan_get_centres", "melt_forward", "melt_forward_ragged", "melt_forward_tap", "melt_last_error",
+    "melt_plan_get_centres", "melt_forward", "melt_forward_host", "melt_forward_ragged", "melt_forward_tap", "melt_last_error",
     "melt_plan_describe", "melt_selftest_umma", "melt_selftest_umma2",
 ]
 
@@ -60,6 +60,7 @@ def lib():
     L.melt_plan_get_centres.argtypes = [vp, C.POINTER(dbl)]
     L.melt_forward.argtypes = [vp, vp, ip, ll, vp, vp]
     L.melt_forward_ragged.argtypes = [vp, vp, vp, ip, vp, vp, vp]
+    L.melt_forward_host.argtypes = [vp, vp, ip, ll, vp, vp]
     L.melt_forward_tap.argtypes = [vp, vp, vp, ip, ll, vp, vp, vp, vp]
     L.melt_last_error.restype = C.c_char_p
     L.melt_plan_describe.restype = C.c_char_p
@@ -123,6 +124,15 @@ def melt_plan_describe(plan):
 
 def melt_forward(plan, x, batch, length, out, stream=0):
     _check(lib().melt_forward(plan, _ptr(x), int(batch), int(length), _ptr(out), stream or None))
+
+
+def melt_forward_host(plan, x_host, batch, length, out_host, stream=0):
+    """x_host / out_host: host pointers (ints), pinned torch CPU tensors or numpy arrays; asynchronous on `stream`."""
+    def hp(t):
+        if isinstance(t, int):
+            return t
+        return int(t.data_ptr()) if hasattr(t, "data_ptr") else int(t.ctypes.data)
+    _check(lib().melt_forward_host(plan, hp(x_host), int(batch), int(length), hp(out_host), stream or None))
 
 
 def melt_forward_ragged(plan, x, offsets, n_clips, out, out_frame_offsets, stream=0):

@@ -42,6 +42,10 @@ constexpr int W_LOAD = 0, W_MMA = 1, W_BASIS = 2, W_MMA2 = 3, W_EPI0 = 4, W_CONV
 
 __device__ __forceinline__ float4 lds128(uint32_t addr) {
     float4 v;
+#ifdef MELT_ABL_NOLDS
+    v.x = __uint_as_float(addr); v.y = v.x; v.z = v.x; v.w = v.x;
+    return v;
+#endif
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
 }
@@ -80,6 +84,12 @@ __device__ __forceinline__ uint64_t half2_to_f2(__half2 h) {
     const float2 f = __half22float2(h);
     return f2_pack(f.x, f.y);
 }
+#ifdef MELT_ABL_NOST
+#define tmem_st8(a, v) do { if ((v)[0] == 0x7fc12345u) asm volatile("trap;"); } while (0)
+#endif
+#ifdef MELT_ABL_NOMMA
+#define umma2_ts_f16(...) do { } while (0)
+#endif
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // Optional event trace (development builds only, -DMELT_TRACE): lane 0 of every warp of cluster 0 appends (tag, clock) pairs.
@@ -149,6 +159,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     cluster_sync_all();
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr_s;
+    if (tid == 0) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the next forward may start filling freed SMs
 
     const int first_tile = (int)cluster_id_x(), tile_step = (int)cluster_nid_x();
     const int n_tiles = p.n_tiles;
@@ -180,11 +191,28 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 const bool by_tma = n_rows > 0 && row0 + n_rows <= (long long)p.tma_rows;
                 if (elect_one()) {
                     const uint32_t full = BAR(V_STG_FULL + slot);
+#ifdef MELT_ABL_NOTMA
+                    mbar_arrive(full);
+                    if (false) {
+#else
                     if (by_tma) {
+#endif
                         // one tensor-map box = the whole chunk: rows_per_chunk hop-rows of pitch width (implicit im2col)
                         mbar_arrive_expect_tx(full, (uint32_t)p.rows_per_chunk * (uint32_t)p.pitch_bytes);
                         tma_load_3d(dst0, p.tmap, 0, (int)row0, b, full);
+                        // The staging ring holds less than two tiles, so the last chunk of the NEXT tile can only be requested
+                        // when this tile ends: pull the tile after next into L2 now, so that request costs an L2 hit, not DRAM
+                        const int ptile = tile + 2 * tile_step;
+                        if (ptile < n_tiles) {
+                            const int pb = ptile / p.tiles_per_clip;
+                            const long long prow = (long long)((ptile - pb * p.tiles_per_clip) * 256 + (int)rank * 128 + 32 * q);
+                            if (prow + p.rows_per_chunk <= (long long)p.tma_rows) tma_prefetch_l2_3d(p.tmap, 0, (int)prow, pb);
+                        }
+#ifdef MELT_ABL_NOTMA
+                    } else if (false) {
+#else
                     } else {
+#endif
                         // clip tail (or no tensor map): one bulk copy per hop-row, clipped to the clip
                         if (total) mbar_arrive_expect_tx(full, total);
                         else mbar_arrive(full);
@@ -260,46 +288,38 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 uint64_t du = 0;
                 for (int u = 0; u < units; u += 2) {
                     const bool two = u + 1 < units;
-                    int aslot1 = aslot + 1;
-                    uint32_t aph1 = aph;
-                    if (aslot1 == a_slots) { aslot1 = 0; aph1 ^= 1u; }
                     if (basis_pending) {
                         mbar_wait(BAR(V_B_FULL + u), 0); mbar_wait_cluster(BAR(V_B_PEER + u), 0);
                         if (two) { mbar_wait(BAR(V_B_FULL + u + 1), 0); mbar_wait_cluster(BAR(V_B_PEER + u + 1), 0); }
                     }
-                    mbar_wait(BAR(V_A_FULL + aslot), aph);
-                    if (two) mbar_wait(BAR(V_A_FULL + aslot1), aph1);
+                    mbar_wait(BAR(V_A_FULL + aslot), aph);      // one operand slot holds the pair of K-steps
                     TRACE(22);
                     tc_fence_after();
                     if (elect_one()) {
-                        const uint32_t a0 = a_base + (uint32_t)aslot * unit_cols, a1 = a_base + (uint32_t)aslot1 * unit_cols;
+                        const uint32_t a0 = a_base + (uint32_t)aslot * 2u * unit_cols, a1 = a0 + unit_cols;
                         const uint32_t acc = u > 0;
                         if (PREC == P2_COMP) {
                             umma2_ts_f16(d, a0, dsc_hi + du, idesc, acc);          // hi . hi
                             umma2_ts_f16(d, a0 + 8, dsc_hi + du, idesc, 1);        // lo . hi
                             umma2_ts_f16(d, a0, dsc_lo + du, idesc, 1);            // hi . lo
-                            tc_commit2(BAR(V_A_EMPTY + aslot), 3);
                             if (two) {
                                 umma2_ts_f16(d, a1, dsc_hi + du + dstep, idesc, 1);
                                 umma2_ts_f16(d, a1 + 8, dsc_hi + du + dstep, idesc, 1);
                                 umma2_ts_f16(d, a1, dsc_lo + du + dstep, idesc, 1);
-                                tc_commit2(BAR(V_A_EMPTY + aslot1), 3);
                             }
                         } else if (PREC == P2_TF32) {
                             umma2_ts_tf32(d, a0, dsc_hi + du, idesc, acc);
-                            tc_commit2(BAR(V_A_EMPTY + aslot), 3);
-                            if (two) { umma2_ts_tf32(d, a1, dsc_hi + du + dstep, idesc, 1); tc_commit2(BAR(V_A_EMPTY + aslot1), 3); }
+                            if (two) umma2_ts_tf32(d, a1, dsc_hi + du + dstep, idesc, 1);
                         } else {
                             umma2_ts_f16(d, a0, dsc_hi + du, idesc, acc);
-                            tc_commit2(BAR(V_A_EMPTY + aslot), 3);
-                            if (two) { umma2_ts_f16(d, a1, dsc_hi + du + dstep, idesc, 1); tc_commit2(BAR(V_A_EMPTY + aslot1), 3); }
+                            if (two) umma2_ts_f16(d, a1, dsc_hi + du + dstep, idesc, 1);
                         }
+                        tc_commit2(BAR(V_A_EMPTY + aslot), 3);
                         if (u + 2 >= units) tc_commit2(BAR(V_ACC_FULL + stage), 3);
                     }
                     __syncwarp();
                     TRACE(23);
                     du += 2 * dstep;
-                    if (two) { aslot = aslot1; aph = aph1; }
                     if (++aslot == a_slots) { aslot = 0; aph ^= 1u; }
                 }
                 basis_pending = false;
@@ -317,6 +337,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         uint32_t sph = 0;
         const long long T = p.frames_per_clip;
         const bool fast_log = p.n_mfcc == 0 && !p.output_power && p.tap == nullptr;
+        bool dep_done = false;
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             const int b = tile / p.tiles_per_clip;
             const int t0 = (tile - b * p.tiles_per_clip) * 256 + (int)rank * 128;
@@ -339,10 +360,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             }
             TRACE(30);
             mbar_wait(BAR(V_ACC_FULL + stage), sph);
+            if (!dep_done) { asm volatile("griddepcontrol.wait;" ::: "memory"); dep_done = true; }   // before the first global store
             TRACE(31);
             tc_fence_after();
             const uint32_t t_r = lane_taddr + (uint32_t)stage * (uint32_t)p.acc_cols, t_i = t_r + (uint32_t)p.nb;
+#ifdef MELT_ABL_NOEPI
+            if (false) {
+#else
             if (fast_log) {
+#endif
                 // log-Mel, no DCT, no tap: the common case, kept to ~8 instructions per element
                 float *o = optr;
                 const float off = p.out_log10_offset;
@@ -362,7 +388,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     }
                 }
             } else {
+#ifdef MELT_ABL_NOEPI
+            for (int c0 = 0; c0 < 0; c0 += 16) {
+#else
             for (int c0 = 0; c0 < p.nb; c0 += 16) {
+#endif
                 uint32_t vr[16], vi[16];
                 tmem_ld16(t_r + (uint32_t)c0, vr);
                 tmem_ld16(t_i + (uint32_t)c0, vi);
@@ -411,13 +441,29 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         uint32_t sph = 0;
         int aslot = g % p.a_slots;               // ring position of unit counter ug = it * units + u, first u = g
         uint32_t aph = (uint32_t)((g / p.a_slots) & 1);
+        const int npairs = (p.units + 1) >> 1;   // one operand slot = a PAIR of K-steps: every hand-off cost is paid per pair
+        int pub_slot = -1;                       // operand slot written (tcgen05.st issued) but not yet handed to the MMA issuers
+#define PUBLISH_PREV()                                                                              \
+        do {                                                                                        \
+            if (pub_slot >= 0) {                                                                    \
+                tmem_wait_st();                                                                     \
+                tc_fence_before();                                                                  \
+                __syncwarp();                                                                       \
+                if (lane == 0) mbar_arrive_remote(a_full_remote + (uint32_t)pub_slot * 8u);         \
+                pub_slot = -1;                                                                      \
+            }                                                                                       \
+        } while (0)
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             TRACE(40);
             mbar_wait(BAR(V_STG_FULL + sslot), sph);
             TRACE(41);
             const uint32_t fb = row_off + (uint32_t)sslot * (uint32_t)p.slot_bytes;
-            int u = g;
-            while (u < p.units) {
+            int pr = g;   // this group's K-step pairs: g, g + 2, ...
+            while (pr < npairs) {
+#pragma unroll 1
+              for (int h = 0; h < 2; ++h) {
+                const int u = 2 * pr + h;
+                if (u >= p.units) break;
                 // ---- loads: NQ forward quads, NQ mirrored quads (+ one single when the mirrored run starts at 1 mod 4)
                 TRACE(42);
                 const short *tb = p.tab[u];
@@ -444,7 +490,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     }
                     bw[0] = lds32(fb + (uint32_t)(int)tb[8]);                       // position KS-1 of the run
                 }
-                const uint32_t dst = lane_taddr + (uint32_t)aslot * (uint32_t)p.unit_cols;
+                const uint32_t dst = lane_taddr + (uint32_t)(2 * aslot + h) * (uint32_t)p.unit_cols;
                 if (PREC == P2_COMP) {
                     // packed fp32 arithmetic (FMUL2 / FADD2): two folded pairs per instruction.  The mirrored samples are
                     // scaled one by one, which also puts them in pair order at no cost; scaling by 2^s is exact, so
@@ -453,6 +499,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     const uint64_t S2 = f2_pack(S_in, S_in);
 #pragma unroll
                     for (int c = 0; c < 8; ++c) {
+#ifdef MELT_ABL_NOMATH
+                        vsh[c] = __float_as_uint(fw[2 * c]); vsl[c] = __float_as_uint(bw[2 * c]); vdh[c] = __float_as_uint(fw[2 * c + 1]); vdl[c] = __float_as_uint(bw[2 * c + 1]);
+                        continue;
+#endif
                         const uint64_t t = f2_mul(f2_pack(fw[2 * c], fw[2 * c + 1]), S2);
                         const uint64_t b = f2_pack(bw[2 * c] * S_in, bw[2 * c + 1] * S_in);
                         const uint64_t s = f2_add(t, b), d = f2_sub(t, b);
@@ -465,7 +515,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         vdl[c] = *reinterpret_cast<const uint32_t *>(&dl);
                     }
                     TRACE(43);
-                    mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    if (h == 0) {
+                        PUBLISH_PREV();
+                        mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    }
                     TRACE(44);
                     tc_fence_after();
                     tmem_st8(dst, vsh);
@@ -482,7 +535,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         v[8 + c] = *reinterpret_cast<const uint32_t *>(&dh);
                     }
                     TRACE(43);
-                    mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    if (h == 0) {
+                        PUBLISH_PREV();
+                        mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    }
                     TRACE(44);
                     tc_fence_after();
                     tmem_st16(dst, v);
@@ -494,28 +550,31 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         v[8 + c] = cvt_tf32_rna(fw[c] - bw[c]);
                     }
                     TRACE(43);
-                    mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    if (h == 0) {
+                        PUBLISH_PREV();
+                        mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    }
                     TRACE(44);
                     tc_fence_after();
                     tmem_st16(dst, v);
                 }
-                tmem_wait_st();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive_remote(a_full_remote + (uint32_t)aslot * 8u);
+              }
+                pub_slot = aslot;   // published after the NEXT pair's first K-step: the tensor-memory stores complete under it
                 TRACE(45);
-                // advance to this group's next unit (the next tile's first one after the last)
-                int du = 2;
-                if (u + 2 >= p.units) du = p.units - u + g;   // ug(next tile, u = g) - ug(this tile, u)
-                u += 2;
-                aslot += du;
+                // advance to this group's next pair (the next tile's first one after the last)
+                int dp = 2;
+                if (pr + 2 >= npairs) dp = npairs - pr + g;   // pg(next tile, pr = g) - pg(this tile, pr)
+                pr += 2;
+                aslot += dp;
                 while (aslot >= p.a_slots) { aslot -= p.a_slots; aph ^= 1u; }
             }
+            PUBLISH_PREV();   // the tile's last K-step
             __syncwarp();
             if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));
             sslot += 4;
             if (sslot >= S) { sslot -= S; sph ^= 1u; }
         }
+#undef PUBLISH_PREV
     }
 
     // ------------------------------------------------------------------ teardown
@@ -551,9 +610,9 @@ int plan_build_v2(melt_plan *p) {
     if (sigma > 1) return MELT_OK;
     p->v2_sigma = sigma;
     k.acc_cols = 2 * k.nb;
-    k.acc_stages = (2 * k.acc_cols + 4 * k.unit_cols <= 512) ? 2 : 1;
+    k.acc_stages = (2 * k.acc_cols + 6 * k.unit_cols <= 512) ? 2 : 1;
     k.a_col0 = k.acc_stages * k.acc_cols;
-    k.a_slots = std::min(V2_MAX_A_SLOTS, (512 - k.a_col0) / k.unit_cols);
+    k.a_slots = std::min(V2_MAX_A_SLOTS, (512 - k.a_col0) / (2 * k.unit_cols));   // a slot holds a pair of K-steps
     if (k.a_slots < 2) return MELT_OK;
     k.rows_per_chunk = 32 + (N - 1) / H;
     if (k.rows_per_chunk > 64) return MELT_OK;
@@ -701,8 +760,22 @@ static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
         MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
         attr_done = true;
     }
-    melt_fwd2_kernel<PREC, SIGMA><<<grid, V2_THREADS, kp.smem_bytes, stream>>>(kp);
-    MELT_CUDA(cudaGetLastError());
+    // Programmatic dependent launch: when the previous operation in the stream is another forward of this library, the
+    // CTAs of this grid are dispatched as soon as SMs of the previous grid free up (its clusters finish at different
+    // times: 384 tiles on 74 pairs), instead of after its last CTA has retired and a fresh launch has ramped up.  The
+    // kernel orders itself behind the previous grid (griddepcontrol.wait) before its first global store; it reads only
+    // the caller's signal and the plan's tables before that.  Any other predecessor serialises as usual.
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid, 1, 1);
+    cfg.blockDim = dim3(V2_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = kp.smem_bytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA>, kp));
     return MELT_OK;
 }
 

@@ -298,6 +298,7 @@ extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window
     p->in_scale_log2 = 12; p->output = MELT_OUTPUT_LOG; p->used = false; p->device = dev; p->sm_count = prop.multiProcessorCount;
     p->d_bimg = nullptr; p->d_bimg2 = nullptr; p->v2_ok = false; p->v2_sigma = 0; p->d_tab = nullptr; p->d_dct = nullptr; p->d_tile_prefix = nullptr; p->d_frame_offsets_scratch = nullptr;
     memset(&p->kp, 0, sizeof(p->kp));
+    p->ws_in = nullptr; p->ws_out = nullptr; p->ws_in_bytes = p->ws_out_bytes = 0;
     // Eq. (1)-(2): M centres uniformly spaced in mel between fmin and fmax, endpoints excluded
     p->centres.resize(n_mels);
     const double mlo = hz_to_mel(fmin), mhi = hz_to_mel(fmax);
@@ -318,6 +319,8 @@ extern "C" void melt_plan_destroy(melt_plan *p) {
     if (!p) return;
     free_device(p);
     cudaFree(p->d_tile_prefix);
+    cudaFree(p->ws_in);
+    cudaFree(p->ws_out);
     delete p;
 }
 
@@ -363,6 +366,33 @@ extern "C" const char *melt_plan_describe(const melt_plan *p) { return p ? p->de
 
 extern "C" int melt_forward(const melt_plan *p, const float *x, int batch, long long len, float *out, void *stream) {
     return forward_impl(p, x, nullptr, batch, len, out, nullptr, nullptr, stream);
+}
+extern "C" int melt_forward_host(melt_plan *p, const float *x_host, int batch, long long len, float *out_host, void *stream) {
+    if (!p) return fail(MELT_ERR_INVALID_ARG, "plan is NULL");
+    if (batch < 0 || len < 0) return fail(MELT_ERR_INVALID_ARG, "negative batch / len");
+    const long long T = frames_for(p, len);
+    if (batch == 0 || T == 0) return MELT_OK;
+    if (!x_host || !out_host) return fail(MELT_ERR_INVALID_ARG, "x_host / out_host is NULL");
+    const size_t in_bytes = (size_t)batch * (size_t)len * sizeof(float);
+    const size_t out_bytes = (size_t)batch * (size_t)T * (size_t)p->kp.n_ch * sizeof(float);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (in_bytes > p->ws_in_bytes || out_bytes > p->ws_out_bytes) {   // (re)size the plan-owned device workspace: first call / bigger batch only
+        MELT_CUDA(cudaStreamSynchronize(st));
+        cudaFree(p->ws_in); cudaFree(p->ws_out);
+        p->ws_in = nullptr; p->ws_out = nullptr; p->ws_in_bytes = p->ws_out_bytes = 0;
+        if (cudaMalloc(&p->ws_in, in_bytes) != cudaSuccess || cudaMalloc(&p->ws_out, out_bytes) != cudaSuccess) {
+            cudaFree(p->ws_in); cudaFree(p->ws_out);
+            p->ws_in = nullptr; p->ws_out = nullptr;
+            (void)cudaGetLastError();
+            return fail(MELT_ERR_ALLOC, "device workspace of %zu + %zu bytes", in_bytes, out_bytes);
+        }
+        p->ws_in_bytes = in_bytes; p->ws_out_bytes = out_bytes;
+    }
+    MELT_CUDA(cudaMemcpyAsync(p->ws_in, x_host, in_bytes, cudaMemcpyHostToDevice, st));
+    const int rc = forward_impl(p, p->ws_in, nullptr, batch, len, p->ws_out, nullptr, nullptr, stream);
+    if (rc) return rc;
+    MELT_CUDA(cudaMemcpyAsync(out_host, p->ws_out, out_bytes, cudaMemcpyDeviceToHost, st));
+    return MELT_OK;
 }
 extern "C" int melt_forward_ragged(const melt_plan *p, const float *x, const long long *offsets, int n_clips, float *out,
                                    long long *out_frame_offsets, void *stream) {

@@ -110,6 +110,8 @@ struct melt_plan {
     float *d_dct;
     int *d_tile_prefix;
     long long *d_frame_offsets_scratch;
+    float *ws_in, *ws_out;             // device workspace of melt_forward_host (grown on demand)
+    size_t ws_in_bytes, ws_out_bytes;
     std::string desc;
 };
 

@@ -340,3 +340,51 @@ def test_forward_is_asynchronous_on_the_given_stream():
         assert torch.equal(outs[0], outs[1])                                  # deterministic
     finally:
         mb.melt_plan_destroy(plan)
+
+
+def test_forward_host_equals_forward_on_device_buffers():
+    """melt_forward_host (H2D + kernel + D2H inside the C call) returns exactly what melt_forward writes."""
+    import torch
+    from paper_2606_01009_b200 import binding as mb
+    c = _cfg("cfg1")
+    x = _wl().make_inputs("cfg1", 3)["x"]
+    ref = pu.gpu_dense(c, x, "compensated")                       # [B, T, C], computed feature-major on device buffers
+    plan = pu.plan_for(c, "compensated")
+    try:
+        B, L = x.shape
+        T, C = mb.melt_num_frames(plan, L), mb.melt_num_channels(plan)
+        x_pin = torch.from_numpy(x).pin_memory()
+        out_pin = torch.full((B, C, T), float("nan")).pin_memory()
+        stream = torch.cuda.current_stream().cuda_stream
+        for _ in range(2):                                        # second call reuses the plan's workspace
+            mb.melt_forward_host(plan, x_pin, B, L, out_pin, stream)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(out_pin.numpy().transpose(0, 2, 1).astype(np.float64), ref)
+        mb.melt_forward_host(plan, x_pin, 0, L, out_pin, stream)  # empty batch: successful no-op
+    finally:
+        mb.melt_plan_destroy(plan)
+
+
+def test_back_to_back_forwards_into_one_buffer_keep_stream_order():
+    """Consecutive forwards overlap on the device (programmatic dependent launch); the second call's stores must still
+    land after the first call's: two different inputs into the SAME output buffer leave the second result."""
+    import torch
+    from paper_2606_01009_b200 import binding as mb
+    c = _cfg("cfg1")
+    d = _wl().make_inputs("cfg1", 12)["x"]
+    xa, xb = d[:6], d[6:]
+    want = pu.gpu_dense(c, xb, "compensated")
+    plan = pu.plan_for(c, "compensated")
+    try:
+        B, L = xa.shape
+        T, C = mb.melt_num_frames(plan, L), mb.melt_num_channels(plan)
+        ta, tb = torch.from_numpy(xa).cuda(), torch.from_numpy(xb).cuda()
+        out = torch.empty((B, C, T), device="cuda")
+        stream = torch.cuda.current_stream().cuda_stream
+        for _ in range(5):
+            mb.melt_forward(plan, ta, B, L, out, stream)
+            mb.melt_forward(plan, tb, B, L, out, stream)
+        torch.cuda.synchronize()
+        np.testing.assert_array_equal(out.cpu().numpy().transpose(0, 2, 1).astype(np.float64), want)
+    finally:
+        mb.melt_plan_destroy(plan)
