@@ -135,7 +135,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
 
     // ------------------------------------------------------------------ one-time setup
     if (tid == 0) {
-        for (int i = 0; i < V2_MAX_STG; ++i) { mbar_init(BAR(V_STG_FULL + i), 1); mbar_init(BAR(V_STG_EMPTY + i), 2); }
+        for (int i = 0; i < V2_MAX_STG; ++i) { mbar_init(BAR(V_STG_FULL + i), 1); mbar_init(BAR(V_STG_EMPTY + i), V2_CONV_GROUPS); }
         for (int i = 0; i < V2_MAX_A_SLOTS; ++i) { mbar_init(BAR(V_A_FULL + i), 8); mbar_init(BAR(V_A_EMPTY + i), 2); }   // both issuers commit
         for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 2); mbar_init(BAR(V_ACC_EMPTY + i), 8); }
         for (int i = 0; i < V2_MAX_UNITS; ++i) { mbar_init(BAR(V_B_FULL + i), 1); mbar_init(BAR(V_B_PEER + i), 1); }
@@ -178,9 +178,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             const int t0 = (tile - b * p.tiles_per_clip) * 256 + (int)rank * 128;
             const float *xb = p.x + (long long)b * len;
             for (int q = 0; q < 4; ++q) {
-                TRACE(10);
-                mbar_wait(BAR(V_STG_EMPTY + slot), ph ^ 1u);
-                TRACE(11);
                 const long long row0 = (long long)(t0 + 32 * q);
                 const int n_rows = row0 < p.frames_per_clip ? p.rows_per_chunk : 0;
                 long long avail = len - row0 * p.hop;                      // samples of the clip from the chunk's first row on
@@ -189,6 +186,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 const uint32_t total = (uint32_t)(avail < want ? avail : want) * 4u;
                 const uint32_t dst0 = sbase + p.off_stg + (uint32_t)slot * (uint32_t)p.slot_bytes;
                 const bool by_tma = n_rows > 0 && row0 + n_rows <= (long long)p.tma_rows;
+                // The staging ring holds less than two tiles, so the loader usually sits here waiting for a slot: pull the
+                // chunk into L2 meanwhile -- when the slot frees, the copy into shared memory costs an L2 hit, not a DRAM access
+                if (by_tma && elect_one()) tma_prefetch_l2_3d(p.tmap, 0, (int)row0, b);
+                __syncwarp();
+                TRACE(10);
+                mbar_wait(BAR(V_STG_EMPTY + slot), ph ^ 1u);
+                TRACE(11);
                 if (elect_one()) {
                     const uint32_t full = BAR(V_STG_FULL + slot);
 #ifdef MELT_ABL_NOTMA
@@ -200,14 +204,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         // one tensor-map box = the whole chunk: rows_per_chunk hop-rows of pitch width (implicit im2col)
                         mbar_arrive_expect_tx(full, (uint32_t)p.rows_per_chunk * (uint32_t)p.pitch_bytes);
                         tma_load_3d(dst0, p.tmap, 0, (int)row0, b, full);
-                        // The staging ring holds less than two tiles, so the last chunk of the NEXT tile can only be requested
-                        // when this tile ends: pull the tile after next into L2 now, so that request costs an L2 hit, not DRAM
-                        const int ptile = tile + 2 * tile_step;
-                        if (ptile < n_tiles) {
-                            const int pb = ptile / p.tiles_per_clip;
-                            const long long prow = (long long)((ptile - pb * p.tiles_per_clip) * 256 + (int)rank * 128 + 32 * q);
-                            if (prow + p.rows_per_chunk <= (long long)p.tma_rows) tma_prefetch_l2_3d(p.tmap, 0, (int)prow, pb);
-                        }
 #ifdef MELT_ABL_NOTMA
                     } else if (false) {
 #else
@@ -369,21 +365,43 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
 #else
             if (fast_log) {
 #endif
-                // log-Mel, no DCT, no tap: the common case, kept to ~8 instructions per element
+                // log-Mel, no DCT, no tap: the common case.  Whole 16-bin blocks take predicated stores without per-element
+                // bounds tests; the tensor-memory loads of the next block are in flight while this one is computed and stored.
                 float *o = optr;
                 const float off = p.out_log10_offset;
-                for (int c0 = 0; c0 < p.nb; c0 += 16) {
-                    uint32_t vr[16], vi[16];
-                    tmem_ld16(t_r + (uint32_t)c0, vr);
-                    tmem_ld16(t_i + (uint32_t)c0, vi);
+                const int n_whole = p.n_mels & ~15;
+                uint32_t vr[16], vi[16];
+                if (n_whole > 0) { tmem_ld16(t_r, vr); tmem_ld16(t_i, vi); }
+                for (int c0 = 0; c0 < n_whole; c0 += 16) {
+                    float v[16];
                     tmem_wait_ld();
-                    const int nfull = p.n_mels - c0;   // columns of this group that are real Mel bins
 #pragma unroll
                     for (int c = 0; c < 16; ++c) {
                         const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
-                        const float praw = fmaf(r, r, im * im);                                              // Eq. (4)
-                        const float v = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, off), -10.f);                    // Eq. (8), contract form
-                        if (valid && c < nfull) *o = v;
+                        v[c] = fmaf(r, r, im * im);                                                          // Eq. (4)
+                    }
+                    if (c0 + 16 < p.nb) { tmem_ld16(t_r + (uint32_t)(c0 + 16), vr); tmem_ld16(t_i + (uint32_t)(c0 + 16), vi); }
+                    if (valid) {
+#pragma unroll
+                        for (int c = 0; c < 16; ++c) {
+#ifdef MELT_ABL_NOSTG
+                            { const float w = fmaxf(fmaf(lg2_ftz(v[c]), kLog10_2, off), -10.f); if (w == 123.456f) *o = w; }
+#else
+                            *o = fmaxf(fmaf(lg2_ftz(v[c]), kLog10_2, off), -10.f);                           // Eq. (8), contract form
+#endif
+                            o += cstride;
+                        }
+                    }
+                }
+                if (n_whole < p.nb) {   // last, partial block (its loads were issued above, or here when it is the only one)
+                    if (n_whole == 0) { tmem_ld16(t_r, vr); tmem_ld16(t_i, vi); }
+                    tmem_wait_ld();
+                    const int nrem = p.n_mels - n_whole;
+#pragma unroll
+                    for (int c = 0; c < 16; ++c) {
+                        const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                        const float praw = fmaf(r, r, im * im);
+                        if (valid && c < nrem) *o = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, off), -10.f);
                         o += cstride;
                     }
                 }
@@ -431,7 +449,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
         }
     } else if (warp >= W_CONV0) {
-        // ============================================================== converters (thread = frame; two groups alternate K-steps)
+        // ============================================================== converters (thread = frame; the groups take K-step pairs round-robin)
         const int q = warp & 3, g = (warp - W_CONV0) >> 2;
         const uint32_t lane_taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)p.a_col0;
         const uint32_t a_full_remote = mapa_cluster(BAR(V_A_FULL), 0);
@@ -458,7 +476,18 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             mbar_wait(BAR(V_STG_FULL + sslot), sph);
             TRACE(41);
             const uint32_t fb = row_off + (uint32_t)sslot * (uint32_t)p.slot_bytes;
-            int pr = g;   // this group's K-step pairs: g, g + 2, ...
+            bool released = false;
+            // The staged chunk is handed back to the loader as soon as this warp's last K-step of the tile has been read and
+            // folded (its samples are in registers), not after the operand store and its hand-off.
+#define STG_RELEASE_IF_LAST()                                                                       \
+            do {                                                                                    \
+                if (pr + V2_CONV_GROUPS >= npairs && (h == 1 || u + 1 >= p.units)) {                \
+                    __syncwarp();                                                                   \
+                    if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));                           \
+                    released = true;                                                                \
+                }                                                                                   \
+            } while (0)
+            int pr = g;   // this group's K-step pairs: g, g + V2_CONV_GROUPS, ...
             while (pr < npairs) {
 #pragma unroll 1
               for (int h = 0; h < 2; ++h) {
@@ -515,6 +544,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         vdl[c] = *reinterpret_cast<const uint32_t *>(&dl);
                     }
                     TRACE(43);
+                    STG_RELEASE_IF_LAST();
                     if (h == 0) {
                         PUBLISH_PREV();
                         mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
@@ -535,6 +565,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         v[8 + c] = *reinterpret_cast<const uint32_t *>(&dh);
                     }
                     TRACE(43);
+                    STG_RELEASE_IF_LAST();
                     if (h == 0) {
                         PUBLISH_PREV();
                         mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
@@ -550,6 +581,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         v[8 + c] = cvt_tf32_rna(fw[c] - bw[c]);
                     }
                     TRACE(43);
+                    STG_RELEASE_IF_LAST();
                     if (h == 0) {
                         PUBLISH_PREV();
                         mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
@@ -562,19 +594,22 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 pub_slot = aslot;   // published after the NEXT pair's first K-step: the tensor-memory stores complete under it
                 TRACE(45);
                 // advance to this group's next pair (the next tile's first one after the last)
-                int dp = 2;
-                if (pr + 2 >= npairs) dp = npairs - pr + g;   // pg(next tile, pr = g) - pg(this tile, pr)
-                pr += 2;
+                int dp = V2_CONV_GROUPS;
+                if (pr + V2_CONV_GROUPS >= npairs) dp = npairs - pr + g;   // pg(next tile, pr = g) - pg(this tile, pr)
+                pr += V2_CONV_GROUPS;
                 aslot += dp;
                 while (aslot >= p.a_slots) { aslot -= p.a_slots; aph ^= 1u; }
             }
             PUBLISH_PREV();   // the tile's last K-step
-            __syncwarp();
-            if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));
+            if (!released) {   // a group without K-steps in this geometry
+                __syncwarp();
+                if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));
+            }
             sslot += 4;
             if (sslot >= S) { sslot -= S; sph ^= 1u; }
         }
 #undef PUBLISH_PREV
+#undef STG_RELEASE_IF_LAST
     }
 
     // ------------------------------------------------------------------ teardown
@@ -773,8 +808,9 @@ static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
+    static const bool no_pdl = getenv("MELT_NO_PDL") != nullptr;   // debug switch
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = no_pdl ? 0 : 1;
     MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA>, kp));
     return MELT_OK;
 }
