@@ -35,7 +35,7 @@ enum { P2_COMP = 0, P2_TF32 = 1, P2_BF16 = 2 };
 // barrier indices (8 bytes each)
 enum {
     V_STG_FULL = 0, V_STG_EMPTY = V2_MAX_STG, V_A_FULL = 2 * V2_MAX_STG, V_A_EMPTY = V_A_FULL + 16, V_ACC_FULL = V_A_EMPTY + 16,
-    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_NBARS = V_B_PEER + V2_MAX_UNITS
+    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_DONE = V_B_PEER + V2_MAX_UNITS, V_NBARS = V_DONE + 1
 };
 constexpr int V2_MAX_A_SLOTS = 16;
 constexpr int W_LOAD = 0, W_MMA = 1, W_BASIS = 2, W_MMA2 = 3, W_EPI0 = 4, W_CONV0 = 8;
@@ -139,6 +139,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         for (int i = 0; i < V2_MAX_A_SLOTS; ++i) { mbar_init(BAR(V_A_FULL + i), 8); mbar_init(BAR(V_A_EMPTY + i), 2); }   // both issuers commit
         for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 2); mbar_init(BAR(V_ACC_EMPTY + i), 8); }
         for (int i = 0; i < V2_MAX_UNITS; ++i) { mbar_init(BAR(V_B_FULL + i), 1); mbar_init(BAR(V_B_PEER + i), 1); }
+        mbar_init(BAR(V_DONE), 2);   // both MMA issuers
         fence_barrier_init();
     }
     if (warp == W_BASIS) {
@@ -165,7 +166,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     const int n_tiles = p.n_tiles;
     TRACE_DECL
     TRACE(1);
+    // Register budget per role (warpgroup-wide, set at the top of each role's branch): the four service warps and the
+    // epilogue give registers up, the converters (fold + split of 32 operand registers per K-step) take them.
+#define REG_DEC(n) do { if (V2_CONV_GROUPS > 2) asm volatile("setmaxnreg.dec.sync.aligned.u32 " #n ";"); } while (0)
+#define REG_INC(n) do { if (V2_CONV_GROUPS > 2) asm volatile("setmaxnreg.inc.sync.aligned.u32 " #n ";"); } while (0)
 
+    if (warp < W_EPI0) {
+    REG_DEC(40);
     if (warp == W_LOAD) {
         // ============================================================== signal loader (bulk-copy engine)
         // The whole warp runs the (uniform) loop; one elected lane issues the copies.
@@ -250,6 +257,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     if (lane == 0) mbar_arrive_remote(mapa_cluster(BAR(V_B_PEER + u), 0));
                 }
             }
+            mbar_wait(BAR(V_DONE), 0);   // all tensor-core work of the pair, and the barrier arrivals it triggers, are done
         }
     } else if (warp == W_MMA || warp == W_MMA2) {
         // ============================================================== MMA issuers (leader CTA)
@@ -284,45 +292,61 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 uint64_t du = 0;
                 for (int u = 0; u < units; u += 2) {
                     const bool two = u + 1 < units;
+                    int aslot1 = aslot + 1;
+                    uint32_t aph1 = aph;
+                    if (aslot1 == a_slots) { aslot1 = 0; aph1 ^= 1u; }
                     if (basis_pending) {
                         mbar_wait(BAR(V_B_FULL + u), 0); mbar_wait_cluster(BAR(V_B_PEER + u), 0);
                         if (two) { mbar_wait(BAR(V_B_FULL + u + 1), 0); mbar_wait_cluster(BAR(V_B_PEER + u + 1), 0); }
                     }
-                    mbar_wait(BAR(V_A_FULL + aslot), aph);      // one operand slot holds the pair of K-steps
+                    mbar_wait(BAR(V_A_FULL + aslot), aph);
+                    if (two) mbar_wait(BAR(V_A_FULL + aslot1), aph1);
                     TRACE(22);
                     tc_fence_after();
                     if (elect_one()) {
-                        const uint32_t a0 = a_base + (uint32_t)aslot * 2u * unit_cols, a1 = a0 + unit_cols;
+                        const uint32_t a0 = a_base + (uint32_t)aslot * unit_cols, a1 = a_base + (uint32_t)aslot1 * unit_cols;
                         const uint32_t acc = u > 0;
                         if (PREC == P2_COMP) {
                             umma2_ts_f16(d, a0, dsc_hi + du, idesc, acc);          // hi . hi
                             umma2_ts_f16(d, a0 + 8, dsc_hi + du, idesc, 1);        // lo . hi
                             umma2_ts_f16(d, a0, dsc_lo + du, idesc, 1);            // hi . lo
+                            tc_commit2(BAR(V_A_EMPTY + aslot), 3);
                             if (two) {
                                 umma2_ts_f16(d, a1, dsc_hi + du + dstep, idesc, 1);
                                 umma2_ts_f16(d, a1 + 8, dsc_hi + du + dstep, idesc, 1);
                                 umma2_ts_f16(d, a1, dsc_lo + du + dstep, idesc, 1);
+                                tc_commit2(BAR(V_A_EMPTY + aslot1), 3);
                             }
                         } else if (PREC == P2_TF32) {
                             umma2_ts_tf32(d, a0, dsc_hi + du, idesc, acc);
-                            if (two) umma2_ts_tf32(d, a1, dsc_hi + du + dstep, idesc, 1);
+                            tc_commit2(BAR(V_A_EMPTY + aslot), 3);
+                            if (two) { umma2_ts_tf32(d, a1, dsc_hi + du + dstep, idesc, 1); tc_commit2(BAR(V_A_EMPTY + aslot1), 3); }
                         } else {
                             umma2_ts_f16(d, a0, dsc_hi + du, idesc, acc);
-                            if (two) umma2_ts_f16(d, a1, dsc_hi + du + dstep, idesc, 1);
+                            tc_commit2(BAR(V_A_EMPTY + aslot), 3);
+                            if (two) { umma2_ts_f16(d, a1, dsc_hi + du + dstep, idesc, 1); tc_commit2(BAR(V_A_EMPTY + aslot1), 3); }
                         }
-                        tc_commit2(BAR(V_A_EMPTY + aslot), 3);
                         if (u + 2 >= units) tc_commit2(BAR(V_ACC_FULL + stage), 3);
                     }
                     __syncwarp();
                     TRACE(23);
                     du += 2 * dstep;
+                    if (two) { aslot = aslot1; aph = aph1; }
                     if (++aslot == a_slots) { aslot = 0; aph ^= 1u; }
                 }
                 basis_pending = false;
                 if (++stage == acc_stages) { stage = 0; sph ^= 1u; }
             }
+            // Nobody waits for the last operand-slot releases (tcgen05.commit arrivals, multicast to both CTAs).  They must not
+            // land after a CTA has exited and the next grid -- which may start on this SM right away (programmatic dependent
+            // launch) -- has re-initialised the barriers at the same shared-memory addresses: one more commit, behind all the
+            // others, is awaited by both CTAs before they retire.
+            if (elect_one()) tc_commit2(BAR(V_DONE), 3);
+            __syncwarp();
         }
+    }
     } else if (warp >= W_EPI0 && warp < W_EPI0 + 4) {
+        REG_DEC(80);
         // ============================================================== epilogue (thread = frame)
         const int q = warp & 3;
         const int row = q * 32 + lane;
@@ -449,6 +473,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
         }
     } else if (warp >= W_CONV0) {
+        REG_INC(112);
         // ============================================================== converters (thread = frame; the groups take K-step pairs round-robin)
         const int q = warp & 3, g = (warp - W_CONV0) >> 2;
         const uint32_t lane_taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)p.a_col0;
@@ -459,18 +484,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         uint32_t sph = 0;
         int aslot = g % p.a_slots;               // ring position of unit counter ug = it * units + u, first u = g
         uint32_t aph = (uint32_t)((g / p.a_slots) & 1);
-        const int npairs = (p.units + 1) >> 1;   // one operand slot = a PAIR of K-steps: every hand-off cost is paid per pair
-        int pub_slot = -1;                       // operand slot written (tcgen05.st issued) but not yet handed to the MMA issuers
-#define PUBLISH_PREV()                                                                              \
-        do {                                                                                        \
-            if (pub_slot >= 0) {                                                                    \
-                tmem_wait_st();                                                                     \
-                tc_fence_before();                                                                  \
-                __syncwarp();                                                                       \
-                if (lane == 0) mbar_arrive_remote(a_full_remote + (uint32_t)pub_slot * 8u);         \
-                pub_slot = -1;                                                                      \
-            }                                                                                       \
-        } while (0)
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             TRACE(40);
             mbar_wait(BAR(V_STG_FULL + sslot), sph);
@@ -481,18 +494,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             // folded (its samples are in registers), not after the operand store and its hand-off.
 #define STG_RELEASE_IF_LAST()                                                                       \
             do {                                                                                    \
-                if (pr + V2_CONV_GROUPS >= npairs && (h == 1 || u + 1 >= p.units)) {                \
+                if (u + V2_CONV_GROUPS >= p.units) {                                                \
                     __syncwarp();                                                                   \
                     if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));                           \
                     released = true;                                                                \
                 }                                                                                   \
             } while (0)
-            int pr = g;   // this group's K-step pairs: g, g + V2_CONV_GROUPS, ...
-            while (pr < npairs) {
-#pragma unroll 1
-              for (int h = 0; h < 2; ++h) {
-                const int u = 2 * pr + h;
-                if (u >= p.units) break;
+            int u = g;   // this group's K-steps: g, g + V2_CONV_GROUPS, ...
+            while (u < p.units) {
                 // ---- loads: NQ forward quads, NQ mirrored quads (+ one single when the mirrored run starts at 1 mod 4)
                 TRACE(42);
                 const short *tb = p.tab[u];
@@ -519,7 +528,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     }
                     bw[0] = lds32(fb + (uint32_t)(int)tb[8]);                       // position KS-1 of the run
                 }
-                const uint32_t dst = lane_taddr + (uint32_t)(2 * aslot + h) * (uint32_t)p.unit_cols;
+                const uint32_t dst = lane_taddr + (uint32_t)aslot * (uint32_t)p.unit_cols;
                 if (PREC == P2_COMP) {
                     // packed fp32 arithmetic (FMUL2 / FADD2): two folded pairs per instruction.  The mirrored samples are
                     // scaled one by one, which also puts them in pair order at no cost; scaling by 2^s is exact, so
@@ -545,10 +554,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     }
                     TRACE(43);
                     STG_RELEASE_IF_LAST();
-                    if (h == 0) {
-                        PUBLISH_PREV();
-                        mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
-                    }
+                    mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
                     TRACE(44);
                     tc_fence_after();
                     tmem_st8(dst, vsh);
@@ -566,10 +572,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     }
                     TRACE(43);
                     STG_RELEASE_IF_LAST();
-                    if (h == 0) {
-                        PUBLISH_PREV();
-                        mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
-                    }
+                    mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
                     TRACE(44);
                     tc_fence_after();
                     tmem_st16(dst, v);
@@ -582,25 +585,24 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     }
                     TRACE(43);
                     STG_RELEASE_IF_LAST();
-                    if (h == 0) {
-                        PUBLISH_PREV();
-                        mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
-                    }
+                    mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
                     TRACE(44);
                     tc_fence_after();
                     tmem_st16(dst, v);
                 }
-              }
-                pub_slot = aslot;   // published after the NEXT pair's first K-step: the tensor-memory stores complete under it
+                // hand the slot to the MMA issuers right away: a slot is held only from its store to the end of its MMAs
+                tmem_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_remote(a_full_remote + (uint32_t)aslot * 8u);
                 TRACE(45);
-                // advance to this group's next pair (the next tile's first one after the last)
-                int dp = V2_CONV_GROUPS;
-                if (pr + V2_CONV_GROUPS >= npairs) dp = npairs - pr + g;   // pg(next tile, pr = g) - pg(this tile, pr)
-                pr += V2_CONV_GROUPS;
-                aslot += dp;
+                // advance to this group's next K-step (the next tile's first one after the last)
+                int du = V2_CONV_GROUPS;
+                if (u + V2_CONV_GROUPS >= p.units) du = p.units - u + g;   // ug(next tile, u = g) - ug(this tile, u)
+                u += V2_CONV_GROUPS;
+                aslot += du;
                 while (aslot >= p.a_slots) { aslot -= p.a_slots; aph ^= 1u; }
             }
-            PUBLISH_PREV();   // the tile's last K-step
             if (!released) {   // a group without K-steps in this geometry
                 __syncwarp();
                 if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));
@@ -608,7 +610,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             sslot += 4;
             if (sslot >= S) { sslot -= S; sph ^= 1u; }
         }
-#undef PUBLISH_PREV
 #undef STG_RELEASE_IF_LAST
     }
 
@@ -645,9 +646,9 @@ int plan_build_v2(melt_plan *p) {
     if (sigma > 1) return MELT_OK;
     p->v2_sigma = sigma;
     k.acc_cols = 2 * k.nb;
-    k.acc_stages = (2 * k.acc_cols + 6 * k.unit_cols <= 512) ? 2 : 1;
+    k.acc_stages = (2 * k.acc_cols + 4 * k.unit_cols <= 512) ? 2 : 1;
     k.a_col0 = k.acc_stages * k.acc_cols;
-    k.a_slots = std::min(V2_MAX_A_SLOTS, (512 - k.a_col0) / (2 * k.unit_cols));   // a slot holds a pair of K-steps
+    k.a_slots = std::min(V2_MAX_A_SLOTS, (512 - k.a_col0) / k.unit_cols);
     if (k.a_slots < 2) return MELT_OK;
     k.rows_per_chunk = 32 + (N - 1) / H;
     if (k.rows_per_chunk > 64) return MELT_OK;
