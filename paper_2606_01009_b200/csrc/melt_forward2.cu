@@ -2,23 +2,24 @@
 // PAIRS (thread-block clusters of two SMs, tcgen05.mma.cta_group::2).  A tile is 256 consecutive frames of one clip:
 // CTA r of the pair owns frames [128 r, 128 r + 128) of it (its 128 tensor-memory lanes).
 //
-//   loader warp       raw fp32 signal (global) -> shared-memory staging ring with the bulk-copy engine (cp.async.bulk), one
-//                     copy per hop-row (`hop` samples) at a padded pitch, in chunks of 32 frames (= one tensor-memory
-//                     lane quarter).  Implicit im2col: a sample is fetched from HBM/L2 once per chunk and the 2.5x frame
-//                     overlap is served from shared memory; nothing is staged through registers.
-//   converter warps   thread = frame.  128-bit conflict-free shared loads (row pitch = 4 * odd words), fold of the frame
-//                     about the window centre (x[c+j] +- x[c-j]), split into tensor-core operands (fp16 hi + lo, or
-//                     bf16, or tf32) and ONE tcgen05.st per K-step straight into TENSOR MEMORY: the A operand never
-//                     exists in shared or global memory.
+//   loader warp       raw fp32 signal (global) -> shared-memory staging ring, implicit im2col by the tensor-map engine: one
+//                     cp.async.bulk.tensor box per chunk of 32 frames over a 3-D map of the signal whose row stride (hop) is
+//                     smaller than its row extent, so overlapping frames are never materialised; the chunk is prefetched
+//                     into L2 while the loader waits for a free slot.  Clip tails fall back to one bulk copy per hop-row.
+//   converter warps   2 groups x 4 warps, thread = frame; the groups take K-steps round-robin.  128-bit conflict-free shared
+//                     loads (row pitch = 4 * odd words), fold of the frame about the window centre (x[c+j] +- x[c-j]), split
+//                     into tensor-core operands (fp16 hi + lo, or bf16, or tf32) with packed fp32 arithmetic and tcgen05.st
+//                     straight into TENSOR MEMORY: the A operand never exists in shared or global memory.
 //   basis             each CTA keeps HALF of the folded cos/sin basis (nb/2 Mel rows per operand kind) resident in shared
-//                     memory; the pair's tensor cores read both halves (cta_group::2), which halves the per-SM shared
-//                     bandwidth and footprint of the B operand and leaves room for a deep staging ring.
-//   MMA issuer        one thread of the leader CTA: tcgen05.mma.cta_group::2 kind::f16 / kind::tf32, M = 256 over the
-//                     pair, A from tensor memory, B from shared memory, fp32 accumulators in tensor memory
-//                     (R in columns [0, nb), I in [nb, 2 nb)), double-buffered when they fit.
+//                     memory, one barrier per K-step slab; the pair's tensor cores read both halves (cta_group::2).
+//   MMA issuers       two warps of the leader CTA on different schedulers: one accumulates R (cos rows), the other I (sin
+//                     rows); tcgen05.mma.cta_group::2 kind::f16 / kind::tf32, M = 256 over the pair, A from tensor memory,
+//                     B from shared memory, fp32 accumulators in tensor memory (R in columns [0, nb), I in [nb, 2 nb)),
+//                     double-buffered when they fit.  An iteration covers two K-steps.
 //   epilogue warps    tcgen05.ld -> R^2 + I^2 -> log10(max(., 1e-10)) -> optional DCT-II (fp32 FMA) -> coalesced stores.
 //
-// Hand-offs are mbarriers; cross-CTA ones are remote arrivals (mapa) and multicast tcgen05.commit.
+// Hand-offs are mbarriers; cross-CTA ones are remote arrivals (mapa) and multicast tcgen05.commit.  Consecutive forwards on a
+// stream overlap through programmatic dependent launch (see launch_one).
 #include "melt_plan.h"
 #include "sm100_ptx.cuh"
 
@@ -42,10 +43,6 @@ constexpr int W_LOAD = 0, W_MMA = 1, W_BASIS = 2, W_MMA2 = 3, W_EPI0 = 4, W_CONV
 
 __device__ __forceinline__ float4 lds128(uint32_t addr) {
     float4 v;
-#ifdef MELT_ABL_NOLDS
-    v.x = __uint_as_float(addr); v.y = v.x; v.z = v.x; v.w = v.x;
-    return v;
-#endif
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
 }
@@ -84,12 +81,6 @@ __device__ __forceinline__ uint64_t half2_to_f2(__half2 h) {
     const float2 f = __half22float2(h);
     return f2_pack(f.x, f.y);
 }
-#ifdef MELT_ABL_NOST
-#define tmem_st8(a, v) do { if ((v)[0] == 0x7fc12345u) asm volatile("trap;"); } while (0)
-#endif
-#ifdef MELT_ABL_NOMMA
-#define umma2_ts_f16(...) do { } while (0)
-#endif
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // Optional event trace (development builds only, -DMELT_TRACE): lane 0 of every warp of cluster 0 appends (tag, clock) pairs.
@@ -166,13 +157,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     const int n_tiles = p.n_tiles;
     TRACE_DECL
     TRACE(1);
-    // Register budget per role (warpgroup-wide, set at the top of each role's branch): the four service warps and the
-    // epilogue give registers up, the converters (fold + split of 32 operand registers per K-step) take them.
-#define REG_DEC(n) do { if (V2_CONV_GROUPS > 2) asm volatile("setmaxnreg.dec.sync.aligned.u32 " #n ";"); } while (0)
-#define REG_INC(n) do { if (V2_CONV_GROUPS > 2) asm volatile("setmaxnreg.inc.sync.aligned.u32 " #n ";"); } while (0)
-
-    if (warp < W_EPI0) {
-    REG_DEC(40);
     if (warp == W_LOAD) {
         // ============================================================== signal loader (bulk-copy engine)
         // The whole warp runs the (uniform) loop; one elected lane issues the copies.
@@ -202,20 +186,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 TRACE(11);
                 if (elect_one()) {
                     const uint32_t full = BAR(V_STG_FULL + slot);
-#ifdef MELT_ABL_NOTMA
-                    mbar_arrive(full);
-                    if (false) {
-#else
                     if (by_tma) {
-#endif
                         // one tensor-map box = the whole chunk: rows_per_chunk hop-rows of pitch width (implicit im2col)
                         mbar_arrive_expect_tx(full, (uint32_t)p.rows_per_chunk * (uint32_t)p.pitch_bytes);
                         tma_load_3d(dst0, p.tmap, 0, (int)row0, b, full);
-#ifdef MELT_ABL_NOTMA
-                    } else if (false) {
-#else
                     } else {
-#endif
                         // clip tail (or no tensor map): one bulk copy per hop-row, clipped to the clip
                         if (total) mbar_arrive_expect_tx(full, total);
                         else mbar_arrive(full);
@@ -344,9 +319,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             if (elect_one()) tc_commit2(BAR(V_DONE), 3);
             __syncwarp();
         }
-    }
     } else if (warp >= W_EPI0 && warp < W_EPI0 + 4) {
-        REG_DEC(80);
         // ============================================================== epilogue (thread = frame)
         const int q = warp & 3;
         const int row = q * 32 + lane;
@@ -384,11 +357,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             TRACE(31);
             tc_fence_after();
             const uint32_t t_r = lane_taddr + (uint32_t)stage * (uint32_t)p.acc_cols, t_i = t_r + (uint32_t)p.nb;
-#ifdef MELT_ABL_NOEPI
-            if (false) {
-#else
             if (fast_log) {
-#endif
                 // log-Mel, no DCT, no tap: the common case.  Whole 16-bin blocks take predicated stores without per-element
                 // bounds tests; the tensor-memory loads of the next block are in flight while this one is computed and stored.
                 float *o = optr;
@@ -408,11 +377,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     if (valid) {
 #pragma unroll
                         for (int c = 0; c < 16; ++c) {
-#ifdef MELT_ABL_NOSTG
-                            { const float w = fmaxf(fmaf(lg2_ftz(v[c]), kLog10_2, off), -10.f); if (w == 123.456f) *o = w; }
-#else
                             *o = fmaxf(fmaf(lg2_ftz(v[c]), kLog10_2, off), -10.f);                           // Eq. (8), contract form
-#endif
                             o += cstride;
                         }
                     }
@@ -430,11 +395,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     }
                 }
             } else {
-#ifdef MELT_ABL_NOEPI
-            for (int c0 = 0; c0 < 0; c0 += 16) {
-#else
             for (int c0 = 0; c0 < p.nb; c0 += 16) {
-#endif
                 uint32_t vr[16], vi[16];
                 tmem_ld16(t_r + (uint32_t)c0, vr);
                 tmem_ld16(t_i + (uint32_t)c0, vi);
@@ -473,7 +434,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
         }
     } else if (warp >= W_CONV0) {
-        REG_INC(112);
         // ============================================================== converters (thread = frame; the groups take K-step pairs round-robin)
         const int q = warp & 3, g = (warp - W_CONV0) >> 2;
         const uint32_t lane_taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)p.a_col0;
@@ -537,10 +497,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     const uint64_t S2 = f2_pack(S_in, S_in);
 #pragma unroll
                     for (int c = 0; c < 8; ++c) {
-#ifdef MELT_ABL_NOMATH
-                        vsh[c] = __float_as_uint(fw[2 * c]); vsl[c] = __float_as_uint(bw[2 * c]); vdh[c] = __float_as_uint(fw[2 * c + 1]); vdl[c] = __float_as_uint(bw[2 * c + 1]);
-                        continue;
-#endif
                         const uint64_t t = f2_mul(f2_pack(fw[2 * c], fw[2 * c + 1]), S2);
                         const uint64_t b = f2_pack(bw[2 * c] * S_in, bw[2 * c + 1] * S_in);
                         const uint64_t s = f2_add(t, b), d = f2_sub(t, b);
