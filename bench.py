@@ -111,10 +111,15 @@ def time_oracle(cfg, n_clips_sample, reps):
     kw = dict(fs=c["fs"], n_fft=c["n_fft"], hop=c["hop"], window_kind=c["window"], n_mels=c["n_mels"], fmin=c["fmin"],
               fmax=c["fmax"], n_mfcc=c["n_mfcc"], drop_last=c["drop_last"], want=("L", "C"))
     frames = 0
+    if d.get("offsets") is not None:   # ragged: clips packed back to back
+        off = d["offsets"]
+        clips = [d["x"][off[i]:off[i + 1]] for i in range(len(off) - 1)]
+    else:
+        clips = [d["x"][b] for b in range(d["x"].shape[0])]
     t0 = time.perf_counter()
     for _ in range(reps):
-        for b in range(d["x"].shape[0]):
-            frames += next(iter(orc.forward(d["x"][b], **kw).values())).shape[0]
+        for xc in clips:
+            frames += next(iter(orc.forward(xc, **kw).values())).shape[0]
     dt = time.perf_counter() - t0
     return frames / dt, dt, orc.num_threads(), frames
 
@@ -126,13 +131,13 @@ def run_reference(args):
         return
     cfg = args.workload
     c = wl.CONFIGS[cfg]
-    sample_clips = args.cpu_clips
-    for _ in range(args.warmup):
-        time_oracle(cfg, 1, 1)
+    for _ in range(max(1, args.warmup)):
+        fps0, _, _, fr0 = time_oracle(cfg, 1, 1)
+    # bounded sample: as many clips per step (<= --cpu-clips) as keep the whole K-step run near one minute
+    sample_clips = max(1, min(args.cpu_clips, int(60.0 * fps0 / (max(1, args.steps) * max(1, fr0)))))
     fps, dt, cores, frames = time_oracle(cfg, sample_clips, args.steps)
-    nums = workload_numbers(cfg, sample_clips)
     sample = "%d of %d clips of %s per step (%d frames), fp64 direct sums, OpenMP over frames" % (
-        sample_clips, c["n_clips"], cfg, nums["frames"])
+        sample_clips, c["n_clips"], cfg, frames // max(1, args.steps))
     line = {
         "impl": "reference", "metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
@@ -151,7 +156,7 @@ def main():
     ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=50)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="cfg1", choices=[k for k in wl.CONFIGS if k != "cfg3"])
+    ap.add_argument("--workload", default="cfg1", choices=list(wl.CONFIGS))
     ap.add_argument("--precision", default="compensated", choices=list(PREC_NAMES))
     ap.add_argument("--clips", type=int, default=0, help="clips per GPU (default: the config's)")
     ap.add_argument("--buffer-sets", type=int, default=0, help="rotating input/output sets (default: enough to exceed 2x L2)")
@@ -181,7 +186,8 @@ def main():
     cfg = args.workload
     c = wl.CONFIGS[cfg]
     n_clips = args.clips or c["n_clips"]
-    nums = workload_numbers(cfg, n_clips)
+    ragged = bool(c.get("ragged"))
+    nums = None if ragged else workload_numbers(cfg, n_clips)
     peaks = load_peaks()
 
     # ---- plan
@@ -194,20 +200,42 @@ def main():
     # ---- inputs: same per-clip streams on every rank but rank-shifted seed (weak scaling: every rank owns a full batch)
     data = wl.make_inputs(cfg, n_clips, seed=c["seed"] + 7919 * rank)
     x_host = torch.from_numpy(data["x"])
-    B, L = x_host.shape
-    T, C = mb.melt_num_frames(plan, L), mb.melt_num_channels(plan)
-    assert B * T == nums["frames"] and C == nums["C"], (B, T, C, nums)
-    set_bytes = x_host.numel() * 4 + B * C * T * 4
+    C = mb.melt_num_channels(plan)
+    if ragged:   # configs[3]: clips packed back to back + int64 offsets; packed frame-major output
+        offs = data["offsets"]
+        lens = np.diff(offs)
+        B, L = len(lens), 0
+        frames = int(sum(mb.melt_num_frames(plan, int(v)) for v in lens))
+        T = frames   # rows of the packed output
+        N_, M_, K_ = c["n_fft"], c["n_mels"], c["n_mfcc"]
+        nums = dict(frames=frames, audio_s=float(lens.sum()) / c["fs"], T=T, C=C,
+                    flops=2.0 * frames * 2 * M_ * N_ + 2.0 * frames * M_ * K_,
+                    bytes_in=4.0 * float(lens.sum()), bytes_out=4.0 * frames * C)
+        off_dev = torch.from_numpy(np.ascontiguousarray(offs, np.int64)).cuda()
+        set_bytes = x_host.numel() * 4 + frames * C * 4
+    else:
+        B, L = x_host.shape
+        T = mb.melt_num_frames(plan, L)
+        assert B * T == nums["frames"] and C == nums["C"], (B, T, C, nums)
+        set_bytes = x_host.numel() * 4 + B * C * T * 4
     l2_bytes = torch.cuda.get_device_properties(local).L2_cache_size
     nsets = args.buffer_sets or max(2, int(np.ceil(2.2 * l2_bytes / set_bytes)) + 1)
     xs = [x_host.cuda() if i == 0 else None for i in range(nsets)]
     for i in range(1, nsets):
-        xs[i] = torch.roll(xs[0], shifts=i, dims=0).contiguous()   # same clips, different addresses and order
-    outs = [torch.empty((B, C, T) if c["layout"] == "feature_major" else (B, T, C), device="cuda") for _ in range(nsets)]
+        # same clips at different addresses (dense: also in a different order)
+        xs[i] = xs[0].clone() if ragged else torch.roll(xs[0], shifts=i, dims=0).contiguous()
+    if ragged:
+        outs = [torch.empty((T, C), device="cuda") for _ in range(nsets)]
+        fo = torch.empty(B + 1, dtype=torch.int64, device="cuda")
+    else:
+        outs = [torch.empty((B, C, T) if c["layout"] == "feature_major" else (B, T, C), device="cuda") for _ in range(nsets)]
     stream = torch.cuda.current_stream()
 
     def step(i):
-        mb.melt_forward(plan, xs[i % nsets], B, L, outs[i % nsets], stream.cuda_stream)
+        if ragged:
+            mb.melt_forward_ragged(plan, xs[i % nsets], off_dev, B, outs[i % nsets], fo, stream.cuda_stream)
+        else:
+            mb.melt_forward(plan, xs[i % nsets], B, L, outs[i % nsets], stream.cuda_stream)
 
     def barrier():
         if dist is not None:
@@ -255,7 +283,12 @@ def main():
     e2e_steps = max(3, min(args.steps, 20))
 
     def e2e_step(i):   # the library's host-buffer entry point: H2D copy, the kernel and the D2H copy all inside the C call
-        mb.melt_forward_host(plan, x_pin, B, L, out_pin, stream.cuda_stream)
+        if ragged:     # packed batches have no host entry point: pinned copies around the device call
+            xs[i % nsets].copy_(x_pin, non_blocking=True)
+            step(i)
+            out_pin.copy_(outs[i % nsets], non_blocking=True)
+        else:
+            mb.melt_forward_host(plan, x_pin, B, L, out_pin, stream.cuda_stream)
 
     for i in range(3):
         e2e_step(i)
@@ -326,7 +359,7 @@ def main():
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "frames/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(x_pin.numel() * 4),
                 "d2h_bytes_per_step": int(out_pin.numel() * 4)},
-        "gpu_launches": args.steps,
+        "gpu_launches": args.steps * (2 if ragged else 1),   # ragged: frame-offset scan + forward kernel
         "roofline": roof,
         "cpu_baseline": cpu,
     }

@@ -421,7 +421,7 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) melt_fwd_kernel(const __grid_c
 // ---------------------------------------------------------------------------------------------- ragged prologue
 // frame counts -> exclusive prefix sums of frames (int64, caller's array) and of 128-frame tiles (int32, plan workspace)
 __global__ void __launch_bounds__(1024, 1) ragged_scan_kernel(const KParams p, const long long *offsets, int n_clips,
-                                                             long long *frame_offsets, int *tile_prefix) {
+                                                             long long *frame_offsets, int *tile_prefix, int tile_m) {
     __shared__ long long wf[32];
     __shared__ int wt[32];
     __shared__ long long carry_f;
@@ -435,7 +435,7 @@ __global__ void __launch_bounds__(1024, 1) ragged_scan_kernel(const KParams p, c
         int t = 0;
         if (i < n_clips) {
             f = frames_of(p, offsets[i + 1] - offsets[i]);
-            t = (int)((f + TILE_M - 1) / TILE_M);
+            t = (int)((f + tile_m - 1) / tile_m);
         }
         long long fi = f;
         int tii = t;
@@ -469,8 +469,8 @@ __global__ void __launch_bounds__(1024, 1) ragged_scan_kernel(const KParams p, c
     if (tid == 0) { frame_offsets[n_clips] = carry_f; tile_prefix[n_clips] = carry_t; }
 }
 
-int launch_ragged_scan(const melt_plan *pl, const long long *offsets, int n_clips, long long *frame_offsets, cudaStream_t stream) {
-    ragged_scan_kernel<<<1, 1024, 0, stream>>>(pl->kp, offsets, n_clips, frame_offsets, pl->d_tile_prefix);
+int launch_ragged_scan(const melt_plan *pl, const long long *offsets, int n_clips, long long *frame_offsets, int tile_m, cudaStream_t stream) {
+    ragged_scan_kernel<<<1, 1024, 0, stream>>>(pl->kp, offsets, n_clips, frame_offsets, pl->d_tile_prefix, tile_m);
     MELT_CUDA(cudaGetLastError());
     return MELT_OK;
 }

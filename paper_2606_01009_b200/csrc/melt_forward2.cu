@@ -36,7 +36,7 @@ enum { P2_COMP = 0, P2_TF32 = 1, P2_BF16 = 2 };
 // barrier indices (8 bytes each)
 enum {
     V_STG_FULL = 0, V_STG_EMPTY = V2_MAX_STG, V_A_FULL = 2 * V2_MAX_STG, V_A_EMPTY = V_A_FULL + 16, V_ACC_FULL = V_A_EMPTY + 16,
-    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_DONE = V_B_PEER + V2_MAX_UNITS, V_NBARS = V_DONE + 1
+    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_DONE = V_B_PEER + V2_MAX_UNITS, V_STG_READY = V_DONE + 1, V_NBARS = V_STG_READY + V2_MAX_STG
 };
 constexpr int V2_MAX_A_SLOTS = 16;
 constexpr int W_LOAD = 0, W_MMA = 1, W_BASIS = 2, W_MMA2 = 3, W_EPI0 = 4, W_CONV0 = 8;
@@ -107,6 +107,35 @@ __device__ __forceinline__ void dct_acc2(float (&cacc)[MAX_MFCC], const float *d
     }
 }
 
+// Where a 256-frame tile lives: dense batches by division, ragged ones by binary search in the device-side tile prefix.
+struct Tile2 {
+    int clip, t0;      // clip index, first frame of the tile within the clip
+    long long T;       // frames of the clip
+    long long s0;      // index of the clip's first sample in x
+    long long f0;      // index of the clip's first frame in the (packed or dense) frame order
+};
+__device__ __forceinline__ void get_tile2(const K2Params &p, int tile, Tile2 &ti) {
+    if (p.offsets == nullptr) {
+        const int b = tile / p.tiles_per_clip;
+        ti.clip = b;
+        ti.t0 = (tile - b * p.tiles_per_clip) * 256;
+        ti.T = p.frames_per_clip;
+        ti.s0 = (long long)b * p.len;
+        ti.f0 = (long long)b * p.frames_per_clip;
+    } else {
+        int lo = 0, hi = p.n_clips;   // largest i with tile_prefix[i] <= tile
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (__ldg(p.tile_prefix + mid) <= tile) lo = mid; else hi = mid;
+        }
+        ti.clip = lo;
+        ti.t0 = (tile - __ldg(p.tile_prefix + lo)) * 256;
+        ti.f0 = p.frame_offsets[lo];
+        ti.T = p.frame_offsets[lo + 1] - ti.f0;
+        ti.s0 = __ldg(p.offsets + lo);
+    }
+}
+
 template <int PREC, int SIGMA>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
     extern __shared__ __align__(128) uint8_t smem[];
@@ -125,12 +154,29 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     const int S = p.stg_slots;
 
     // ------------------------------------------------------------------ one-time setup
+    if (tid == 32 && p.tma_rows > 0 && p.offsets == nullptr) {
+        // First thing, before any set-up: pull this CTA's first two tiles into L2.  The staging copies are issued ~1000
+        // cycles from now (after barrier / tensor-memory set-up) and one after the other; with the DRAM accesses of all
+        // chunks started here, in parallel, they cost L2 hits -- the first MMA starts ~1.5 us earlier.
+        const int cid = (int)cluster_id_x(), cstep = (int)cluster_nid_x();
+        for (int k = 0; k < 2; ++k) {
+            const int tile = cid + k * cstep;
+            if (tile >= p.n_tiles) break;
+            const int b = tile / p.tiles_per_clip;
+            const int t0 = (tile - b * p.tiles_per_clip) * 256 + (int)cluster_ctarank() * 128;
+            for (int q = 0; q < 4; ++q) {
+                const long long row0 = (long long)(t0 + 32 * q);
+                if (row0 < p.frames_per_clip && row0 + p.rows_per_chunk <= (long long)p.tma_rows) tma_prefetch_l2_3d(p.tmap, 0, (int)row0, b);
+            }
+        }
+    }
     if (tid == 0) {
         for (int i = 0; i < V2_MAX_STG; ++i) { mbar_init(BAR(V_STG_FULL + i), 1); mbar_init(BAR(V_STG_EMPTY + i), V2_CONV_GROUPS); }
         for (int i = 0; i < V2_MAX_A_SLOTS; ++i) { mbar_init(BAR(V_A_FULL + i), 8); mbar_init(BAR(V_A_EMPTY + i), 2); }   // both issuers commit
         for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 2); mbar_init(BAR(V_ACC_EMPTY + i), 8); }
         for (int i = 0; i < V2_MAX_UNITS; ++i) { mbar_init(BAR(V_B_FULL + i), 1); mbar_init(BAR(V_B_PEER + i), 1); }
         mbar_init(BAR(V_DONE), 2);   // both MMA issuers
+        for (int i = 0; i < V2_MAX_STG; ++i) mbar_init(BAR(V_STG_READY + i), 1);
         fence_barrier_init();
     }
     if (warp == W_BASIS) {
@@ -154,7 +200,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     if (tid == 0) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the next forward may start filling freed SMs
 
     const int first_tile = (int)cluster_id_x(), tile_step = (int)cluster_nid_x();
-    const int n_tiles = p.n_tiles;
+    const int n_tiles = p.offsets ? p.tile_prefix[p.n_clips] : p.n_tiles;   // ragged: counted by the scan kernel
     TRACE_DECL
     TRACE(1);
     if (warp == W_LOAD) {
@@ -164,39 +210,69 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         uint32_t ph = 0;
         const long long len = p.len;
         if (p.tma_rows > 0 && lane == 0) tma_prefetch_desc(p.tmap);
+        const bool ragged = p.offsets != nullptr;
+        const long long total = ragged ? p.offsets[p.n_clips] : 0;   // samples in the packed buffer
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
-            const int b = tile / p.tiles_per_clip;
-            const int t0 = (tile - b * p.tiles_per_clip) * 256 + (int)rank * 128;
-            const float *xb = p.x + (long long)b * len;
+            Tile2 ti;
+            get_tile2(p, tile, ti);
+            const int b = ti.clip;
+            const int t0 = ti.t0 + (int)rank * 128;
+            const float *xb = p.x + ti.s0;
+            const long long clip_len = ragged ? p.offsets[b + 1] - ti.s0 : len;
             for (int q = 0; q < 4; ++q) {
                 const long long row0 = (long long)(t0 + 32 * q);
-                const int n_rows = row0 < p.frames_per_clip ? p.rows_per_chunk : 0;
-                long long avail = len - row0 * p.hop;                      // samples of the clip from the chunk's first row on
+                const int n_rows = row0 < ti.T ? p.rows_per_chunk : 0;
+                long long avail = clip_len - row0 * p.hop;                 // samples of the clip from the chunk's first row on
                 avail = avail < 0 ? 0 : avail;
                 const long long want = (long long)n_rows * p.hop;
-                const uint32_t total = (uint32_t)(avail < want ? avail : want) * 4u;
+                const uint32_t total_b = (uint32_t)(avail < want ? avail : want) * 4u;
                 const uint32_t dst0 = sbase + p.off_stg + (uint32_t)slot * (uint32_t)p.slot_bytes;
-                const bool by_tma = n_rows > 0 && row0 + n_rows <= (long long)p.tma_rows;
+                // ragged: the chunk starts at sample s of the packed buffer = column s % hop of hop-row s / hop of the 2-D map
+                // The tensor-map engine wants the box to start on a 16-byte boundary: it is fetched from the aligned sample below
+                // (clip starts are arbitrary; hop % 4 == 0, so every chunk of a clip has the same misalignment) and the
+                // converter warp that owns the chunk shifts it down by (s0 & 3) words in shared memory.
+                const long long s = (ti.s0 & ~3ll) + row0 * p.hop;
+                const int c0 = ragged ? (int)(s % p.hop) : 0, c1 = ragged ? (int)(s / p.hop) : (int)row0, c2 = ragged ? 0 : b;
+                const bool by_tma = n_rows > 0 && (ragged ? s + (long long)(p.rows_per_chunk - 1) * p.hop + (p.pitch_bytes >> 2) <= total
+                                                          : row0 + n_rows <= (long long)p.tma_rows);
                 // The staging ring holds less than two tiles, so the loader usually sits here waiting for a slot: pull the
                 // chunk into L2 meanwhile -- when the slot frees, the copy into shared memory costs an L2 hit, not a DRAM access
-                if (by_tma && elect_one()) tma_prefetch_l2_3d(p.tmap, 0, (int)row0, b);
+                if (by_tma && elect_one()) tma_prefetch_l2_3d(p.tmap, c0, c1, c2);
                 __syncwarp();
                 TRACE(10);
                 mbar_wait(BAR(V_STG_EMPTY + slot), ph ^ 1u);
                 TRACE(11);
+                if (ragged && !by_tma) {
+                    // the few chunks that reach beyond the packed buffer (end of the last clip), or rows of no valid frame:
+                    // plain bounds-checked loads by the whole warp (the bulk-copy engine needs 16-byte aligned sources)
+                    const int pw = p.pitch_bytes >> 2;
+                    const int n_el = n_rows * pw;
+                    float *dstp = reinterpret_cast<float *>(smem + p.off_stg + (size_t)slot * p.slot_bytes);
+                    for (int idx = lane; idx < n_el; idx += 32) {
+                        const int r = idx / pw;
+                        const long long g = s + (long long)r * p.hop + (idx - r * pw);
+                        dstp[idx] = g < total ? __ldg(p.x + g) : 0.f;
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(BAR(V_STG_FULL + slot));
+                    __syncwarp();
+                    TRACE(12);
+                    if (++slot == S) { slot = 0; ph ^= 1u; }
+                    continue;
+                }
                 if (elect_one()) {
                     const uint32_t full = BAR(V_STG_FULL + slot);
                     if (by_tma) {
                         // one tensor-map box = the whole chunk: rows_per_chunk hop-rows of pitch width (implicit im2col)
                         mbar_arrive_expect_tx(full, (uint32_t)p.rows_per_chunk * (uint32_t)p.pitch_bytes);
-                        tma_load_3d(dst0, p.tmap, 0, (int)row0, b, full);
+                        tma_load_3d(dst0, p.tmap, c0, c1, c2, full);
                     } else {
                         // clip tail (or no tensor map): one bulk copy per hop-row, clipped to the clip
-                        if (total) mbar_arrive_expect_tx(full, total);
+                        if (total_b) mbar_arrive_expect_tx(full, total_b);
                         else mbar_arrive(full);
                         uint32_t dst = dst0;
                         const float *src = xb + row0 * p.hop;
-                        uint32_t left = total;
+                        uint32_t left = total_b;
                         const uint32_t row_bytes = (uint32_t)p.hop * 4u;
                         while (left) {
                             const uint32_t nb = left < row_bytes ? left : row_bytes;
@@ -328,12 +404,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         const float kLog10_2 = 0.30102999566398120f;
         int stage = 0;
         uint32_t sph = 0;
-        const long long T = p.frames_per_clip;
         const bool fast_log = p.n_mfcc == 0 && !p.output_power && p.tap == nullptr;
         bool dep_done = false;
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
-            const int b = tile / p.tiles_per_clip;
-            const int t0 = (tile - b * p.tiles_per_clip) * 256 + (int)rank * 128;
+            Tile2 ti;
+            get_tile2(p, tile, ti);
+            const int b = ti.clip;
+            const int t0 = ti.t0 + (int)rank * 128;
+            const long long T = ti.T;
             const bool valid = (long long)(t0 + row) < T;
             float cacc[MAX_MFCC];
             if (p.n_mfcc > 0) {
@@ -346,9 +424,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 optr = p.out + ((long long)b * p.n_ch) * T + t0 + row;
                 tptr = p.tap ? p.tap + ((long long)b * p.n_mels) * T + t0 + row : nullptr;
                 cstride = T;
-            } else {
-                optr = p.out + ((long long)b * T + t0 + row) * p.n_ch;
-                tptr = p.tap ? p.tap + ((long long)b * T + t0 + row) * p.n_mels : nullptr;
+            } else {   // frame-major; ragged batches: packed, the clip starts at frame ti.f0
+                optr = p.out + (ti.f0 + t0 + row) * p.n_ch;
+                tptr = p.tap ? p.tap + (ti.f0 + t0 + row) * p.n_mels : nullptr;
                 cstride = 1;
             }
             TRACE(30);
@@ -447,6 +525,32 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             TRACE(40);
             mbar_wait(BAR(V_STG_FULL + sslot), sph);
+            if (p.offsets != nullptr) {
+                // ragged: group 0's warp realigns its chunk (see the loader), the other groups wait for it
+                if (g == 0) {
+                    Tile2 ti;
+                    get_tile2(p, tile, ti);
+                    const int dlt = (int)(ti.s0 & 3);
+                    if (dlt) {
+                        float *w = reinterpret_cast<float *>(smem + p.off_stg + (size_t)sslot * p.slot_bytes);
+                        const int n = p.rows_per_chunk * (p.pitch_bytes >> 2) - dlt;
+                        for (int i = lane; i < n; i += 128) {
+                            float v[4];
+#pragma unroll
+                            for (int j = 0; j < 4; ++j) v[j] = (i + 32 * j < n) ? w[i + 32 * j + dlt] : 0.f;
+                            __syncwarp();   // every lane has read before any lane overwrites (lane l writes what lane l - dlt read)
+#pragma unroll
+                            for (int j = 0; j < 4; ++j)
+                                if (i + 32 * j < n) w[i + 32 * j] = v[j];
+                            __syncwarp();
+                        }
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(BAR(V_STG_READY + sslot));
+                } else {
+                    mbar_wait(BAR(V_STG_READY + sslot), sph);
+                }
+            }
             TRACE(41);
             const uint32_t fb = row_off + (uint32_t)sslot * (uint32_t)p.slot_bytes;
             bool released = false;
@@ -741,6 +845,31 @@ int v2_encode_tmap(K2Params &k) {
     return MELT_OK;
 }
 
+// Ragged batches: ONE 2-D map over the whole packed buffer, rows of `hop` samples that are (hop + pitch) samples wide, so a
+// box of pitch x rows_per_chunk samples can start at any sample s: column s % hop of row s / hop.  The row count is not
+// known on the host (the offsets live on the device): the map is declared far longer than any buffer and the kernel only
+// requests boxes that lie inside [0, offsets[n_clips]).
+int v2_encode_tmap_ragged(K2Params &k) {
+    k.tma_rows = 0;
+    EncodeTiledFn enc = encode_tiled_fn();
+    const long long W = k.pitch_bytes / 4;
+    if (!enc || W > 256 || k.rows_per_chunk > 256) return MELT_OK;
+    CUtensorMap tm;
+    const cuuint64_t rows = 1ull << 30;
+    const cuuint64_t gdim[3] = {(cuuint64_t)(W + k.hop), rows, 1};
+    const cuuint64_t gstr[2] = {(cuuint64_t)k.hop * 4u, (cuuint64_t)k.hop * 4u * rows};
+    const cuuint32_t box[3] = {(cuuint32_t)W, (cuuint32_t)k.rows_per_chunk, 1u};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    if ((gstr[0] & 15) || gstr[1] >= (1ull << 40)) return MELT_OK;
+    const CUresult r = enc(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float *>(k.x), gdim, gstr, box, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return MELT_OK;   // the general kernel takes the batch
+    memcpy(k.tmap, &tm, 128);
+    k.tma_rows = 1;
+    return MELT_OK;
+}
+
 bool v2_accepts(const melt_plan *p, const float *x, long long len) {
     return p->v2_ok && (((uintptr_t)x & 15) == 0) && ((len & 3) == 0);
 }
@@ -767,14 +896,14 @@ static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     static const bool no_pdl = getenv("MELT_NO_PDL") != nullptr;   // debug switch
     cfg.attrs = attr;
-    cfg.numAttrs = no_pdl ? 0 : 1;
+    cfg.numAttrs = (no_pdl || kp.offsets != nullptr) ? 0 : 1;   // ragged: the scan kernel's results are read at kernel entry
     MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA>, kp));
     return MELT_OK;
 }
 
 int launch_forward2(const melt_plan *pl, const K2Params &kp, cudaStream_t stream) {
     int pairs = pl->sm_count / 2;
-    if (kp.n_tiles < pairs) pairs = kp.n_tiles;
+    if (kp.n_tiles >= 0 && kp.n_tiles < pairs) pairs = kp.n_tiles;   // ragged (n_tiles < 0): counted on the device
     if (pairs < 1) return MELT_OK;
     const int grid = 2 * pairs;
     const int sg = pl->v2_sigma;

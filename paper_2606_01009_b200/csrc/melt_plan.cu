@@ -241,7 +241,17 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
         if (n_clips > MAX_CLIPS) return fail(MELT_ERR_UNSUPPORTED, "n_clips=%d exceeds %d", n_clips, MAX_CLIPS);
         if (!out_frame_offsets) return fail(MELT_ERR_INVALID_ARG, "out_frame_offsets is NULL");
         if (kp.feature_major) return fail(MELT_ERR_UNSUPPORTED, "ragged batches are frame-major only");
-        rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, st);
+        if (p->v2_ok && (((uintptr_t)x & 15) == 0)) {
+            // the CTA-pair kernel: 256-frame tiles, looked up on the device; chunks start at any sample of the packed buffer
+            rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, 256, st);
+            if (rc) return rc;
+            K2Params k2 = p->k2;
+            k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = 0; k2.frames_per_clip = 0;
+            k2.tiles_per_clip = 0; k2.n_tiles = -1;
+            k2.offsets = offsets; k2.frame_offsets = out_frame_offsets; k2.tile_prefix = p->d_tile_prefix;
+            if (v2_encode_tmap_ragged(k2) == MELT_OK && k2.tma_rows > 0) return launch_forward2(p, k2, st);
+        }
+        rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, TILE_M, st);
         if (rc) return rc;
         kp.offsets = offsets; kp.frame_offsets = out_frame_offsets; kp.tile_prefix = p->d_tile_prefix;
         kp.len = 0; kp.frames_per_clip = 0; kp.tiles_per_clip = 0; kp.n_tiles = -1;
@@ -257,6 +267,7 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
             if (tpc2 * n_clips > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
             k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = len; k2.frames_per_clip = T;
             k2.tiles_per_clip = (int)tpc2; k2.n_tiles = (int)(tpc2 * n_clips);
+            k2.offsets = nullptr; k2.frame_offsets = nullptr; k2.tile_prefix = nullptr;
             v2_encode_tmap(k2);
             return launch_forward2(p, k2, st);
         }

@@ -80,6 +80,10 @@ struct K2Params {
     int n_clips;
     long long len, frames_per_clip;
     int tiles_per_clip, n_tiles;  // 256-frame tiles
+    // ---- batch (ragged: clips packed back to back; offsets != nullptr selects this form, frame-major output only)
+    const long long *offsets;        // device sample offsets (n_clips + 1)
+    const long long *frame_offsets;  // device frame offsets (n_clips + 1), written by the scan kernel
+    const int *tile_prefix;          // device exclusive prefix of 256-frame tiles per clip (n_clips + 1)
     // ---- plan-owned device data
     const uint8_t *b_img;  // [b_replicas][2 ranks][units] slabs of unit_b_bytes
     int b_replicas;
@@ -123,6 +127,7 @@ int launch_forward(const melt_plan *p, const KParams &kp, cudaStream_t stream);
 int plan_build_v2(melt_plan *p);   // fills p->k2 / p->v2_ok (never fails the plan: v1 remains the general path)
 bool v2_accepts(const melt_plan *p, const float *x, long long len);
 int launch_forward2(const melt_plan *p, const K2Params &kp, cudaStream_t stream);
-int v2_encode_tmap(K2Params &kp);   // fills kp.tmap / kp.tma_rows for this call's (x, len, batch); never fails the call
-int launch_ragged_scan(const melt_plan *p, const long long *offsets, int n_clips, long long *frame_offsets, cudaStream_t stream);
+int v2_encode_tmap(K2Params &kp);
+int v2_encode_tmap_ragged(K2Params &kp);   // 2-D map over the packed buffer (any start sample, rows of `hop` samples)   // fills kp.tmap / kp.tma_rows for this call's (x, len, batch); never fails the call
+int launch_ragged_scan(const melt_plan *p, const long long *offsets, int n_clips, long long *frame_offsets, int tile_m, cudaStream_t stream);
 }  // namespace melt
