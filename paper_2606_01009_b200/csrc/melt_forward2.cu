@@ -95,15 +95,53 @@ __device__ long long *g_melt_trace = nullptr;   // [2 ranks][16 warps][1024] eve
 #define TRACE(tag) do { } while (0)
 #endif
 
+// Epilogue of one tile for one thread (= frame) in the general case: power or log output, optional tap of the log-Mel
+// matrix, optional DCT-II with 4 * KQ accumulators (KQ = 0: no DCT).  Returns after handing the accumulator stage back.
 template <int KQ>
-__device__ __forceinline__ void dct_acc2(float (&cacc)[MAX_MFCC], const float *drow, float v) {
+__device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uint32_t t_i, const float *dct_s, float *optr, float *tptr,
+                                            long long cstride, bool valid, int lane, uint32_t acc_empty_bar) {
+    const float kLog10_2 = 0.30102999566398120f;
+    float cacc[KQ > 0 ? 4 * KQ : 1];
 #pragma unroll
-    for (int q = 0; q < KQ; ++q) {
-        const float4 d = *reinterpret_cast<const float4 *>(drow + 4 * q);
-        cacc[4 * q + 0] = fmaf(d.x, v, cacc[4 * q + 0]);
-        cacc[4 * q + 1] = fmaf(d.y, v, cacc[4 * q + 1]);
-        cacc[4 * q + 2] = fmaf(d.z, v, cacc[4 * q + 2]);
-        cacc[4 * q + 3] = fmaf(d.w, v, cacc[4 * q + 3]);
+    for (int k = 0; k < (KQ > 0 ? 4 * KQ : 1); ++k) cacc[k] = 0.f;
+    for (int c0 = 0; c0 < p.nb; c0 += 16) {
+        uint32_t vr[16], vi[16];
+        tmem_ld16(t_r + (uint32_t)c0, vr);
+        tmem_ld16(t_i + (uint32_t)c0, vi);
+        tmem_wait_ld();
+#pragma unroll
+        for (int c = 0; c < 16; ++c) {
+            const int m = c0 + c;
+            if (m < p.n_mels) {
+                const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                const float praw = fmaf(r, r, im * im);                                          // Eq. (4)
+                float v;
+                if (p.output_power) v = praw * p.out_scale;
+                else v = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, p.out_log10_offset), -10.f);       // Eq. (8), contract form
+                if (KQ > 0) {
+                    const float *drow = dct_s + m * p.dct_pitch;
+#pragma unroll
+                    for (int q4 = 0; q4 < KQ; ++q4) {
+                        const float4 d = *reinterpret_cast<const float4 *>(drow + 4 * q4);
+                        cacc[4 * q4 + 0] = fmaf(d.x, v, cacc[4 * q4 + 0]);
+                        cacc[4 * q4 + 1] = fmaf(d.y, v, cacc[4 * q4 + 1]);
+                        cacc[4 * q4 + 2] = fmaf(d.z, v, cacc[4 * q4 + 2]);
+                        cacc[4 * q4 + 3] = fmaf(d.w, v, cacc[4 * q4 + 3]);
+                    }
+                    if (tptr && valid) tptr[m * cstride] = v;
+                } else if (valid) {
+                    optr[m * cstride] = v;
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive_remote(acc_empty_bar);
+    if (KQ > 0 && valid) {                                                                      // Eq. (9)
+#pragma unroll
+        for (int k = 0; k < 4 * KQ; ++k)
+            if (k < p.n_mfcc) optr[k * cstride] = cacc[k];
     }
 }
 
@@ -413,11 +451,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             const int t0 = ti.t0 + (int)rank * 128;
             const long long T = ti.T;
             const bool valid = (long long)(t0 + row) < T;
-            float cacc[MAX_MFCC];
-            if (p.n_mfcc > 0) {
-#pragma unroll
-                for (int k = 0; k < MAX_MFCC; ++k) cacc[k] = 0.f;
-            }
             float *optr, *tptr;
             long long cstride;
             if (p.feature_major) {
@@ -472,43 +505,17 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         o += cstride;
                     }
                 }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
             } else {
-            for (int c0 = 0; c0 < p.nb; c0 += 16) {
-                uint32_t vr[16], vi[16];
-                tmem_ld16(t_r + (uint32_t)c0, vr);
-                tmem_ld16(t_i + (uint32_t)c0, vi);
-                tmem_wait_ld();
-#pragma unroll
-                for (int c = 0; c < 16; ++c) {
-                    const int m = c0 + c;
-                    if (m < p.n_mels) {
-                        const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
-                        const float praw = fmaf(r, r, im * im);                                          // Eq. (4)
-                        float v;
-                        if (p.output_power) v = praw * p.out_scale;
-                        else v = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, p.out_log10_offset), -10.f);       // Eq. (8), contract form
-                        if (p.n_mfcc > 0) {
-                            const float *drow = dct_s + m * p.dct_pitch;
-                            if (p.dct_pitch <= 16) dct_acc2<4>(cacc, drow, v);
-                            else if (p.dct_pitch <= 40) dct_acc2<10>(cacc, drow, v);
-                            else dct_acc2<16>(cacc, drow, v);
-                            if (tptr && valid) tptr[m * cstride] = v;
-                        } else if (valid) {
-                            optr[m * cstride] = v;
-                        }
-                    }
-                }
+                const uint32_t eb = acc_empty_remote + (uint32_t)stage * 8u;
+                if (p.n_mfcc == 0) epi_generic<0>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb);
+                else if (p.dct_pitch <= 16) epi_generic<4>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb);
+                else if (p.dct_pitch <= 40) epi_generic<10>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb);
+                else epi_generic<16>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb);
             }
-            }
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
             TRACE(32);
-            if (p.n_mfcc > 0 && valid) {                                                                  // Eq. (9)
-#pragma unroll
-                for (int k = 0; k < MAX_MFCC; ++k)
-                    if (k < p.n_mfcc) optr[k * cstride] = cacc[k];
-            }
             if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
         }
     } else if (warp >= W_CONV0) {
