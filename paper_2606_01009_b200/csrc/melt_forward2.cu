@@ -152,8 +152,9 @@ struct Tile2 {
     long long s0;      // index of the clip's first sample in x
     long long f0;      // index of the clip's first frame in the (packed or dense) frame order
 };
+template <bool RAGGED>
 __device__ __forceinline__ void get_tile2(const K2Params &p, int tile, Tile2 &ti) {
-    if (p.offsets == nullptr) {
+    if (!RAGGED) {
         const int b = tile / p.tiles_per_clip;
         ti.clip = b;
         ti.t0 = (tile - b * p.tiles_per_clip) * 256;
@@ -174,7 +175,33 @@ __device__ __forceinline__ void get_tile2(const K2Params &p, int tile, Tile2 &ti
     }
 }
 
-template <int PREC, int SIGMA>
+// Ragged batches: shifts a staged chunk down by (clip offset & 3) words (see the loader).  Out of line on purpose: it runs
+// once per chunk on ragged batches only and must not take registers from the converter loop it is called from.
+__device__ __noinline__ void ragged_realign(const long long *offsets, const int *tile_prefix, int n_clips, int tile, float *w,
+                                            int n_words, int lane) {
+    int lo = 0, hi = n_clips;   // largest i with tile_prefix[i] <= tile
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (__ldg(tile_prefix + mid) <= tile) lo = mid; else hi = mid;
+    }
+    const int dlt = (int)(__ldg(offsets + lo) & 3);
+    if (dlt) {
+        const int n = n_words - dlt;
+        for (int i = lane; i < n; i += 128) {
+            float v[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) v[j] = (i + 32 * j < n) ? w[i + 32 * j + dlt] : 0.f;
+            __syncwarp();   // every lane has read before any lane overwrites (lane l writes what lane l - dlt read)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (i + 32 * j < n) w[i + 32 * j] = v[j];
+            __syncwarp();
+        }
+    }
+    __syncwarp();
+}
+
+template <int PREC, int SIGMA, bool RAGGED>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
     extern __shared__ __align__(128) uint8_t smem[];
     TRACE_CTA(0);
@@ -192,7 +219,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     const int S = p.stg_slots;
 
     // ------------------------------------------------------------------ one-time setup
-    if (tid == 32 && p.tma_rows > 0 && p.offsets == nullptr) {
+    if (!RAGGED && tid == 32 && p.tma_rows > 0) {
         // First thing, before any set-up: pull this CTA's first two tiles into L2.  The staging copies are issued ~1000
         // cycles from now (after barrier / tensor-memory set-up) and one after the other; with the DRAM accesses of all
         // chunks started here, in parallel, they cost L2 hits -- the first MMA starts ~1.5 us earlier.
@@ -238,7 +265,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     if (tid == 0) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the next forward may start filling freed SMs
 
     const int first_tile = (int)cluster_id_x(), tile_step = (int)cluster_nid_x();
-    const int n_tiles = p.offsets ? p.tile_prefix[p.n_clips] : p.n_tiles;   // ragged: counted by the scan kernel
+    const int n_tiles = RAGGED ? p.tile_prefix[p.n_clips] : p.n_tiles;   // ragged: counted by the scan kernel
     TRACE_DECL
     TRACE(1);
     if (warp == W_LOAD) {
@@ -248,11 +275,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         uint32_t ph = 0;
         const long long len = p.len;
         if (p.tma_rows > 0 && lane == 0) tma_prefetch_desc(p.tmap);
-        const bool ragged = p.offsets != nullptr;
+        constexpr bool ragged = RAGGED;
         const long long total = ragged ? p.offsets[p.n_clips] : 0;   // samples in the packed buffer
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             Tile2 ti;
-            get_tile2(p, tile, ti);
+            get_tile2<RAGGED>(p, tile, ti);
             const int b = ti.clip;
             const int t0 = ti.t0 + (int)rank * 128;
             const float *xb = p.x + ti.s0;
@@ -269,10 +296,17 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 // The tensor-map engine wants the box to start on a 16-byte boundary: it is fetched from the aligned sample below
                 // (clip starts are arbitrary; hop % 4 == 0, so every chunk of a clip has the same misalignment) and the
                 // converter warp that owns the chunk shifts it down by (s0 & 3) words in shared memory.
-                const long long s = (ti.s0 & ~3ll) + row0 * p.hop;
-                const int c0 = ragged ? (int)(s % p.hop) : 0, c1 = ragged ? (int)(s / p.hop) : (int)row0, c2 = ragged ? 0 : b;
-                const bool by_tma = n_rows > 0 && (ragged ? s + (long long)(p.rows_per_chunk - 1) * p.hop + (p.pitch_bytes >> 2) <= total
-                                                          : row0 + n_rows <= (long long)p.tma_rows);
+                long long s = 0;
+                int c0 = 0, c1 = (int)row0, c2 = b;
+                bool by_tma;
+                if (!ragged) {
+                    by_tma = n_rows > 0 && row0 + n_rows <= (long long)p.tma_rows;
+                } else {
+                    s = (ti.s0 & ~3ll) + row0 * p.hop;
+                    const long long r = s / p.hop;
+                    c0 = (int)(s - r * p.hop); c1 = (int)r; c2 = 0;
+                    by_tma = n_rows > 0 && s + (long long)(p.rows_per_chunk - 1) * p.hop + (p.pitch_bytes >> 2) <= total;
+                }
                 // The staging ring holds less than two tiles, so the loader usually sits here waiting for a slot: pull the
                 // chunk into L2 meanwhile -- when the slot frees, the copy into shared memory costs an L2 hit, not a DRAM access
                 if (by_tma && elect_one()) tma_prefetch_l2_3d(p.tmap, c0, c1, c2);
@@ -446,7 +480,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         bool dep_done = false;
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             Tile2 ti;
-            get_tile2(p, tile, ti);
+            get_tile2<RAGGED>(p, tile, ti);
             const int b = ti.clip;
             const int t0 = ti.t0 + (int)rank * 128;
             const long long T = ti.T;
@@ -532,27 +566,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             TRACE(40);
             mbar_wait(BAR(V_STG_FULL + sslot), sph);
-            if (p.offsets != nullptr) {
+            if (RAGGED) {   // a template parameter: the dense instantiation must not carry this call in its converter loop
                 // ragged: group 0's warp realigns its chunk (see the loader), the other groups wait for it
                 if (g == 0) {
-                    Tile2 ti;
-                    get_tile2(p, tile, ti);
-                    const int dlt = (int)(ti.s0 & 3);
-                    if (dlt) {
-                        float *w = reinterpret_cast<float *>(smem + p.off_stg + (size_t)sslot * p.slot_bytes);
-                        const int n = p.rows_per_chunk * (p.pitch_bytes >> 2) - dlt;
-                        for (int i = lane; i < n; i += 128) {
-                            float v[4];
-#pragma unroll
-                            for (int j = 0; j < 4; ++j) v[j] = (i + 32 * j < n) ? w[i + 32 * j + dlt] : 0.f;
-                            __syncwarp();   // every lane has read before any lane overwrites (lane l writes what lane l - dlt read)
-#pragma unroll
-                            for (int j = 0; j < 4; ++j)
-                                if (i + 32 * j < n) w[i + 32 * j] = v[j];
-                            __syncwarp();
-                        }
-                    }
-                    __syncwarp();
+                    ragged_realign(p.offsets, p.tile_prefix, p.n_clips, tile,
+                                   reinterpret_cast<float *>(smem + p.off_stg + (size_t)sslot * p.slot_bytes),
+                                   p.rows_per_chunk * (p.pitch_bytes >> 2), lane);
                     if (lane == 0) mbar_arrive(BAR(V_STG_READY + sslot));
                 } else {
                     mbar_wait(BAR(V_STG_READY + sslot), sph);
@@ -881,11 +900,11 @@ bool v2_accepts(const melt_plan *p, const float *x, long long len) {
     return p->v2_ok && (((uintptr_t)x & 15) == 0) && ((len & 3) == 0);
 }
 
-template <int PREC, int SIGMA>
-static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
+template <int PREC, int SIGMA, bool RAGGED>
+static int launch_one_r(const K2Params &kp, int grid, cudaStream_t stream) {
     static bool attr_done = false;
     if (!attr_done) {
-        MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
+        MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA, RAGGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
         attr_done = true;
     }
     // Programmatic dependent launch: when the previous operation in the stream is another forward of this library, the
@@ -904,8 +923,13 @@ static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
     static const bool no_pdl = getenv("MELT_NO_PDL") != nullptr;   // debug switch
     cfg.attrs = attr;
     cfg.numAttrs = (no_pdl || kp.offsets != nullptr) ? 0 : 1;   // ragged: the scan kernel's results are read at kernel entry
-    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA>, kp));
+    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA, RAGGED>, kp));
     return MELT_OK;
+}
+
+template <int PREC, int SIGMA>
+static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
+    return kp.offsets ? launch_one_r<PREC, SIGMA, true>(kp, grid, stream) : launch_one_r<PREC, SIGMA, false>(kp, grid, stream);
 }
 
 int launch_forward2(const melt_plan *pl, const K2Params &kp, cudaStream_t stream) {
