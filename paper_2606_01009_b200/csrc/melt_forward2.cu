@@ -95,6 +95,39 @@ __device__ long long *g_melt_trace = nullptr;   // [2 ranks][16 warps][1024] eve
 #define TRACE(tag) do { } while (0)
 #endif
 
+// Log-Mel epilogue of the 16-bin blocks blk0, blk0 + step, ... of one tile for one thread (= frame).  Used when a tile's
+// accumulator is drained by several warps per lane quarter (single accumulator stage: the MMAs of the next tile cannot
+// start before the drain, so the converter warps take their share of it instead of waiting).
+__device__ __forceinline__ void epi_fast_share(uint32_t t_r, uint32_t t_i, int nb, int n_mels, float *optr, long long cstride,
+                                               bool valid, float off, int blk0, int step) {
+    const float kLog10_2 = 0.30102999566398120f;
+    for (int c0 = 16 * blk0; c0 < nb; c0 += 16 * step) {
+        uint32_t vr[16], vi[16];
+        tmem_ld16(t_r + (uint32_t)c0, vr);
+        tmem_ld16(t_i + (uint32_t)c0, vi);
+        tmem_wait_ld();
+        const int nrem = n_mels - c0;   // bins of this block that exist
+        float *o = optr + (long long)c0 * cstride;
+        if (nrem >= 16) {
+            if (valid) {
+#pragma unroll
+                for (int c = 0; c < 16; ++c) {
+                    const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                    *o = fmaxf(fmaf(lg2_ftz(fmaf(r, r, im * im)), kLog10_2, off), -10.f);   // Eq. (4), Eq. (8) in contract form
+                    o += cstride;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < 16; ++c) {
+                const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                if (valid && c < nrem) *o = fmaxf(fmaf(lg2_ftz(fmaf(r, r, im * im)), kLog10_2, off), -10.f);
+                o += cstride;
+            }
+        }
+    }
+}
+
 // Epilogue of one tile for one thread (= frame) in the general case: power or log output, optional tap of the log-Mel
 // matrix, optional DCT-II with 4 * KQ accumulators (KQ = 0: no DCT).  Returns after handing the accumulator stage back.
 template <int KQ>
@@ -201,7 +234,7 @@ __device__ __noinline__ void ragged_realign(const long long *offsets, const int 
     __syncwarp();
 }
 
-template <int PREC, int SIGMA, bool RAGGED>
+template <int PREC, int SIGMA, bool RAGGED, bool SHARE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
     extern __shared__ __align__(128) uint8_t smem[];
     TRACE_CTA(0);
@@ -238,7 +271,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     if (tid == 0) {
         for (int i = 0; i < V2_MAX_STG; ++i) { mbar_init(BAR(V_STG_FULL + i), 1); mbar_init(BAR(V_STG_EMPTY + i), V2_CONV_GROUPS); }
         for (int i = 0; i < V2_MAX_A_SLOTS; ++i) { mbar_init(BAR(V_A_FULL + i), 8); mbar_init(BAR(V_A_EMPTY + i), 2); }   // both issuers commit
-        for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 2); mbar_init(BAR(V_ACC_EMPTY + i), 8); }
+        for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 2); mbar_init(BAR(V_ACC_EMPTY + i), SHARE ? 8 * (1 + V2_CONV_GROUPS) : 8); }
         for (int i = 0; i < V2_MAX_UNITS; ++i) { mbar_init(BAR(V_B_FULL + i), 1); mbar_init(BAR(V_B_PEER + i), 1); }
         mbar_init(BAR(V_DONE), 2);   // both MMA issuers
         for (int i = 0; i < V2_MAX_STG; ++i) mbar_init(BAR(V_STG_READY + i), 1);
@@ -502,7 +535,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             TRACE(31);
             tc_fence_after();
             const uint32_t t_r = lane_taddr + (uint32_t)stage * (uint32_t)p.acc_cols, t_i = t_r + (uint32_t)p.nb;
-            if (fast_log) {
+            if (SHARE) {
+                // single accumulator stage, log-Mel: this warp drains every third 16-bin block, the two converter warps of the
+                // lane quarter the others
+                epi_fast_share(t_r, t_i, p.nb, p.n_mels, optr, cstride, valid, p.out_log10_offset, 0, 1 + V2_CONV_GROUPS);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
+            } else if (fast_log) {
                 // log-Mel, no DCT, no tap: the common case.  Whole 16-bin blocks take predicated stores without per-element
                 // bounds tests; the tensor-memory loads of the next block are in flight while this one is computed and stored.
                 float *o = optr;
@@ -563,6 +603,32 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         uint32_t sph = 0;
         int aslot = g % p.a_slots;               // ring position of unit counter ug = it * units + u, first u = g
         uint32_t aph = (uint32_t)((g / p.a_slots) & 1);
+        // SHARE (single accumulator stage, log-Mel): this warp also drains its share of the previous tile's accumulator --
+        // after its second K-step of the next tile, so that the MMAs find operands waiting when the drain releases them.
+        int pend_tile = -1;
+        uint32_t dph = 0;
+        bool dep_done = false;
+        const uint32_t acc_empty_remote = mapa_cluster(BAR(V_ACC_EMPTY), 0);
+#define DRAIN_PENDING()                                                                                          \
+        do {                                                                                                     \
+            Tile2 dt;                                                                                            \
+            get_tile2<RAGGED>(p, pend_tile, dt);                                                                 \
+            const int drow = q * 32 + lane, dt0 = dt.t0 + (int)rank * 128;                                       \
+            const bool dvalid = (long long)(dt0 + drow) < dt.T;                                                  \
+            float *doptr = p.feature_major ? p.out + ((long long)dt.clip * p.n_ch) * dt.T + dt0 + drow            \
+                                           : p.out + (dt.f0 + dt0 + drow) * p.n_ch;                              \
+            mbar_wait(BAR(V_ACC_FULL), dph);                                                                     \
+            dph ^= 1u;                                                                                           \
+            if (!dep_done) { asm volatile("griddepcontrol.wait;" ::: "memory"); dep_done = true; }               \
+            tc_fence_after();                                                                                    \
+            const uint32_t dtr = tmem_base + ((uint32_t)(q * 32) << 16);                                         \
+            epi_fast_share(dtr, dtr + (uint32_t)p.nb, p.nb, p.n_mels, doptr, p.feature_major ? dt.T : 1, dvalid, \
+                           p.out_log10_offset, 1 + g, 1 + V2_CONV_GROUPS);                                       \
+            tc_fence_before();                                                                                   \
+            __syncwarp();                                                                                        \
+            if (lane == 0) mbar_arrive_remote(acc_empty_remote);                                                 \
+            pend_tile = -1;                                                                                      \
+        } while (0)
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             TRACE(40);
             mbar_wait(BAR(V_STG_FULL + sslot), sph);
@@ -592,6 +658,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             } while (0)
             int u = g;   // this group's K-steps: g, g + V2_CONV_GROUPS, ...
             while (u < p.units) {
+                if (SHARE && pend_tile >= 0 && u >= g + 2 * V2_CONV_GROUPS) DRAIN_PENDING();
                 // ---- loads: NQ forward quads, NQ mirrored quads (+ one single when the mirrored run starts at 1 mod 4)
                 TRACE(42);
                 const short *tb = p.tab[u];
@@ -695,8 +762,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             }
             sslot += 4;
             if (sslot >= S) { sslot -= S; sph ^= 1u; }
+            if (SHARE) {
+                if (pend_tile >= 0) DRAIN_PENDING();   // short windows: fewer than three K-steps per group
+                pend_tile = tile;
+            }
         }
+        if (SHARE && pend_tile >= 0) DRAIN_PENDING();   // the last tile
 #undef STG_RELEASE_IF_LAST
+#undef DRAIN_PENDING
     }
 
     // ------------------------------------------------------------------ teardown
@@ -900,11 +973,11 @@ bool v2_accepts(const melt_plan *p, const float *x, long long len) {
     return p->v2_ok && (((uintptr_t)x & 15) == 0) && ((len & 3) == 0);
 }
 
-template <int PREC, int SIGMA, bool RAGGED>
+template <int PREC, int SIGMA, bool RAGGED, bool SHARE>
 static int launch_one_r(const K2Params &kp, int grid, cudaStream_t stream) {
     static bool attr_done = false;
     if (!attr_done) {
-        MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA, RAGGED>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
+        MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA, RAGGED, SHARE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
         attr_done = true;
     }
     // Programmatic dependent launch: when the previous operation in the stream is another forward of this library, the
@@ -923,13 +996,16 @@ static int launch_one_r(const K2Params &kp, int grid, cudaStream_t stream) {
     static const bool no_pdl = getenv("MELT_NO_PDL") != nullptr;   // debug switch
     cfg.attrs = attr;
     cfg.numAttrs = (no_pdl || kp.offsets != nullptr) ? 0 : 1;   // ragged: the scan kernel's results are read at kernel entry
-    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA, RAGGED>, kp));
+    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA, RAGGED, SHARE>, kp));
     return MELT_OK;
 }
 
 template <int PREC, int SIGMA>
 static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
-    return kp.offsets ? launch_one_r<PREC, SIGMA, true>(kp, grid, stream) : launch_one_r<PREC, SIGMA, false>(kp, grid, stream);
+    // SHARE: with a single accumulator stage (wide bases) and plain log-Mel output the converter warps help draining
+    const bool share = kp.acc_stages == 1 && kp.n_mfcc == 0 && !kp.output_power && kp.tap == nullptr;
+    if (kp.offsets) return share ? launch_one_r<PREC, SIGMA, true, true>(kp, grid, stream) : launch_one_r<PREC, SIGMA, true, false>(kp, grid, stream);
+    return share ? launch_one_r<PREC, SIGMA, false, true>(kp, grid, stream) : launch_one_r<PREC, SIGMA, false, false>(kp, grid, stream);
 }
 
 int launch_forward2(const melt_plan *pl, const K2Params &kp, cudaStream_t stream) {
