@@ -234,9 +234,17 @@ __device__ __noinline__ void ragged_realign(const long long *offsets, const int 
     __syncwarp();
 }
 
-template <int PREC, int SIGMA, bool RAGGED, bool SHARE>
+template <int PREC, int SIGMA, bool RAGGED, int MODE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
     extern __shared__ __align__(128) uint8_t smem[];
+    // Who drains the accumulators: MODE 0 the four epilogue warps alone; MODE 1 (single accumulator stage, log-Mel) the epilogue
+    // warps and the converter warps together; MODE 2 (log-Mel) there are no epilogue warps -- they form a third converter
+    // group and every converter warp drains a third of the bins of the previous tile.
+    constexpr bool SHARE = MODE != 0;
+    constexpr int NG = MODE == 2 ? V2_CONV_GROUPS + 1 : V2_CONV_GROUPS;   // converter groups
+    constexpr int CONV0 = MODE == 2 ? W_EPI0 : W_CONV0;                   // first converter warp
+    constexpr int DRAINERS = MODE == 2 ? NG : 1 + NG;                     // warps per lane quarter that drain (SHARE)
+    constexpr int DRAIN0 = MODE == 2 ? 0 : 1;                             // block index of converter group 0's share
     TRACE_CTA(0);
     constexpr int KS = (PREC == P2_TF32) ? 8 : 16;  // folded pairs per K-step
     constexpr int NQ = KS / 4;                      // 128-bit loads per direction per K-step
@@ -269,9 +277,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         }
     }
     if (tid == 0) {
-        for (int i = 0; i < V2_MAX_STG; ++i) { mbar_init(BAR(V_STG_FULL + i), 1); mbar_init(BAR(V_STG_EMPTY + i), V2_CONV_GROUPS); }
+        for (int i = 0; i < V2_MAX_STG; ++i) { mbar_init(BAR(V_STG_FULL + i), 1); mbar_init(BAR(V_STG_EMPTY + i), NG); }
         for (int i = 0; i < V2_MAX_A_SLOTS; ++i) { mbar_init(BAR(V_A_FULL + i), 8); mbar_init(BAR(V_A_EMPTY + i), 2); }   // both issuers commit
-        for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 2); mbar_init(BAR(V_ACC_EMPTY + i), SHARE ? 8 * (1 + V2_CONV_GROUPS) : 8); }
+        for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 2); mbar_init(BAR(V_ACC_EMPTY + i), SHARE ? 8 * DRAINERS : 8); }
         for (int i = 0; i < V2_MAX_UNITS; ++i) { mbar_init(BAR(V_B_FULL + i), 1); mbar_init(BAR(V_B_PEER + i), 1); }
         mbar_init(BAR(V_DONE), 2);   // both MMA issuers
         for (int i = 0; i < V2_MAX_STG; ++i) mbar_init(BAR(V_STG_READY + i), 1);
@@ -500,7 +508,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             if (elect_one()) tc_commit2(BAR(V_DONE), 3);
             __syncwarp();
         }
-    } else if (warp >= W_EPI0 && warp < W_EPI0 + 4) {
+    } else if (MODE != 2 && warp >= W_EPI0 && warp < W_EPI0 + 4) {
         // ============================================================== epilogue (thread = frame)
         const int q = warp & 3;
         const int row = q * 32 + lane;
@@ -538,7 +546,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             if (SHARE) {
                 // single accumulator stage, log-Mel: this warp drains every third 16-bin block, the two converter warps of the
                 // lane quarter the others
-                epi_fast_share(t_r, t_i, p.nb, p.n_mels, optr, cstride, valid, p.out_log10_offset, 0, 1 + V2_CONV_GROUPS);
+                epi_fast_share(t_r, t_i, p.nb, p.n_mels, optr, cstride, valid, p.out_log10_offset, 0, DRAINERS);
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
@@ -592,9 +600,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             TRACE(32);
             if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
         }
-    } else if (warp >= W_CONV0) {
+    } else if (warp >= CONV0) {
         // ============================================================== converters (thread = frame; the groups take K-step pairs round-robin)
-        const int q = warp & 3, g = (warp - W_CONV0) >> 2;
+        const int q = warp & 3, g = (warp - CONV0) >> 2;
         const uint32_t lane_taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)p.a_col0;
         const uint32_t a_full_remote = mapa_cluster(BAR(V_A_FULL), 0);
         const uint32_t row_off = sbase + p.off_stg + (uint32_t)lane * (uint32_t)p.pitch_bytes;
@@ -605,7 +613,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         uint32_t aph = (uint32_t)((g / p.a_slots) & 1);
         // SHARE (single accumulator stage, log-Mel): this warp also drains its share of the previous tile's accumulator --
         // after its second K-step of the next tile, so that the MMAs find operands waiting when the drain releases them.
-        int pend_tile = -1;
+        int pend_tile = -1, dstage = 0;
         uint32_t dph = 0;
         bool dep_done = false;
         const uint32_t acc_empty_remote = mapa_cluster(BAR(V_ACC_EMPTY), 0);
@@ -617,16 +625,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             const bool dvalid = (long long)(dt0 + drow) < dt.T;                                                  \
             float *doptr = p.feature_major ? p.out + ((long long)dt.clip * p.n_ch) * dt.T + dt0 + drow            \
                                            : p.out + (dt.f0 + dt0 + drow) * p.n_ch;                              \
-            mbar_wait(BAR(V_ACC_FULL), dph);                                                                     \
-            dph ^= 1u;                                                                                           \
+            mbar_wait(BAR(V_ACC_FULL + dstage), dph);                                                            \
             if (!dep_done) { asm volatile("griddepcontrol.wait;" ::: "memory"); dep_done = true; }               \
             tc_fence_after();                                                                                    \
-            const uint32_t dtr = tmem_base + ((uint32_t)(q * 32) << 16);                                         \
+            const uint32_t dtr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)dstage * (uint32_t)p.acc_cols; \
             epi_fast_share(dtr, dtr + (uint32_t)p.nb, p.nb, p.n_mels, doptr, p.feature_major ? dt.T : 1, dvalid, \
-                           p.out_log10_offset, 1 + g, 1 + V2_CONV_GROUPS);                                       \
+                           p.out_log10_offset, DRAIN0 + g, DRAINERS);                                            \
             tc_fence_before();                                                                                   \
             __syncwarp();                                                                                        \
-            if (lane == 0) mbar_arrive_remote(acc_empty_remote);                                                 \
+            if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)dstage * 8u);                         \
+            if (++dstage == p.acc_stages) { dstage = 0; dph ^= 1u; }                                             \
             pend_tile = -1;                                                                                      \
         } while (0)
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
@@ -650,15 +658,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             // folded (its samples are in registers), not after the operand store and its hand-off.
 #define STG_RELEASE_IF_LAST()                                                                       \
             do {                                                                                    \
-                if (u + V2_CONV_GROUPS >= p.units) {                                                \
+                if (u + NG >= p.units) {                                                            \
                     __syncwarp();                                                                   \
                     if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));                           \
                     released = true;                                                                \
                 }                                                                                   \
             } while (0)
-            int u = g;   // this group's K-steps: g, g + V2_CONV_GROUPS, ...
+            int u = g;   // this group's K-steps: g, g + NG, ...
             while (u < p.units) {
-                if (SHARE && pend_tile >= 0 && u >= g + 2 * V2_CONV_GROUPS) DRAIN_PENDING();
+                if (SHARE && pend_tile >= 0 && u >= g + 2 * NG) DRAIN_PENDING();
                 // ---- loads: NQ forward quads, NQ mirrored quads (+ one single when the mirrored run starts at 1 mod 4)
                 TRACE(42);
                 const short *tb = p.tab[u];
@@ -750,9 +758,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 if (lane == 0) mbar_arrive_remote(a_full_remote + (uint32_t)aslot * 8u);
                 TRACE(45);
                 // advance to this group's next K-step (the next tile's first one after the last)
-                int du = V2_CONV_GROUPS;
-                if (u + V2_CONV_GROUPS >= p.units) du = p.units - u + g;   // ug(next tile, u = g) - ug(this tile, u)
-                u += V2_CONV_GROUPS;
+                int du = NG;
+                if (u + NG >= p.units) du = p.units - u + g;   // ug(next tile, u = g) - ug(this tile, u)
+                u += NG;
                 aslot += du;
                 while (aslot >= p.a_slots) { aslot -= p.a_slots; aph ^= 1u; }
             }
@@ -973,11 +981,11 @@ bool v2_accepts(const melt_plan *p, const float *x, long long len) {
     return p->v2_ok && (((uintptr_t)x & 15) == 0) && ((len & 3) == 0);
 }
 
-template <int PREC, int SIGMA, bool RAGGED, bool SHARE>
+template <int PREC, int SIGMA, bool RAGGED, int MODE>
 static int launch_one_r(const K2Params &kp, int grid, cudaStream_t stream) {
     static bool attr_done = false;
     if (!attr_done) {
-        MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA, RAGGED, SHARE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
+        MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
         attr_done = true;
     }
     // Programmatic dependent launch: when the previous operation in the stream is another forward of this library, the
@@ -996,16 +1004,26 @@ static int launch_one_r(const K2Params &kp, int grid, cudaStream_t stream) {
     static const bool no_pdl = getenv("MELT_NO_PDL") != nullptr;   // debug switch
     cfg.attrs = attr;
     cfg.numAttrs = (no_pdl || kp.offsets != nullptr) ? 0 : 1;   // ragged: the scan kernel's results are read at kernel entry
-    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA, RAGGED, SHARE>, kp));
+    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE>, kp));
     return MELT_OK;
 }
 
 template <int PREC, int SIGMA>
 static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
-    // SHARE: with a single accumulator stage (wide bases) and plain log-Mel output the converter warps help draining
-    const bool share = kp.acc_stages == 1 && kp.n_mfcc == 0 && !kp.output_power && kp.tap == nullptr;
-    if (kp.offsets) return share ? launch_one_r<PREC, SIGMA, true, true>(kp, grid, stream) : launch_one_r<PREC, SIGMA, true, false>(kp, grid, stream);
-    return share ? launch_one_r<PREC, SIGMA, false, true>(kp, grid, stream) : launch_one_r<PREC, SIGMA, false, false>(kp, grid, stream);
+    // Plain log-Mel output: no dedicated epilogue warps, three converter groups that also drain (MODE 2); everything else keeps
+    // the four epilogue warps (MODE 0).  MODE 1 (epilogue + converter warps drain a single-stage accumulator) is kept for tuning.
+    static const int forced = getenv("MELT_V2_MODE") ? atoi(getenv("MELT_V2_MODE")) : -1;   // debug switch
+    const bool plain = kp.n_mfcc == 0 && !kp.output_power && kp.tap == nullptr;
+    int mode = plain ? 2 : 0;
+    if (forced >= 0 && (plain || forced == 0)) mode = (forced == 1 && kp.acc_stages != 1) ? 0 : forced;
+    if (kp.offsets) {
+        if (mode == 2) return launch_one_r<PREC, SIGMA, true, 2>(kp, grid, stream);
+        if (mode == 1) return launch_one_r<PREC, SIGMA, true, 1>(kp, grid, stream);
+        return launch_one_r<PREC, SIGMA, true, 0>(kp, grid, stream);
+    }
+    if (mode == 2) return launch_one_r<PREC, SIGMA, false, 2>(kp, grid, stream);
+    if (mode == 1) return launch_one_r<PREC, SIGMA, false, 1>(kp, grid, stream);
+    return launch_one_r<PREC, SIGMA, false, 0>(kp, grid, stream);
 }
 
 int launch_forward2(const melt_plan *pl, const K2Params &kp, cudaStream_t stream) {
