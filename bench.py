@@ -103,6 +103,63 @@ class ClockSampler:
                 "samples": len(self.sm), "reasons": sorted(self.reasons)}
 
 
+def torch_context(cfg, c, x_dev, steps=20):
+    """Same-box context, NOT the target (north_star): (i) the matched conventional pipeline torch.stft -> |.|^2 -> dense HTK
+    triangular filterbank matmul -> log10 clamp; (ii) the paper-style direct projection x.unfold @ basis^T with TF32 allowed,
+    then square / add / log.  Plain torch library calls on the device-resident batch; ms per batch."""
+    import torch
+    fs, N, H, M = c["fs"], c["n_fft"], c["hop"], c["n_mels"]
+    dev = x_dev.device
+    hz2mel = lambda f: 2595.0 * np.log10(1.0 + f / 700.0)
+    mel2hz = lambda m: 700.0 * (10.0 ** (m / 2595.0) - 1.0)
+    pts = mel2hz(np.linspace(hz2mel(c["fmin"]), hz2mel(c["fmax"]), M + 2))
+    freqs = np.arange(N // 2 + 1) * fs / N
+    fb = np.zeros((M, N // 2 + 1), np.float32)
+    for m in range(M):
+        lo, ce, hi = pts[m], pts[m + 1], pts[m + 2]
+        fb[m] = np.maximum(0.0, np.minimum((freqs - lo) / max(ce - lo, 1e-9), (hi - freqs) / max(hi - ce, 1e-9)))
+    fb_t = torch.from_numpy(fb).to(dev)
+    win = torch.hann_window(N, periodic=True, device=dev)
+    n = np.arange(N)
+    basis = np.concatenate([np.cos(2 * np.pi * np.outer(pts[1:-1], n) / fs), np.sin(2 * np.pi * np.outer(pts[1:-1], n) / fs)]) * \
+        (0.5 - 0.5 * np.cos(2 * np.pi * n / N))
+    basis_t = torch.from_numpy(basis.astype(np.float32)).to(dev)
+
+    def stft_mel():
+        sp = torch.stft(x_dev, N, hop_length=H, window=win, center=False, return_complex=True)
+        return torch.log10(torch.clamp(fb_t @ (sp.real ** 2 + sp.imag ** 2), min=1e-10))
+
+    def unfold_gemm():
+        fr = x_dev.unfold(-1, N, H)
+        y = fr @ basis_t.t()
+        return torch.log10(torch.clamp(y[..., :M] ** 2 + y[..., M:] ** 2, min=1e-10))
+
+    out = {}
+    old = torch.backends.cuda.matmul.allow_tf32
+    torch.backends.cuda.matmul.allow_tf32 = True
+    try:
+        for name, fn in (("torch_stft_mel_ms", stft_mel), ("torch_unfold_matmul_tf32_ms", unfold_gemm)):
+            try:
+                for _ in range(3):
+                    fn()
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for _ in range(steps):
+                    fn()
+                e1.record()
+                torch.cuda.synchronize()
+                out[name] = e0.elapsed_time(e1) / steps
+            except Exception as e:  # noqa: BLE001  (e.g. out of memory on the largest configs)
+                out[name] = None
+                out[name + "_error"] = str(e)[:80]
+                torch.cuda.empty_cache()
+    finally:
+        torch.backends.cuda.matmul.allow_tf32 = old
+    out["note"] = "same-box torch library pipelines on the same device-resident batch; context, not the target"
+    return out
+
+
 def time_oracle(cfg, n_clips_sample, reps):
     """The fp64 oracle as it stands on the host cores, on a bounded sample of the workload (frames/s)."""
     from oracle import melt_oracle as orc
@@ -162,6 +219,7 @@ def main():
     ap.add_argument("--buffer-sets", type=int, default=0, help="rotating input/output sets (default: enough to exceed 2x L2)")
     ap.add_argument("--cpu-clips", type=int, default=8, help="clips in the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-context", action="store_true", help="skip the same-box torch.stft / unfold-matmul context timings")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
         args.warmup = 3
@@ -337,6 +395,9 @@ def main():
         with open(prof) as fh:
             roof["traffic"] = json.load(fh).get("dram_bytes_per_launch")
 
+    context = None
+    if not ragged and not args.no_context:
+        context = torch_context(cfg, c, xs[0])
     cpu = None
     if not args.no_cpu_baseline:
         fps, dt, cores, frames = time_oracle(cfg, args.cpu_clips, 1)      # calibration pass (also warms the OpenMP pool)
@@ -362,6 +423,7 @@ def main():
         "gpu_launches": args.steps * (2 if ragged else 1),   # ragged: frame-offset scan + forward kernel
         "roofline": roof,
         "cpu_baseline": cpu,
+        "context": context,
     }
     print(json.dumps(line))
     mb.melt_plan_destroy(plan)
