@@ -36,7 +36,7 @@ enum { P2_COMP = 0, P2_TF32 = 1, P2_BF16 = 2 };
 // barrier indices (8 bytes each)
 enum {
     V_STG_FULL = 0, V_STG_EMPTY = V2_MAX_STG, V_A_FULL = 2 * V2_MAX_STG, V_A_EMPTY = V_A_FULL + 16, V_ACC_FULL = V_A_EMPTY + 16,
-    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_DONE = V_B_PEER + V2_MAX_UNITS, V_STG_READY = V_DONE + 1, V_NBARS = V_STG_READY + V2_MAX_STG
+    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_DONE = V_B_PEER + V2_MAX_UNITS, V_STG_READY = V_DONE + 1, V_B_EMPTY = V_STG_READY + V2_MAX_STG, V_NBARS = V_B_EMPTY + 8
 };
 constexpr int V2_MAX_A_SLOTS = 16;
 constexpr int W_LOAD = 0, W_MMA = 1, W_BASIS = 2, W_MMA2 = 3, W_EPI0 = 4, W_CONV0 = 8;
@@ -234,7 +234,7 @@ __device__ __noinline__ void ragged_realign(const long long *offsets, const int 
     __syncwarp();
 }
 
-template <int PREC, int SIGMA, bool RAGGED, int MODE>
+template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
     extern __shared__ __align__(128) uint8_t smem[];
     // Who drains the accumulators: MODE 0 the four epilogue warps alone; MODE 1 (single accumulator stage, log-Mel) the epilogue
@@ -280,8 +280,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         for (int i = 0; i < V2_MAX_STG; ++i) { mbar_init(BAR(V_STG_FULL + i), 1); mbar_init(BAR(V_STG_EMPTY + i), NG); }
         for (int i = 0; i < V2_MAX_A_SLOTS; ++i) { mbar_init(BAR(V_A_FULL + i), 8); mbar_init(BAR(V_A_EMPTY + i), 2); }   // both issuers commit
         for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 2); mbar_init(BAR(V_ACC_EMPTY + i), SHARE ? 8 * DRAINERS : 8); }
-        for (int i = 0; i < V2_MAX_UNITS; ++i) { mbar_init(BAR(V_B_FULL + i), 1); mbar_init(BAR(V_B_PEER + i), 1); }
+        for (int i = 0; i < p.b_slots; ++i) { mbar_init(BAR(V_B_FULL + i), 1); mbar_init(BAR(V_B_PEER + i), 1); }   // b_slots = units when resident
         mbar_init(BAR(V_DONE), 2);   // both MMA issuers
+        if (STREAM)
+            for (int i = 0; i < 8; ++i) mbar_init(BAR(V_B_EMPTY + i), 2);   // streamed basis: both issuers release a slab
         for (int i = 0; i < V2_MAX_STG; ++i) mbar_init(BAR(V_STG_READY + i), 1);
         fence_barrier_init();
     }
@@ -403,22 +405,40 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         // ============================================================== basis: this CTA's half, resident
         // One barrier per K-step slab, so that the first tile's MMAs start as soon as the first slabs have landed.
         if (first_tile < n_tiles) {
-            if (elect_one()) {
-                // the image is replicated in global memory: 74 clusters fetching the same lines at once serialise in L2
-                const uint8_t *src = p.b_img + ((size_t)(cluster_id_x() % (uint32_t)p.b_replicas) * 2 + rank) * p.units * p.unit_b_bytes;
-                for (int u = 0; u < p.units; ++u) {
-                    mbar_arrive_expect_tx(BAR(V_B_FULL + u), p.unit_b_bytes);
-                    bulk_g2s(sbase + p.off_b + (uint32_t)u * p.unit_b_bytes, src + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL + u));
+            // the image is replicated in global memory: 74 clusters fetching the same lines at once serialise in L2
+            const uint8_t *src = p.b_img + ((size_t)(cluster_id_x() % (uint32_t)p.b_replicas) * 2 + rank) * p.units * p.unit_b_bytes;
+            if (!STREAM) {   // a template parameter: the resident instantiation carries no streaming code (0.7 us per cfg1 step)
+                if (elect_one()) {
+                    for (int u = 0; u < p.units; ++u) {
+                        mbar_arrive_expect_tx(BAR(V_B_FULL + u), p.unit_b_bytes);
+                        bulk_g2s(sbase + p.off_b + (uint32_t)u * p.unit_b_bytes, src + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL + u));
+                    }
                 }
-            }
-            __syncwarp();
-            if (rank == 1) {  // tell the leader, slab by slab, that the peer half has landed
-                for (int u = 0; u < p.units; ++u) {
-                    mbar_wait(BAR(V_B_FULL + u), 0);
-                    // complete_tx has made the slab visible in this CTA's shared memory; the tensor core of the pair reads
-                    // it through the async proxy, so a plain remote arrival (no cluster-scope fence, which costs ~1000 cycles
-                    // with bulk copies in flight) is the hand-off
-                    if (lane == 0) mbar_arrive_remote(mapa_cluster(BAR(V_B_PEER + u), 0));
+                __syncwarp();
+                if (rank == 1) {  // tell the leader, slab by slab, that the peer half has landed
+                    for (int u = 0; u < p.units; ++u) {
+                        mbar_wait(BAR(V_B_FULL + u), 0);
+                        // complete_tx has made the slab visible in this CTA's shared memory; the tensor core of the pair reads
+                        // it through the async proxy, so a plain remote arrival (no cluster-scope fence, which costs ~1000 cycles
+                        // with bulk copies in flight) is the hand-off
+                        if (lane == 0) mbar_arrive_remote(mapa_cluster(BAR(V_B_PEER + u), 0));
+                    }
+                }
+            } else {
+                // long windows: the K-step slabs of every tile stream from L2 through a ring of b_slots slabs; the issuers
+                // release a slab (multicast tcgen05.commit to both CTAs) when its MMAs have completed
+                int slot = 0;
+                uint32_t ph = 0;
+                for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+                    for (int u = 0; u < p.units; ++u) {
+                        mbar_wait(BAR(V_B_EMPTY + slot), ph ^ 1u);
+                        if (elect_one()) {
+                            mbar_arrive_expect_tx(BAR(V_B_FULL + slot), p.unit_b_bytes);
+                            bulk_g2s(sbase + p.off_b + (uint32_t)slot * p.unit_b_bytes, src + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL + slot));
+                        }
+                        __syncwarp();
+                        if (++slot == p.b_slots) { slot = 0; ph ^= 1u; }
+                    }
                 }
             }
             mbar_wait(BAR(V_DONE), 0);   // all tensor-core work of the pair, and the barrier arrivals it triggers, are done
@@ -430,6 +450,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         // An iteration covers two K-steps: the fixed cost of a hand-off (barrier probe, fence, election, operand set-up) is
         // then paid once per ~480 cycles of tensor work instead of once per ~240, which a warp that shares its scheduler
         // with three busy converter / epilogue warps could not keep up with.
+        if (STREAM && rank == 1 && warp == W_MMA && first_tile < n_tiles) {
+            // streamed basis: this (otherwise idle) warp of the peer CTA tells the leader when a slab of the peer half has landed
+            int slot = 0;
+            uint32_t ph = 0;
+            for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+                for (int u = 0; u < p.units; ++u) {
+                    mbar_wait(BAR(V_B_FULL + slot), ph);
+                    if (lane == 0) mbar_arrive_remote(mapa_cluster(BAR(V_B_PEER + slot), 0));
+                    __syncwarp();
+                    if (++slot == p.b_slots) { slot = 0; ph ^= 1u; }
+                }
+            }
+        }
         if (rank == 0 && first_tile < n_tiles) {
             const int which = warp == W_MMA ? 0 : 1;
             const uint32_t idesc = umma_idesc(PREC == P2_COMP ? UMMA_F16 : (PREC == P2_BF16 ? UMMA_BF16 : UMMA_TF32), (uint32_t)p.nb, 256u);
@@ -448,20 +481,33 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             int aslot = 0, stage = 0;
             uint32_t aph = 0, sph = 0;
             bool basis_pending = true;
+            constexpr bool b_res = !STREAM;
+            const int b_slots = p.b_slots;
+            int bslot = 0;          // streamed basis: ring slot of the next K-step's slab (resident basis: slot = K-step)
+            uint32_t bph = 0;
             for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
                 TRACE(20);
                 mbar_wait(BAR(V_ACC_EMPTY + stage), sph ^ 1u);
                 TRACE(21);
                 const uint32_t d = d_base + (uint32_t)stage * acc_cols;
-                uint64_t du = 0;
-                for (int u = 0; u < units; u += 2) {
+                uint64_t du = 0;   // resident basis: descriptor offset of K-step u
+                for (int u = 0; u < units; u += 2, du += 2 * dstep) {
                     const bool two = u + 1 < units;
                     int aslot1 = aslot + 1;
                     uint32_t aph1 = aph;
                     if (aslot1 == a_slots) { aslot1 = 0; aph1 ^= 1u; }
-                    if (basis_pending) {
-                        mbar_wait(BAR(V_B_FULL + u), 0); mbar_wait_cluster(BAR(V_B_PEER + u), 0);
-                        if (two) { mbar_wait(BAR(V_B_FULL + u + 1), 0); mbar_wait_cluster(BAR(V_B_PEER + u + 1), 0); }
+                    int bs0, bs1;
+                    uint32_t bp0 = 0, bp1 = 0;
+                    if (b_res) {
+                        bs0 = u; bs1 = u + 1;
+                    } else {
+                        bs0 = bslot; bp0 = bph;
+                        bs1 = bslot + 1; bp1 = bph;
+                        if (bs1 == b_slots) { bs1 = 0; bp1 ^= 1u; }
+                    }
+                    if (basis_pending || !b_res) {
+                        mbar_wait(BAR(V_B_FULL + bs0), bp0); mbar_wait_cluster(BAR(V_B_PEER + bs0), bp0);
+                        if (two) { mbar_wait(BAR(V_B_FULL + bs1), bp1); mbar_wait_cluster(BAR(V_B_PEER + bs1), bp1); }
                     }
                     mbar_wait(BAR(V_A_FULL + aslot), aph);
                     if (two) mbar_wait(BAR(V_A_FULL + aslot1), aph1);
@@ -469,32 +515,42 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     tc_fence_after();
                     if (elect_one()) {
                         const uint32_t a0 = a_base + (uint32_t)aslot * unit_cols, a1 = a_base + (uint32_t)aslot1 * unit_cols;
+                        const uint64_t du0 = b_res ? du : (uint64_t)bs0 * dstep, du1 = b_res ? du + dstep : (uint64_t)bs1 * dstep;
                         const uint32_t acc = u > 0;
                         if (PREC == P2_COMP) {
-                            umma2_ts_f16(d, a0, dsc_hi + du, idesc, acc);          // hi . hi
-                            umma2_ts_f16(d, a0 + 8, dsc_hi + du, idesc, 1);        // lo . hi
-                            umma2_ts_f16(d, a0, dsc_lo + du, idesc, 1);            // hi . lo
-                            tc_commit2(BAR(V_A_EMPTY + aslot), 3);
-                            if (two) {
-                                umma2_ts_f16(d, a1, dsc_hi + du + dstep, idesc, 1);
-                                umma2_ts_f16(d, a1 + 8, dsc_hi + du + dstep, idesc, 1);
-                                umma2_ts_f16(d, a1, dsc_lo + du + dstep, idesc, 1);
-                                tc_commit2(BAR(V_A_EMPTY + aslot1), 3);
-                            }
+                            umma2_ts_f16(d, a0, dsc_hi + du0, idesc, acc);          // hi . hi
+                            umma2_ts_f16(d, a0 + 8, dsc_hi + du0, idesc, 1);        // lo . hi
+                            umma2_ts_f16(d, a0, dsc_lo + du0, idesc, 1);            // hi . lo
                         } else if (PREC == P2_TF32) {
-                            umma2_ts_tf32(d, a0, dsc_hi + du, idesc, acc);
-                            tc_commit2(BAR(V_A_EMPTY + aslot), 3);
-                            if (two) { umma2_ts_tf32(d, a1, dsc_hi + du + dstep, idesc, 1); tc_commit2(BAR(V_A_EMPTY + aslot1), 3); }
+                            umma2_ts_tf32(d, a0, dsc_hi + du0, idesc, acc);
                         } else {
-                            umma2_ts_f16(d, a0, dsc_hi + du, idesc, acc);
-                            tc_commit2(BAR(V_A_EMPTY + aslot), 3);
-                            if (two) { umma2_ts_f16(d, a1, dsc_hi + du + dstep, idesc, 1); tc_commit2(BAR(V_A_EMPTY + aslot1), 3); }
+                            umma2_ts_f16(d, a0, dsc_hi + du0, idesc, acc);
+                        }
+                        tc_commit2(BAR(V_A_EMPTY + aslot), 3);
+                        if (!b_res) tc_commit2(BAR(V_B_EMPTY + bs0), 3);
+                        if (two) {
+                            if (PREC == P2_COMP) {
+                                umma2_ts_f16(d, a1, dsc_hi + du1, idesc, 1);
+                                umma2_ts_f16(d, a1 + 8, dsc_hi + du1, idesc, 1);
+                                umma2_ts_f16(d, a1, dsc_lo + du1, idesc, 1);
+                            } else if (PREC == P2_TF32) {
+                                umma2_ts_tf32(d, a1, dsc_hi + du1, idesc, 1);
+                            } else {
+                                umma2_ts_f16(d, a1, dsc_hi + du1, idesc, 1);
+                            }
+                            tc_commit2(BAR(V_A_EMPTY + aslot1), 3);
+                            if (!b_res) tc_commit2(BAR(V_B_EMPTY + bs1), 3);
                         }
                         if (u + 2 >= units) tc_commit2(BAR(V_ACC_FULL + stage), 3);
                     }
                     __syncwarp();
                     TRACE(23);
-                    du += 2 * dstep;
+                    if (!b_res) {
+                        bslot = bs0; bph = bp0;
+                        const int adv = two ? 2 : 1;
+                        for (int k = 0; k < adv; ++k)
+                            if (++bslot == b_slots) { bslot = 0; bph ^= 1u; }
+                    }
                     if (two) { aslot = aslot1; aph = aph1; }
                     if (++aslot == a_slots) { aslot = 0; aph ^= 1u; }
                 }
@@ -829,10 +885,19 @@ int plan_build_v2(melt_plan *p) {
     const uint32_t dct_bytes = p->n_mfcc > 0 ? (uint32_t)(M * k.dct_pitch * 4) : 0;
     const uint32_t bar_bytes = (uint32_t)round_up2(V_NBARS * 8 + 16, 128);
     k.off_b = 0;
-    k.off_stg = (uint32_t)round_up2((int)b_bytes, 128) + 128;  // 128-byte zero guard in front of the ring
-    const long long room = (long long)SMEM_BUDGET - k.off_stg - 128 - dct_bytes - bar_bytes - 256;
-    k.stg_slots = (int)std::min<long long>(room / k.slot_bytes, V2_MAX_STG);
-    if (k.stg_slots < 5) return MELT_OK;
+    // The basis half stays resident when that leaves room for at least five staging slots; otherwise (long windows) its
+    // K-step slabs are streamed from L2 through the deepest ring (<= 8 slabs) that still leaves five slots.
+    k.b_resident = 1; k.b_slots = k.units;
+    for (;;) {
+        const uint32_t ring_bytes = (uint32_t)k.b_slots * k.unit_b_bytes;
+        k.off_stg = (uint32_t)round_up2((int)ring_bytes, 128) + 128;  // 128-byte zero guard in front of the staging ring
+        const long long room = (long long)SMEM_BUDGET - k.off_stg - 128 - dct_bytes - bar_bytes - 256;
+        k.stg_slots = (int)std::min<long long>(room > 0 ? room / k.slot_bytes : 0, V2_MAX_STG);
+        if (k.stg_slots >= 5) break;
+        if (k.b_resident) { k.b_resident = 0; k.b_slots = std::min(8, k.units - 1); }
+        else --k.b_slots;
+        if (k.b_slots < 3) return MELT_OK;
+    }
     k.off_dct = (uint32_t)round_up2((int)(k.off_stg + (uint32_t)k.stg_slots * k.slot_bytes + 128), 128);
     k.off_bar = (uint32_t)round_up2((int)(k.off_dct + dct_bytes), 128);
     k.smem_bytes = k.off_bar + bar_bytes;
@@ -904,9 +969,9 @@ int plan_build_v2(melt_plan *p) {
     char buf[512];
     snprintf(buf, sizeof(buf),
              "melt_b200 v2 (CTA pair, 256-frame tiles) prec=%s fold(a0=%d,b0=%d,kf=%d) kstep=%d units=%d nb=%d tmem(acc=%dx%d,"
-             "a_slots=%d) basis=resident half (%u B/CTA) staging=%d x %d B chunks of 32 frames (pitch %d B) smem=%u B",
+             "a_slots=%d) basis=%s half (%d x %u B/CTA) staging=%d x %d B chunks of 32 frames (pitch %d B) smem=%u B",
              comp ? "fp16x3" : (kind == OP_BF16 ? "bf16" : "tf32"), k1.a0, k1.b0, k1.kf, k.kstep, k.units, k.nb, k.acc_stages,
-             k.acc_cols, k.a_slots, b_bytes, k.stg_slots, k.slot_bytes, k.pitch_bytes, k.smem_bytes);
+             k.acc_cols, k.a_slots, k.b_resident ? "resident" : "streamed", k.b_slots, k.unit_b_bytes, k.stg_slots, k.slot_bytes, k.pitch_bytes, k.smem_bytes);
     p->desc = std::string(buf) + " | general path: " + p->desc;
     return MELT_OK;
 }
@@ -981,11 +1046,11 @@ bool v2_accepts(const melt_plan *p, const float *x, long long len) {
     return p->v2_ok && (((uintptr_t)x & 15) == 0) && ((len & 3) == 0);
 }
 
-template <int PREC, int SIGMA, bool RAGGED, int MODE>
-static int launch_one_r(const K2Params &kp, int grid, cudaStream_t stream) {
+template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM>
+static int launch_one_s(const K2Params &kp, int grid, cudaStream_t stream) {
     static bool attr_done = false;
     if (!attr_done) {
-        MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
+        MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE, STREAM>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
         attr_done = true;
     }
     // Programmatic dependent launch: when the previous operation in the stream is another forward of this library, the
@@ -1004,26 +1069,26 @@ static int launch_one_r(const K2Params &kp, int grid, cudaStream_t stream) {
     static const bool no_pdl = getenv("MELT_NO_PDL") != nullptr;   // debug switch
     cfg.attrs = attr;
     cfg.numAttrs = (no_pdl || kp.offsets != nullptr) ? 0 : 1;   // ragged: the scan kernel's results are read at kernel entry
-    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE>, kp));
+    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE, STREAM>, kp));
     return MELT_OK;
+}
+
+template <int PREC, int SIGMA, bool RAGGED, int MODE>
+static int launch_one_r(const K2Params &kp, int grid, cudaStream_t stream) {
+    return kp.b_resident ? launch_one_s<PREC, SIGMA, RAGGED, MODE, false>(kp, grid, stream)
+                         : launch_one_s<PREC, SIGMA, RAGGED, MODE, true>(kp, grid, stream);
 }
 
 template <int PREC, int SIGMA>
 static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
     // Plain log-Mel output: no dedicated epilogue warps, three converter groups that also drain (MODE 2); everything else keeps
-    // the four epilogue warps (MODE 0).  MODE 1 (epilogue + converter warps drain a single-stage accumulator) is kept for tuning.
-    static const int forced = getenv("MELT_V2_MODE") ? atoi(getenv("MELT_V2_MODE")) : -1;   // debug switch
+    // the four epilogue warps (MODE 0).  (MODE 1, epilogue + converter warps draining a single-stage accumulator, measured the
+    // same as MODE 2 on cfg2 and is not instantiated.)
+    static const int forced = getenv("MELT_V2_MODE") ? atoi(getenv("MELT_V2_MODE")) : -1;   // debug switch: 0 forces the epilogue warps
     const bool plain = kp.n_mfcc == 0 && !kp.output_power && kp.tap == nullptr;
-    int mode = plain ? 2 : 0;
-    if (forced >= 0 && (plain || forced == 0)) mode = (forced == 1 && kp.acc_stages != 1) ? 0 : forced;
-    if (kp.offsets) {
-        if (mode == 2) return launch_one_r<PREC, SIGMA, true, 2>(kp, grid, stream);
-        if (mode == 1) return launch_one_r<PREC, SIGMA, true, 1>(kp, grid, stream);
-        return launch_one_r<PREC, SIGMA, true, 0>(kp, grid, stream);
-    }
-    if (mode == 2) return launch_one_r<PREC, SIGMA, false, 2>(kp, grid, stream);
-    if (mode == 1) return launch_one_r<PREC, SIGMA, false, 1>(kp, grid, stream);
-    return launch_one_r<PREC, SIGMA, false, 0>(kp, grid, stream);
+    const int mode = (plain && forced != 0) ? 2 : 0;
+    if (kp.offsets) return mode == 2 ? launch_one_r<PREC, SIGMA, true, 2>(kp, grid, stream) : launch_one_r<PREC, SIGMA, true, 0>(kp, grid, stream);
+    return mode == 2 ? launch_one_r<PREC, SIGMA, false, 2>(kp, grid, stream) : launch_one_r<PREC, SIGMA, false, 0>(kp, grid, stream);
 }
 
 int launch_forward2(const melt_plan *pl, const K2Params &kp, cudaStream_t stream) {
