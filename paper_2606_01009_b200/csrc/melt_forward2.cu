@@ -46,6 +46,16 @@ __device__ __forceinline__ float4 lds128(uint32_t addr) {
     asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
 }
+__device__ __forceinline__ float4 ldg128(const char *p) {   // read-only path, 16-byte aligned
+    float4 v;
+    asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float ldg32(const char *p) {
+    float v;
+    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ float lds32(uint32_t addr) {
     float v;
     asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
@@ -132,7 +142,7 @@ __device__ __forceinline__ void epi_fast_share(uint32_t t_r, uint32_t t_i, int n
 // matrix, optional DCT-II with 4 * KQ accumulators (KQ = 0: no DCT).  Returns after handing the accumulator stage back.
 template <int KQ>
 __device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uint32_t t_i, const float *dct_s, float *optr, float *tptr,
-                                            long long cstride, bool valid, int lane, uint32_t acc_empty_bar) {
+                                            long long cstride, bool valid, int lane, uint32_t acc_empty_bar, int nm) {
     const float kLog10_2 = 0.30102999566398120f;
     float cacc[KQ > 0 ? 4 * KQ : 1];
 #pragma unroll
@@ -145,7 +155,7 @@ __device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uin
 #pragma unroll
         for (int c = 0; c < 16; ++c) {
             const int m = c0 + c;
-            if (m < p.n_mels) {
+            if (m < nm) {
                 const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
                 const float praw = fmaf(r, r, im * im);                                          // Eq. (4)
                 float v;
@@ -184,9 +194,13 @@ struct Tile2 {
     long long T;       // frames of the clip
     long long s0;      // index of the clip's first sample in x
     long long f0;      // index of the clip's first frame in the (packed or dense) frame order
+    int pass;          // pass over the Mel bins (more than 128 bins: every tile is visited once per pass)
 };
 template <bool RAGGED>
-__device__ __forceinline__ void get_tile2(const K2Params &p, int tile, Tile2 &ti) {
+__device__ __forceinline__ void get_tile2(const K2Params &p, int vtile, Tile2 &ti) {
+    int tile = vtile;
+    ti.pass = 0;
+    if (p.passes > 1) { tile = vtile / p.passes; ti.pass = vtile - tile * p.passes; }
     if (!RAGGED) {
         const int b = tile / p.tiles_per_clip;
         ti.clip = b;
@@ -234,7 +248,7 @@ __device__ __noinline__ void ragged_realign(const long long *offsets, const int 
     __syncwarp();
 }
 
-template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM>
+template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM, bool DIRECT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
     extern __shared__ __align__(128) uint8_t smem[];
     // Who drains the accumulators: MODE 0 the four epilogue warps alone; MODE 1 (single accumulator stage, log-Mel) the epilogue
@@ -260,7 +274,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     const int S = p.stg_slots;
 
     // ------------------------------------------------------------------ one-time setup
-    if (!RAGGED && tid == 32 && p.tma_rows > 0) {
+    if (!RAGGED && !DIRECT && tid == 32 && p.tma_rows > 0 && p.passes == 1) {
         // First thing, before any set-up: pull this CTA's first two tiles into L2.  The staging copies are issued ~1000
         // cycles from now (after barrier / tensor-memory set-up) and one after the other; with the DRAM accesses of all
         // chunks started here, in parallel, they cost L2 hits -- the first MMA starts ~1.5 us earlier.
@@ -308,10 +322,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     if (tid == 0) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the next forward may start filling freed SMs
 
     const int first_tile = (int)cluster_id_x(), tile_step = (int)cluster_nid_x();
-    const int n_tiles = RAGGED ? p.tile_prefix[p.n_clips] : p.n_tiles;   // ragged: counted by the scan kernel
+    const int n_tiles = (RAGGED ? p.tile_prefix[p.n_clips] : p.n_tiles) * p.passes;   // ragged: counted by the scan kernel; one visit per pass over the bins
     TRACE_DECL
     TRACE(1);
-    if (warp == W_LOAD) {
+    if (warp == W_LOAD && DIRECT) {
+        // windows too long for staged 32-frame chunks: the converter threads read their frames straight from global memory
+    } else if (warp == W_LOAD) {
         // ============================================================== signal loader (bulk-copy engine)
         // The whole warp runs the (uniform) loop; one elected lane issues the copies.
         int slot = 0;
@@ -406,7 +422,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         // One barrier per K-step slab, so that the first tile's MMAs start as soon as the first slabs have landed.
         if (first_tile < n_tiles) {
             // the image is replicated in global memory: 74 clusters fetching the same lines at once serialise in L2
-            const uint8_t *src = p.b_img + ((size_t)(cluster_id_x() % (uint32_t)p.b_replicas) * 2 + rank) * p.units * p.unit_b_bytes;
+            const uint8_t *src = p.b_img + ((size_t)(cluster_id_x() % (uint32_t)p.b_replicas) * 2 + rank) * p.passes * p.units * p.unit_b_bytes;
             if (!STREAM) {   // a template parameter: the resident instantiation carries no streaming code (0.7 us per cfg1 step)
                 if (elect_one()) {
                     for (int u = 0; u < p.units; ++u) {
@@ -430,11 +446,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 int slot = 0;
                 uint32_t ph = 0;
                 for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+                    const uint8_t *psrc = src + (size_t)(tile % p.passes) * p.units * p.unit_b_bytes;   // this pass' rows of the basis
                     for (int u = 0; u < p.units; ++u) {
                         mbar_wait(BAR(V_B_EMPTY + slot), ph ^ 1u);
                         if (elect_one()) {
                             mbar_arrive_expect_tx(BAR(V_B_FULL + slot), p.unit_b_bytes);
-                            bulk_g2s(sbase + p.off_b + (uint32_t)slot * p.unit_b_bytes, src + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL + slot));
+                            bulk_g2s(sbase + p.off_b + (uint32_t)slot * p.unit_b_bytes, psrc + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL + slot));
                         }
                         __syncwarp();
                         if (++slot == p.b_slots) { slot = 0; ph ^= 1u; }
@@ -584,13 +601,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             const bool valid = (long long)(t0 + row) < T;
             float *optr, *tptr;
             long long cstride;
+            const int c_off = ti.pass * p.nb;                                   // first bin of this pass
+            const int nm = p.n_mels - c_off < p.nb ? p.n_mels - c_off : p.nb;   // bins of this pass
             if (p.feature_major) {
-                optr = p.out + ((long long)b * p.n_ch) * T + t0 + row;
-                tptr = p.tap ? p.tap + ((long long)b * p.n_mels) * T + t0 + row : nullptr;
+                optr = p.out + ((long long)b * p.n_ch + c_off) * T + t0 + row;
+                tptr = p.tap ? p.tap + ((long long)b * p.n_mels + c_off) * T + t0 + row : nullptr;
                 cstride = T;
             } else {   // frame-major; ragged batches: packed, the clip starts at frame ti.f0
-                optr = p.out + (ti.f0 + t0 + row) * p.n_ch;
-                tptr = p.tap ? p.tap + (ti.f0 + t0 + row) * p.n_mels : nullptr;
+                optr = p.out + (ti.f0 + t0 + row) * p.n_ch + c_off;
+                tptr = p.tap ? p.tap + (ti.f0 + t0 + row) * p.n_mels + c_off : nullptr;
                 cstride = 1;
             }
             TRACE(30);
@@ -602,7 +621,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             if (SHARE) {
                 // single accumulator stage, log-Mel: this warp drains every third 16-bin block, the two converter warps of the
                 // lane quarter the others
-                epi_fast_share(t_r, t_i, p.nb, p.n_mels, optr, cstride, valid, p.out_log10_offset, 0, DRAINERS);
+                epi_fast_share(t_r, t_i, p.nb, nm, optr, cstride, valid, p.out_log10_offset, 0, DRAINERS);
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
@@ -611,7 +630,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 // bounds tests; the tensor-memory loads of the next block are in flight while this one is computed and stored.
                 float *o = optr;
                 const float off = p.out_log10_offset;
-                const int n_whole = p.n_mels & ~15;
+                const int n_whole = nm & ~15;
                 uint32_t vr[16], vi[16];
                 if (n_whole > 0) { tmem_ld16(t_r, vr); tmem_ld16(t_i, vi); }
                 for (int c0 = 0; c0 < n_whole; c0 += 16) {
@@ -634,7 +653,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 if (n_whole < p.nb) {   // last, partial block (its loads were issued above, or here when it is the only one)
                     if (n_whole == 0) { tmem_ld16(t_r, vr); tmem_ld16(t_i, vi); }
                     tmem_wait_ld();
-                    const int nrem = p.n_mels - n_whole;
+                    const int nrem = nm - n_whole;
 #pragma unroll
                     for (int c = 0; c < 16; ++c) {
                         const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
@@ -648,10 +667,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
             } else {
                 const uint32_t eb = acc_empty_remote + (uint32_t)stage * 8u;
-                if (p.n_mfcc == 0) epi_generic<0>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb);
-                else if (p.dct_pitch <= 16) epi_generic<4>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb);
-                else if (p.dct_pitch <= 40) epi_generic<10>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb);
-                else epi_generic<16>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb);
+                if (p.n_mfcc == 0) epi_generic<0>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm);
+                else if (p.dct_pitch <= 16) epi_generic<4>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm);
+                else if (p.dct_pitch <= 40) epi_generic<10>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm);
+                else epi_generic<16>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm);
             }
             TRACE(32);
             if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
@@ -679,13 +698,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             get_tile2<RAGGED>(p, pend_tile, dt);                                                                 \
             const int drow = q * 32 + lane, dt0 = dt.t0 + (int)rank * 128;                                       \
             const bool dvalid = (long long)(dt0 + drow) < dt.T;                                                  \
-            float *doptr = p.feature_major ? p.out + ((long long)dt.clip * p.n_ch) * dt.T + dt0 + drow            \
-                                           : p.out + (dt.f0 + dt0 + drow) * p.n_ch;                              \
+            const int dc_off = dt.pass * p.nb;                                                                   \
+            const int dnm = p.n_mels - dc_off < p.nb ? p.n_mels - dc_off : p.nb;                                 \
+            float *doptr = p.feature_major ? p.out + ((long long)dt.clip * p.n_ch + dc_off) * dt.T + dt0 + drow   \
+                                           : p.out + (dt.f0 + dt0 + drow) * p.n_ch + dc_off;                     \
             mbar_wait(BAR(V_ACC_FULL + dstage), dph);                                                            \
             if (!dep_done) { asm volatile("griddepcontrol.wait;" ::: "memory"); dep_done = true; }               \
             tc_fence_after();                                                                                    \
             const uint32_t dtr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)dstage * (uint32_t)p.acc_cols; \
-            epi_fast_share(dtr, dtr + (uint32_t)p.nb, p.nb, p.n_mels, doptr, p.feature_major ? dt.T : 1, dvalid, \
+            epi_fast_share(dtr, dtr + (uint32_t)p.nb, p.nb, dnm, doptr, p.feature_major ? dt.T : 1, dvalid,      \
                            p.out_log10_offset, DRAIN0 + g, DRAINERS);                                            \
             tc_fence_before();                                                                                   \
             __syncwarp();                                                                                        \
@@ -695,7 +716,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         } while (0)
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             TRACE(40);
-            mbar_wait(BAR(V_STG_FULL + sslot), sph);
+            const char *gxb = nullptr;   // DIRECT: this thread's frame in global memory
+            if (DIRECT) {
+                Tile2 ti;
+                get_tile2<RAGGED>(p, tile, ti);
+                const long long trow = ti.t0 + (int)rank * 128 + q * 32 + lane;
+                gxb = reinterpret_cast<const char *>(p.x + ti.s0 + (trow < ti.T ? trow : 0) * p.hop);   // rows of no frame re-read frame 0
+            } else {
+                mbar_wait(BAR(V_STG_FULL + sslot), sph);
+            }
             if (RAGGED) {   // a template parameter: the dense instantiation must not carry this call in its converter loop
                 // ragged: group 0's warp realigns its chunk (see the loader), the other groups wait for it
                 if (g == 0) {
@@ -714,7 +743,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             // folded (its samples are in registers), not after the operand store and its hand-off.
 #define STG_RELEASE_IF_LAST()                                                                       \
             do {                                                                                    \
-                if (u + NG >= p.units) {                                                            \
+                if (!DIRECT && u + NG >= p.units) {                                                 \
                     __syncwarp();                                                                   \
                     if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));                           \
                     released = true;                                                                \
@@ -729,25 +758,25 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 float fw[KS], bw[KS];
 #pragma unroll
                 for (int i = 0; i < NQ; ++i) {
-                    const float4 f = lds128(fb + (uint32_t)(int)tb[i]);
+                    const float4 f = DIRECT ? ldg128(gxb + (int)tb[i]) : lds128(fb + (uint32_t)(int)tb[i]);
                     fw[4 * i + 0] = f.x; fw[4 * i + 1] = f.y; fw[4 * i + 2] = f.z; fw[4 * i + 3] = f.w;
                 }
                 // mirrored partner of pair e is the sample at position KS-1-e of the descending run
                 if (SIGMA == 0) {
 #pragma unroll
                     for (int i = 0; i < NQ; ++i) {
-                        const float4 f = lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs+4i .. rs+4i+3
+                        const float4 f = DIRECT ? ldg128(gxb + (int)tb[4 + i]) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs+4i .. rs+4i+3
                         bw[KS - 1 - (4 * i + 0)] = f.x; bw[KS - 1 - (4 * i + 1)] = f.y;
                         bw[KS - 1 - (4 * i + 2)] = f.z; bw[KS - 1 - (4 * i + 3)] = f.w;
                     }
                 } else {
 #pragma unroll
                     for (int i = 0; i < NQ; ++i) {
-                        const float4 f = lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs-1+4i .. rs+2+4i
+                        const float4 f = DIRECT ? ldg128(gxb + (int)tb[4 + i]) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs-1+4i .. rs+2+4i
                         if (i > 0) bw[KS - 1 - (4 * i - 1)] = f.x;                  // position 4i-1 of the run
                         bw[KS - 1 - (4 * i + 0)] = f.y; bw[KS - 1 - (4 * i + 1)] = f.z; bw[KS - 1 - (4 * i + 2)] = f.w;
                     }
-                    bw[0] = lds32(fb + (uint32_t)(int)tb[8]);                       // position KS-1 of the run
+                    bw[0] = DIRECT ? ldg32(gxb + (int)tb[8]) : lds32(fb + (uint32_t)(int)tb[8]);   // position KS-1 of the run
                 }
                 const uint32_t dst = lane_taddr + (uint32_t)aslot * (uint32_t)p.unit_cols;
                 if (PREC == P2_COMP) {
@@ -820,7 +849,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 aslot += du;
                 while (aslot >= p.a_slots) { aslot -= p.a_slots; aph ^= 1u; }
             }
-            if (!released) {   // a group without K-steps in this geometry
+            if (!DIRECT && !released) {   // a group without K-steps in this geometry
                 __syncwarp();
                 if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));
             }
@@ -860,10 +889,12 @@ int plan_build_v2(melt_plan *p) {
     k.units = (k1.kf + k.kstep - 1) / k.kstep;
     k.nk = comp ? 4 : 2;
     k.unit_cols = k.nk * 8;
-    k.nb = round_up2(M, 16);
+    k.passes = (M + 127) / 128;                                   // more than 128 bins: several passes, each tile visited once per pass
+    k.nb = round_up2((M + k.passes - 1) / k.passes, 16);
     if (k.nb < 32) k.nb = 32;
     // ---- what the kernel covers (everything else stays on the general v1 kernel)
-    if (M > 128 || k.units > V2_MAX_UNITS || (H & 3) || (k1.a0 & 3) || p->pad != MELT_PAD_NONE) return MELT_OK;
+    if (k.units > V2_MAX_UNITS || (H & 3) || (k1.a0 & 3) || p->pad != MELT_PAD_NONE) return MELT_OK;
+    if (k.passes > 1 && p->n_mfcc > 0) return MELT_OK;             // the DCT needs all bins of a frame in one pass
     const int rs = k1.b0 - (k.kstep - 1);           // lowest sample of the mirrored run of unit 0
     const int sigma = ((rs % 4) + 4) % 4;
     if (sigma > 1) return MELT_OK;
@@ -888,6 +919,7 @@ int plan_build_v2(melt_plan *p) {
     // The basis half stays resident when that leaves room for at least five staging slots; otherwise (long windows) its
     // K-step slabs are streamed from L2 through the deepest ring (<= 8 slabs) that still leaves five slots.
     k.b_resident = 1; k.b_slots = k.units;
+    if (k.passes > 1) { k.b_resident = 0; k.b_slots = std::min(8, k.units - 1); }   // every pass needs other rows: streamed
     for (;;) {
         const uint32_t ring_bytes = (uint32_t)k.b_slots * k.unit_b_bytes;
         k.off_stg = (uint32_t)round_up2((int)ring_bytes, 128) + 128;  // 128-byte zero guard in front of the staging ring
@@ -896,7 +928,13 @@ int plan_build_v2(melt_plan *p) {
         if (k.stg_slots >= 5) break;
         if (k.b_resident) { k.b_resident = 0; k.b_slots = std::min(8, k.units - 1); }
         else --k.b_slots;
-        if (k.b_slots < 3) return MELT_OK;
+        if (k.b_slots < 3) {
+            // not even a streamed basis leaves room for staged chunks (windows of thousands of samples): no staging at all,
+            // the converter threads read their frames from global memory (L2 serves the 4x frame overlap)
+            k.direct = 1; k.b_slots = std::min(8, k.units - 1); k.stg_slots = 0;
+            k.off_stg = (uint32_t)round_up2((int)((uint32_t)k.b_slots * k.unit_b_bytes), 128) + 128;
+            break;
+        }
     }
     k.off_dct = (uint32_t)round_up2((int)(k.off_stg + (uint32_t)k.stg_slots * k.slot_bytes + 128), 128);
     k.off_bar = (uint32_t)round_up2((int)(k.off_dct + dct_bytes), 128);
@@ -907,6 +945,7 @@ int plan_build_v2(melt_plan *p) {
 
     // ---- per-unit load table: byte offset of sample n of a frame = ((n div H) * pitch + n mod H) * 4 (floor division)
     auto off_of = [&](int n) -> int {
+        if (k.direct) return 4 * n;   // byte offset within the frame in global memory
         int row = n >= 0 ? n / H : -((-n + H - 1) / H);
         return (row * pitch_words + (n - row * H)) * 4;
     };
@@ -917,7 +956,10 @@ int plan_build_v2(melt_plan *p) {
         for (int i = 0; i < nq; ++i) k.tab[u][4 + i] = (short)off_of(run - sigma + 4 * i);
         k.tab[u][8] = (short)off_of(run + k.kstep - 1);
         for (int i = 0; i < V2_TAB; ++i)
-            if (k.tab[u][i] < -128 || k.tab[u][i] + 16 > k.slot_bytes + 128) return MELT_OK;   // stays inside ring + guards
+            if (k.direct) {   // every read must stay inside the frame: [0, N) samples
+                const bool quad = i < nq || (i >= 4 && i < 4 + nq), single = i == 8 && sigma == 1;
+                if ((quad && (k.tab[u][i] < 0 || k.tab[u][i] + 16 > 4 * N)) || (single && (k.tab[u][i] < 0 || k.tab[u][i] + 4 > 4 * N))) return MELT_OK;
+            } else if (k.tab[u][i] < -128 || k.tab[u][i] + 16 > k.slot_bytes + 128) return MELT_OK;   // stays inside ring + guards
     }
 
     // ---- basis image: [rank][unit][kind][nb/2 rows] slabs (same folded coefficients as v1, split by Mel row)
@@ -938,21 +980,24 @@ int plan_build_v2(melt_plan *p) {
         if (kind == OP_BF16) return bf16_bits_to_f64(f64_to_bf16_bits(v));
         return tf32_bits_to_f64(f64_to_tf32_bits(v));
     };
-    const size_t img_bytes = (size_t)2 * b_bytes;
+    // image: [rank][pass][unit] slabs; pass ps covers Mel rows [ps * nb, ps * nb + nb), CTA rank r the half [r * nb/2, ...) of them
+    const size_t img_bytes = (size_t)2 * k.passes * b_bytes;
     std::vector<uint8_t> img(img_bytes, 0);
     const int nh = k.nb / 2;
     for (int r = 0; r < 2; ++r)
-        for (int u = 0; u < k.units; ++u) {
-            uint8_t *slab = img.data() + ((size_t)r * k.units + u) * k.unit_b_bytes;
-            for (int kk = 0; kk < k.nk; ++kk) {
-                const bool sine = comp ? (kk >= 2) : (kk == 1);
-                const bool lo = comp && (kk & 1);
-                pack_b_slab(kind, nh, [&](int row, int kq) {
-                    double v = coef(r * nh + row, u * k.kstep + kq, sine);
-                    return lo ? v - hi_of(v) : v;
-                }, slab + (size_t)kk * k.kind_bytes);
+        for (int ps = 0; ps < k.passes; ++ps)
+            for (int u = 0; u < k.units; ++u) {
+                uint8_t *slab = img.data() + (((size_t)r * k.passes + ps) * k.units + u) * k.unit_b_bytes;
+                for (int kk = 0; kk < k.nk; ++kk) {
+                    const bool sine = comp ? (kk >= 2) : (kk == 1);
+                    const bool lo = comp && (kk & 1);
+                    pack_b_slab(kind, nh, [&](int row, int kq) {
+                        const int m = ps * k.nb + r * nh + row;
+                        double v = (r * nh + row < k.nb) ? coef(m, u * k.kstep + kq, sine) : 0.0;
+                        return lo ? v - hi_of(v) : v;
+                    }, slab + (size_t)kk * k.kind_bytes);
+                }
             }
-        }
     cudaFree(p->d_bimg2);
     p->d_bimg2 = nullptr;
     {   // replicas of the image spread the clusters' simultaneous first fetch over more L2 lines (tuning knob; default 1)
@@ -994,6 +1039,7 @@ static EncodeTiledFn encode_tiled_fn() {
 
 int v2_encode_tmap(K2Params &k) {
     k.tma_rows = 0;
+    if (k.direct) return MELT_OK;   // no staging, no tensor map
     static const bool disabled = getenv("MELT_DISABLE_TMA") != nullptr;   // debug switch: per-row bulk copies everywhere
     if (disabled) return MELT_OK;
     EncodeTiledFn enc = encode_tiled_fn();
@@ -1046,11 +1092,11 @@ bool v2_accepts(const melt_plan *p, const float *x, long long len) {
     return p->v2_ok && (((uintptr_t)x & 15) == 0) && ((len & 3) == 0);
 }
 
-template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM>
+template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM, bool DIRECT>
 static int launch_one_s(const K2Params &kp, int grid, cudaStream_t stream) {
     static bool attr_done = false;
     if (!attr_done) {
-        MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE, STREAM>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
+        MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE, STREAM, DIRECT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
         attr_done = true;
     }
     // Programmatic dependent launch: when the previous operation in the stream is another forward of this library, the
@@ -1069,14 +1115,18 @@ static int launch_one_s(const K2Params &kp, int grid, cudaStream_t stream) {
     static const bool no_pdl = getenv("MELT_NO_PDL") != nullptr;   // debug switch
     cfg.attrs = attr;
     cfg.numAttrs = (no_pdl || kp.offsets != nullptr) ? 0 : 1;   // ragged: the scan kernel's results are read at kernel entry
-    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE, STREAM>, kp));
+    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE, STREAM, DIRECT>, kp));
     return MELT_OK;
 }
 
 template <int PREC, int SIGMA, bool RAGGED, int MODE>
 static int launch_one_r(const K2Params &kp, int grid, cudaStream_t stream) {
-    return kp.b_resident ? launch_one_s<PREC, SIGMA, RAGGED, MODE, false>(kp, grid, stream)
-                         : launch_one_s<PREC, SIGMA, RAGGED, MODE, true>(kp, grid, stream);
+    if (kp.direct) {   // dense, streamed basis only (plan_build_v2)
+        if (RAGGED) return fail(MELT_ERR_UNSUPPORTED, "internal: direct mode is dense only");
+        return launch_one_s<PREC, SIGMA, false, MODE, true, true>(kp, grid, stream);
+    }
+    return kp.b_resident ? launch_one_s<PREC, SIGMA, RAGGED, MODE, false, false>(kp, grid, stream)
+                         : launch_one_s<PREC, SIGMA, RAGGED, MODE, true, false>(kp, grid, stream);
 }
 
 template <int PREC, int SIGMA>
@@ -1093,7 +1143,7 @@ static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
 
 int launch_forward2(const melt_plan *pl, const K2Params &kp, cudaStream_t stream) {
     int pairs = pl->sm_count / 2;
-    if (kp.n_tiles >= 0 && kp.n_tiles < pairs) pairs = kp.n_tiles;   // ragged (n_tiles < 0): counted on the device
+    if (kp.n_tiles >= 0 && (long long)kp.n_tiles * kp.passes < pairs) pairs = kp.n_tiles * kp.passes;   // ragged (n_tiles < 0): counted on the device
     if (pairs < 1) return MELT_OK;
     const int grid = 2 * pairs;
     const int sg = pl->v2_sigma;

@@ -241,7 +241,7 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
         if (n_clips > MAX_CLIPS) return fail(MELT_ERR_UNSUPPORTED, "n_clips=%d exceeds %d", n_clips, MAX_CLIPS);
         if (!out_frame_offsets) return fail(MELT_ERR_INVALID_ARG, "out_frame_offsets is NULL");
         if (kp.feature_major) return fail(MELT_ERR_UNSUPPORTED, "ragged batches are frame-major only");
-        if (p->v2_ok && (((uintptr_t)x & 15) == 0)) {
+        if (p->v2_ok && !p->k2.direct && (((uintptr_t)x & 15) == 0)) {
             // the CTA-pair kernel: 256-frame tiles, looked up on the device; chunks start at any sample of the packed buffer
             rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, 256, st);
             if (rc) return rc;
@@ -264,7 +264,7 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
         if (v2_accepts(p, x, len) && !(tap && ((uintptr_t)tap & 3))) {
             K2Params k2 = p->k2;
             const long long tpc2 = (T + 255) / 256;
-            if (tpc2 * n_clips > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
+            if (tpc2 * n_clips * std::max(1, p->k2.passes) > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
             k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = len; k2.frames_per_clip = T;
             k2.tiles_per_clip = (int)tpc2; k2.n_tiles = (int)(tpc2 * n_clips);
             k2.offsets = nullptr; k2.frame_offsets = nullptr; k2.tile_prefix = nullptr;

@@ -57,7 +57,7 @@ struct KParams {
 constexpr int V2_CONV_GROUPS = 2;     // converter groups of 4 warps (one warp per tensor-memory lane quarter); 3 groups
                                       // (640 threads, 96 registers) measured no faster on the Whisper shape
 constexpr int V2_THREADS = 128 * (2 + V2_CONV_GROUPS);   // warps: loader, MMA issuer R, basis/TMEM, MMA issuer I, 4 epilogue, 4 per converter group
-constexpr int V2_MAX_UNITS = 64;      // K-steps per tile the per-unit load table covers
+constexpr int V2_MAX_UNITS = 128;     // K-steps per tile the per-unit load table covers
 constexpr int V2_MAX_STG = 12;        // staging ring slots (32-frame chunks)
 constexpr int V2_TAB = 12;            // int16 entries per unit: [0,4) forward quads, [4,8) backward quads, [8] single
 
@@ -87,6 +87,8 @@ struct K2Params {
     // ---- plan-owned device data
     const uint8_t *b_img;  // [b_replicas][2 ranks][units] slabs of unit_b_bytes
     int b_replicas;
+    int passes;                // passes over the Mel bins (nb bins each); > 1 needs the streamed basis
+    int direct;                // no staging: converter threads read their frames from global memory (very long windows)
     int b_resident, b_slots;   // basis half resident in shared memory (b_slots = units), or streamed through a ring of b_slots K-step slabs
     const float *dct;      // [n_mels][dct_pitch]
     // ---- per-unit shared-memory byte offsets (relative to the first sample of the thread's frame)
