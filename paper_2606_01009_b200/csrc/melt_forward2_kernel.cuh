@@ -1,0 +1,929 @@
+#pragma once
+// melt_forward2_kernel.cuh -- the hot path (steps S1-S6 of SURVEY.md 8(a)) as ONE persistent, warp-specialised kernel on CTA
+// PAIRS (thread-block clusters of two SMs, tcgen05.mma.cta_group::2).  A tile is 256 consecutive frames of one clip:
+// CTA r of the pair owns frames [128 r, 128 r + 128) of it (its 128 tensor-memory lanes).
+//
+//   loader warp       raw fp32 signal (global) -> shared-memory staging ring, implicit im2col by the tensor-map engine: one
+//                     cp.async.bulk.tensor box per chunk of 32 frames over a 3-D map of the signal whose row stride (hop) is
+//                     smaller than its row extent, so overlapping frames are never materialised; the chunk is prefetched
+//                     into L2 while the loader waits for a free slot.  Clip tails fall back to one bulk copy per hop-row.
+//   converter warps   2 groups x 4 warps, thread = frame; the groups take K-steps round-robin.  128-bit conflict-free shared
+//                     loads (row pitch = 4 * odd words), fold of the frame about the window centre (x[c+j] +- x[c-j]), split
+//                     into tensor-core operands (fp16 hi + lo, or bf16, or tf32) with packed fp32 arithmetic and tcgen05.st
+//                     straight into TENSOR MEMORY: the A operand never exists in shared or global memory.
+//   basis             each CTA keeps HALF of the folded cos/sin basis (nb/2 Mel rows per operand kind) resident in shared
+//                     memory, one barrier per K-step slab; the pair's tensor cores read both halves (cta_group::2).
+//   MMA issuers       two warps of the leader CTA on different schedulers: one accumulates R (cos rows), the other I (sin
+//                     rows); tcgen05.mma.cta_group::2 kind::f16 / kind::tf32, M = 256 over the pair, A from tensor memory,
+//                     B from shared memory, fp32 accumulators in tensor memory (R in columns [0, nb), I in [nb, 2 nb)),
+//                     double-buffered when they fit.  An iteration covers two K-steps.
+//   epilogue warps    tcgen05.ld -> R^2 + I^2 -> log10(max(., 1e-10)) -> optional DCT-II (fp32 FMA) -> coalesced stores.
+//
+// Hand-offs are mbarriers; cross-CTA ones are remote arrivals (mapa) and multicast tcgen05.commit.  Consecutive forwards on a
+// stream overlap through programmatic dependent launch (see launch_one).
+#include "melt_plan.h"
+#include "sm100_ptx.cuh"
+
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include <algorithm>
+#include <cstdlib>
+
+namespace melt {
+
+enum { P2_COMP = 0, P2_TF32 = 1, P2_BF16 = 2 };
+// barrier indices (8 bytes each)
+enum {
+    V_STG_FULL = 0, V_STG_EMPTY = V2_MAX_STG, V_A_FULL = 2 * V2_MAX_STG, V_A_EMPTY = V_A_FULL + 16, V_ACC_FULL = V_A_EMPTY + 16,
+    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_DONE = V_B_PEER + V2_MAX_UNITS, V_STG_READY = V_DONE + 1, V_B_EMPTY = V_STG_READY + V2_MAX_STG, V_NBARS = V_B_EMPTY + 8
+};
+constexpr int V2_MAX_A_SLOTS = 16;
+constexpr int W_LOAD = 0, W_MMA = 1, W_BASIS = 2, W_MMA2 = 3, W_EPI0 = 4, W_CONV0 = 8;
+
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ float4 ldg128(const char *p) {   // read-only path, 16-byte aligned
+    float4 v;
+    asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float ldg32(const char *p) {
+    float v;
+    asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ float lds32(uint32_t addr) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr));
+    return v;
+}
+// packed fp32 pairs in one 64-bit register (sm_100 FADD2 / FMUL2: two lanes per issue slot)
+__device__ __forceinline__ uint64_t f2_pack(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ uint64_t f2_add(uint64_t a, uint64_t b) {
+    uint64_t r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ uint64_t f2_sub(uint64_t a, uint64_t b) {
+    uint64_t r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ uint64_t f2_mul(uint64_t a, uint64_t b) {
+    uint64_t r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ __half2 f2_to_half2(uint64_t a) {   // round to nearest even, lane 0 -> low half
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a));
+    return __floats2half2_rn(lo, hi);
+}
+__device__ __forceinline__ uint64_t half2_to_f2(__half2 h) {
+    const float2 f = __half22float2(h);
+    return f2_pack(f.x, f.y);
+}
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// Optional event trace (development builds only, -DMELT_TRACE): lane 0 of every warp of cluster 0 appends (tag, clock) pairs.
+#ifdef MELT_TRACE
+extern __device__ long long *g_melt_trace;   // [2 ranks][16 warps][1024] events
+#define TRACE_DECL int tr_n = 0; long long *tr_buf = (g_melt_trace && cluster_id_x() == 0 && (threadIdx.x & 31) == 0) ? g_melt_trace + ((size_t)cluster_ctarank() * 16 + (threadIdx.x >> 5)) * 1024 : nullptr;
+#define TRACE(tag) do { if (tr_buf && tr_n < 1023) tr_buf[++tr_n] = ((long long)(tag) << 48) | (clock64() & 0xFFFFFFFFFFFFll); if (tr_buf) tr_buf[0] = tr_n; } while (0)
+#define TRACE_CTA(which) do { if (g_melt_trace && threadIdx.x == 0) g_melt_trace[2 * 16 * 1024 + blockIdx.x * 2 + (which)] = (long long)globaltimer_ns(); } while (0)
+#else
+#define TRACE_CTA(which) do { } while (0)
+#define TRACE_DECL
+#define TRACE(tag) do { } while (0)
+#endif
+
+// Log-Mel epilogue of the 16-bin blocks blk0, blk0 + step, ... of one tile for one thread (= frame).  Used when a tile's
+// accumulator is drained by several warps per lane quarter (single accumulator stage: the MMAs of the next tile cannot
+// start before the drain, so the converter warps take their share of it instead of waiting).
+__device__ __forceinline__ void epi_fast_share(uint32_t t_r, uint32_t t_i, int nb, int n_mels, float *optr, long long cstride,
+                                               bool valid, float off, int blk0, int step) {
+    const float kLog10_2 = 0.30102999566398120f;
+    for (int c0 = 16 * blk0; c0 < nb; c0 += 16 * step) {
+        uint32_t vr[16], vi[16];
+        tmem_ld16(t_r + (uint32_t)c0, vr);
+        tmem_ld16(t_i + (uint32_t)c0, vi);
+        tmem_wait_ld();
+        const int nrem = n_mels - c0;   // bins of this block that exist
+        float *o = optr + (long long)c0 * cstride;
+        if (nrem >= 16) {
+            if (valid) {
+#pragma unroll
+                for (int c = 0; c < 16; ++c) {
+                    const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                    *o = fmaxf(fmaf(lg2_ftz(fmaf(r, r, im * im)), kLog10_2, off), -10.f);   // Eq. (4), Eq. (8) in contract form
+                    o += cstride;
+                }
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < 16; ++c) {
+                const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                if (valid && c < nrem) *o = fmaxf(fmaf(lg2_ftz(fmaf(r, r, im * im)), kLog10_2, off), -10.f);
+                o += cstride;
+            }
+        }
+    }
+}
+
+// Epilogue of one tile for one thread (= frame) in the general case: power or log output, optional tap of the log-Mel
+// matrix, optional DCT-II with 4 * KQ accumulators (KQ = 0: no DCT).  Returns after handing the accumulator stage back.
+template <int KQ>
+__device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uint32_t t_i, const float *dct_s, float *optr, float *tptr,
+                                            long long cstride, bool valid, int lane, uint32_t acc_empty_bar, int nm) {
+    const float kLog10_2 = 0.30102999566398120f;
+    float cacc[KQ > 0 ? 4 * KQ : 1];
+#pragma unroll
+    for (int k = 0; k < (KQ > 0 ? 4 * KQ : 1); ++k) cacc[k] = 0.f;
+    for (int c0 = 0; c0 < p.nb; c0 += 16) {
+        uint32_t vr[16], vi[16];
+        tmem_ld16(t_r + (uint32_t)c0, vr);
+        tmem_ld16(t_i + (uint32_t)c0, vi);
+        tmem_wait_ld();
+#pragma unroll
+        for (int c = 0; c < 16; ++c) {
+            const int m = c0 + c;
+            if (m < nm) {
+                const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                const float praw = fmaf(r, r, im * im);                                          // Eq. (4)
+                float v;
+                if (p.output_power) v = praw * p.out_scale;
+                else v = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, p.out_log10_offset), -10.f);       // Eq. (8), contract form
+                if (KQ > 0) {
+                    const float *drow = dct_s + m * p.dct_pitch;
+#pragma unroll
+                    for (int q4 = 0; q4 < KQ; ++q4) {
+                        const float4 d = *reinterpret_cast<const float4 *>(drow + 4 * q4);
+                        cacc[4 * q4 + 0] = fmaf(d.x, v, cacc[4 * q4 + 0]);
+                        cacc[4 * q4 + 1] = fmaf(d.y, v, cacc[4 * q4 + 1]);
+                        cacc[4 * q4 + 2] = fmaf(d.z, v, cacc[4 * q4 + 2]);
+                        cacc[4 * q4 + 3] = fmaf(d.w, v, cacc[4 * q4 + 3]);
+                    }
+                    if (tptr && valid) tptr[m * cstride] = v;
+                } else if (valid) {
+                    optr[m * cstride] = v;
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive_remote(acc_empty_bar);
+    if (KQ > 0 && valid) {                                                                      // Eq. (9)
+#pragma unroll
+        for (int k = 0; k < 4 * KQ; ++k)
+            if (k < p.n_mfcc) optr[k * cstride] = cacc[k];
+    }
+}
+
+// Where a 256-frame tile lives: dense batches by division, ragged ones by binary search in the device-side tile prefix.
+struct Tile2 {
+    int clip, t0;      // clip index, first frame of the tile within the clip
+    long long T;       // frames of the clip
+    long long s0;      // index of the clip's first sample in x
+    long long f0;      // index of the clip's first frame in the (packed or dense) frame order
+    int pass;          // pass over the Mel bins (more than 128 bins: every tile is visited once per pass)
+};
+template <bool RAGGED>
+__device__ __forceinline__ void get_tile2(const K2Params &p, int vtile, Tile2 &ti) {
+    int tile = vtile;
+    ti.pass = 0;
+    if (p.passes > 1) { tile = vtile / p.passes; ti.pass = vtile - tile * p.passes; }
+    if (!RAGGED) {
+        const int b = tile / p.tiles_per_clip;
+        ti.clip = b;
+        ti.t0 = (tile - b * p.tiles_per_clip) * 256;
+        ti.T = p.frames_per_clip;
+        ti.s0 = (long long)b * p.len;
+        ti.f0 = (long long)b * p.frames_per_clip;
+    } else {
+        int lo = 0, hi = p.n_clips;   // largest i with tile_prefix[i] <= tile
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (__ldg(p.tile_prefix + mid) <= tile) lo = mid; else hi = mid;
+        }
+        ti.clip = lo;
+        ti.t0 = (tile - __ldg(p.tile_prefix + lo)) * 256;
+        ti.f0 = p.frame_offsets[lo];
+        ti.T = p.frame_offsets[lo + 1] - ti.f0;
+        ti.s0 = __ldg(p.offsets + lo);
+    }
+}
+
+// Ragged batches: shifts a staged chunk down by (clip offset & 3) words (see the loader).  Out of line on purpose: it runs
+// once per chunk on ragged batches only and must not take registers from the converter loop it is called from.
+static __device__ __noinline__ void ragged_realign(const long long *offsets, const int *tile_prefix, int n_clips, int tile, float *w,
+                                            int n_words, int lane) {
+    int lo = 0, hi = n_clips;   // largest i with tile_prefix[i] <= tile
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (__ldg(tile_prefix + mid) <= tile) lo = mid; else hi = mid;
+    }
+    const int dlt = (int)(__ldg(offsets + lo) & 3);
+    if (dlt) {
+        const int n = n_words - dlt;
+        for (int i = lane; i < n; i += 128) {
+            float v[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) v[j] = (i + 32 * j < n) ? w[i + 32 * j + dlt] : 0.f;
+            __syncwarp();   // every lane has read before any lane overwrites (lane l writes what lane l - dlt read)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (i + 32 * j < n) w[i + 32 * j] = v[j];
+            __syncwarp();
+        }
+    }
+    __syncwarp();
+}
+
+template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM, bool DIRECT>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    // Who drains the accumulators: MODE 0 the four epilogue warps alone; MODE 1 (single accumulator stage, log-Mel) the epilogue
+    // warps and the converter warps together; MODE 2 (log-Mel) there are no epilogue warps -- they form a third converter
+    // group and every converter warp drains a third of the bins of the previous tile.
+    constexpr bool SHARE = MODE != 0;
+    constexpr int NG = MODE == 2 ? V2_CONV_GROUPS + 1 : V2_CONV_GROUPS;   // converter groups
+    constexpr int CONV0 = MODE == 2 ? W_EPI0 : W_CONV0;                   // first converter warp
+    constexpr int DRAINERS = MODE == 2 ? NG : 1 + NG;                     // warps per lane quarter that drain (SHARE)
+    constexpr int DRAIN0 = MODE == 2 ? 0 : 1;                             // block index of converter group 0's share
+    TRACE_CTA(0);
+    constexpr int KS = (PREC == P2_TF32) ? 8 : 16;  // folded pairs per K-step
+    constexpr int NQ = KS / 4;                      // 128-bit loads per direction per K-step
+    const uint32_t sbase = smem_u32(smem);
+    const uint32_t bar0 = sbase + p.off_bar;
+    auto BAR = [&](int idx) -> uint32_t { return bar0 + (uint32_t)idx * 8u; };
+    uint32_t *tmem_ptr_s = reinterpret_cast<uint32_t *>(smem + p.off_bar + V_NBARS * 8);
+    float *dct_s = reinterpret_cast<float *>(smem + p.off_dct);
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);   // provably warp-uniform: role branches stay non-divergent
+    const uint32_t rank = cluster_ctarank();
+    const int S = p.stg_slots;
+
+    // ------------------------------------------------------------------ one-time setup
+    if (!RAGGED && !DIRECT && tid == 32 && p.tma_rows > 0 && p.passes == 1) {
+        // First thing, before any set-up: pull this CTA's first two tiles into L2.  The staging copies are issued ~1000
+        // cycles from now (after barrier / tensor-memory set-up) and one after the other; with the DRAM accesses of all
+        // chunks started here, in parallel, they cost L2 hits -- the first MMA starts ~1.5 us earlier.
+        const int cid = (int)cluster_id_x(), cstep = (int)cluster_nid_x();
+        for (int k = 0; k < 2; ++k) {
+            const int tile = cid + k * cstep;
+            if (tile >= p.n_tiles) break;
+            const int b = tile / p.tiles_per_clip;
+            const int t0 = (tile - b * p.tiles_per_clip) * 256 + (int)cluster_ctarank() * 128;
+            for (int q = 0; q < 4; ++q) {
+                const long long row0 = (long long)(t0 + 32 * q);
+                if (row0 < p.frames_per_clip && row0 + p.rows_per_chunk <= (long long)p.tma_rows) tma_prefetch_l2_3d(p.tmap, 0, (int)row0, b);
+            }
+        }
+    }
+    if (tid == 0) {
+        for (int i = 0; i < V2_MAX_STG; ++i) { mbar_init(BAR(V_STG_FULL + i), 1); mbar_init(BAR(V_STG_EMPTY + i), NG); }
+        for (int i = 0; i < V2_MAX_A_SLOTS; ++i) { mbar_init(BAR(V_A_FULL + i), 8); mbar_init(BAR(V_A_EMPTY + i), 2); }   // both issuers commit
+        for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 2); mbar_init(BAR(V_ACC_EMPTY + i), SHARE ? 8 * DRAINERS : 8); }
+        for (int i = 0; i < p.b_slots; ++i) { mbar_init(BAR(V_B_FULL + i), 1); mbar_init(BAR(V_B_PEER + i), 1); }   // b_slots = units when resident
+        mbar_init(BAR(V_DONE), 2);   // both MMA issuers
+        if (STREAM)
+            for (int i = 0; i < 8; ++i) mbar_init(BAR(V_B_EMPTY + i), 2);   // streamed basis: both issuers release a slab
+        for (int i = 0; i < V2_MAX_STG; ++i) mbar_init(BAR(V_STG_READY + i), 1);
+        fence_barrier_init();
+    }
+    if (warp == W_BASIS) {
+        tmem_alloc2(smem_u32(tmem_ptr_s), 512);
+        tmem_relinquish2();
+    }
+    {   // staging ring (and its guard bands) starts finite: stale rows are multiplied by zero basis entries or belong to
+        // frames that are never stored, but must never be NaN / Inf bit patterns
+        float4 *z = reinterpret_cast<float4 *>(smem + p.off_stg - 128);
+        const int n16 = (S * p.slot_bytes + 256) / 16;
+        for (int i = tid; i < n16; i += V2_THREADS) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    if (p.n_mfcc > 0)
+        for (int i = tid; i < p.n_mels * p.dct_pitch; i += V2_THREADS) dct_s[i] = __ldg(p.dct + i);
+    fence_proxy_async_smem();  // the zero fill (generic proxy) is ordered before the bulk copies (async proxy) that follow
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    tc_fence_after();
+    const uint32_t tmem_base = *tmem_ptr_s;
+    if (tid == 0) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the next forward may start filling freed SMs
+
+    const int first_tile = (int)cluster_id_x(), tile_step = (int)cluster_nid_x();
+    const int n_tiles = (RAGGED ? p.tile_prefix[p.n_clips] : p.n_tiles) * p.passes;   // ragged: counted by the scan kernel; one visit per pass over the bins
+    TRACE_DECL
+    TRACE(1);
+    if (warp == W_LOAD && DIRECT) {
+        // windows too long for staged 32-frame chunks: the converter threads read their frames straight from global memory
+    } else if (warp == W_LOAD) {
+        // ============================================================== signal loader (bulk-copy engine)
+        // The whole warp runs the (uniform) loop; one elected lane issues the copies.
+        int slot = 0;
+        uint32_t ph = 0;
+        const long long len = p.len;
+        if (p.tma_rows > 0 && lane == 0) tma_prefetch_desc(p.tmap);
+        constexpr bool ragged = RAGGED;
+        const long long total = ragged ? p.offsets[p.n_clips] : 0;   // samples in the packed buffer
+        for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+            Tile2 ti;
+            get_tile2<RAGGED>(p, tile, ti);
+            const int b = ti.clip;
+            const int t0 = ti.t0 + (int)rank * 128;
+            const float *xb = p.x + ti.s0;
+            const long long clip_len = ragged ? p.offsets[b + 1] - ti.s0 : len;
+            for (int q = 0; q < 4; ++q) {
+                const long long row0 = (long long)(t0 + 32 * q);
+                const int n_rows = row0 < ti.T ? p.rows_per_chunk : 0;
+                long long avail = clip_len - row0 * p.hop;                 // samples of the clip from the chunk's first row on
+                avail = avail < 0 ? 0 : avail;
+                const long long want = (long long)n_rows * p.hop;
+                const uint32_t total_b = (uint32_t)(avail < want ? avail : want) * 4u;
+                const uint32_t dst0 = sbase + p.off_stg + (uint32_t)slot * (uint32_t)p.slot_bytes;
+                // ragged: the chunk starts at sample s of the packed buffer = column s % hop of hop-row s / hop of the 2-D map
+                // The tensor-map engine wants the box to start on a 16-byte boundary: it is fetched from the aligned sample below
+                // (clip starts are arbitrary; hop % 4 == 0, so every chunk of a clip has the same misalignment) and the
+                // converter warp that owns the chunk shifts it down by (s0 & 3) words in shared memory.
+                long long s = 0;
+                int c0 = 0, c1 = (int)row0, c2 = b;
+                bool by_tma;
+                if (!ragged) {
+                    by_tma = n_rows > 0 && row0 + n_rows <= (long long)p.tma_rows;
+                } else {
+                    s = (ti.s0 & ~3ll) + row0 * p.hop;
+                    const long long r = s / p.hop;
+                    c0 = (int)(s - r * p.hop); c1 = (int)r; c2 = 0;
+                    by_tma = n_rows > 0 && s + (long long)(p.rows_per_chunk - 1) * p.hop + (p.pitch_bytes >> 2) <= total;
+                }
+                // The staging ring holds less than two tiles, so the loader usually sits here waiting for a slot: pull the
+                // chunk into L2 meanwhile -- when the slot frees, the copy into shared memory costs an L2 hit, not a DRAM access
+                if (by_tma && elect_one()) tma_prefetch_l2_3d(p.tmap, c0, c1, c2);
+                __syncwarp();
+                TRACE(10);
+                mbar_wait(BAR(V_STG_EMPTY + slot), ph ^ 1u);
+                TRACE(11);
+                if (ragged && !by_tma) {
+                    // the few chunks that reach beyond the packed buffer (end of the last clip), or rows of no valid frame:
+                    // plain bounds-checked loads by the whole warp (the bulk-copy engine needs 16-byte aligned sources)
+                    const int pw = p.pitch_bytes >> 2;
+                    const int n_el = n_rows * pw;
+                    float *dstp = reinterpret_cast<float *>(smem + p.off_stg + (size_t)slot * p.slot_bytes);
+                    for (int idx = lane; idx < n_el; idx += 32) {
+                        const int r = idx / pw;
+                        const long long g = s + (long long)r * p.hop + (idx - r * pw);
+                        dstp[idx] = g < total ? __ldg(p.x + g) : 0.f;
+                    }
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(BAR(V_STG_FULL + slot));
+                    __syncwarp();
+                    TRACE(12);
+                    if (++slot == S) { slot = 0; ph ^= 1u; }
+                    continue;
+                }
+                if (elect_one()) {
+                    const uint32_t full = BAR(V_STG_FULL + slot);
+                    if (by_tma) {
+                        // one tensor-map box = the whole chunk: rows_per_chunk hop-rows of pitch width (implicit im2col)
+                        mbar_arrive_expect_tx(full, (uint32_t)p.rows_per_chunk * (uint32_t)p.pitch_bytes);
+                        tma_load_3d(dst0, p.tmap, c0, c1, c2, full);
+                    } else {
+                        // clip tail (or no tensor map): one bulk copy per hop-row, clipped to the clip
+                        if (total_b) mbar_arrive_expect_tx(full, total_b);
+                        else mbar_arrive(full);
+                        uint32_t dst = dst0;
+                        const float *src = xb + row0 * p.hop;
+                        uint32_t left = total_b;
+                        const uint32_t row_bytes = (uint32_t)p.hop * 4u;
+                        while (left) {
+                            const uint32_t nb = left < row_bytes ? left : row_bytes;
+                            bulk_g2s(dst, src, nb, full);
+                            dst += (uint32_t)p.pitch_bytes; src += p.hop; left -= nb;
+                        }
+                    }
+                }
+                __syncwarp();
+                TRACE(12);
+                if (++slot == S) { slot = 0; ph ^= 1u; }
+            }
+        }
+    } else if (warp == W_BASIS) {
+        // ============================================================== basis: this CTA's half, resident
+        // One barrier per K-step slab, so that the first tile's MMAs start as soon as the first slabs have landed.
+        if (first_tile < n_tiles) {
+            // the image is replicated in global memory: 74 clusters fetching the same lines at once serialise in L2
+            const uint8_t *src = p.b_img + ((size_t)(cluster_id_x() % (uint32_t)p.b_replicas) * 2 + rank) * p.passes * p.units * p.unit_b_bytes;
+            if (!STREAM) {   // a template parameter: the resident instantiation carries no streaming code (0.7 us per cfg1 step)
+                if (elect_one()) {
+                    for (int u = 0; u < p.units; ++u) {
+                        mbar_arrive_expect_tx(BAR(V_B_FULL + u), p.unit_b_bytes);
+                        bulk_g2s(sbase + p.off_b + (uint32_t)u * p.unit_b_bytes, src + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL + u));
+                    }
+                }
+                __syncwarp();
+                if (rank == 1) {  // tell the leader, slab by slab, that the peer half has landed
+                    for (int u = 0; u < p.units; ++u) {
+                        mbar_wait(BAR(V_B_FULL + u), 0);
+                        // complete_tx has made the slab visible in this CTA's shared memory; the tensor core of the pair reads
+                        // it through the async proxy, so a plain remote arrival (no cluster-scope fence, which costs ~1000 cycles
+                        // with bulk copies in flight) is the hand-off
+                        if (lane == 0) mbar_arrive_remote(mapa_cluster(BAR(V_B_PEER + u), 0));
+                    }
+                }
+            } else {
+                // long windows: the K-step slabs of every tile stream from L2 through a ring of b_slots slabs; the issuers
+                // release a slab (multicast tcgen05.commit to both CTAs) when its MMAs have completed
+                int slot = 0;
+                uint32_t ph = 0;
+                for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+                    const uint8_t *psrc = src + (size_t)(tile % p.passes) * p.units * p.unit_b_bytes;   // this pass' rows of the basis
+                    for (int u = 0; u < p.units; ++u) {
+                        mbar_wait(BAR(V_B_EMPTY + slot), ph ^ 1u);
+                        if (elect_one()) {
+                            mbar_arrive_expect_tx(BAR(V_B_FULL + slot), p.unit_b_bytes);
+                            bulk_g2s(sbase + p.off_b + (uint32_t)slot * p.unit_b_bytes, psrc + (size_t)u * p.unit_b_bytes, p.unit_b_bytes, BAR(V_B_FULL + slot));
+                        }
+                        __syncwarp();
+                        if (++slot == p.b_slots) { slot = 0; ph ^= 1u; }
+                    }
+                }
+            }
+            mbar_wait(BAR(V_DONE), 0);   // all tensor-core work of the pair, and the barrier arrivals it triggers, are done
+        }
+    } else if (warp == W_MMA || warp == W_MMA2) {
+        // ============================================================== MMA issuers (leader CTA)
+        // Two issuer warps on different schedulers: W_MMA accumulates R (A = folded sums, B = cos rows), W_MMA2 accumulates I
+        // (A = folded differences, B = sin rows).  Every accumulator has ONE issuing thread, so the summation order is fixed.
+        // An iteration covers two K-steps: the fixed cost of a hand-off (barrier probe, fence, election, operand set-up) is
+        // then paid once per ~480 cycles of tensor work instead of once per ~240, which a warp that shares its scheduler
+        // with three busy converter / epilogue warps could not keep up with.
+        if (STREAM && rank == 1 && warp == W_MMA && first_tile < n_tiles) {
+            // streamed basis: this (otherwise idle) warp of the peer CTA tells the leader when a slab of the peer half has landed
+            int slot = 0;
+            uint32_t ph = 0;
+            for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+                for (int u = 0; u < p.units; ++u) {
+                    mbar_wait(BAR(V_B_FULL + slot), ph);
+                    if (lane == 0) mbar_arrive_remote(mapa_cluster(BAR(V_B_PEER + slot), 0));
+                    __syncwarp();
+                    if (++slot == p.b_slots) { slot = 0; ph ^= 1u; }
+                }
+            }
+        }
+        if (rank == 0 && first_tile < n_tiles) {
+            const int which = warp == W_MMA ? 0 : 1;
+            const uint32_t idesc = umma_idesc(PREC == P2_COMP ? UMMA_F16 : (PREC == P2_BF16 ? UMMA_BF16 : UMMA_TF32), (uint32_t)p.nb, 256u);
+            // shared-memory descriptors of K-step 0; K-step u adds u * unit_b_bytes (in 16-byte units) to the address field
+            // B kinds: COMPENSATED [wc_hi, wc_lo, ws_hi, ws_lo]; single pass [wc, ws]
+            const uint32_t b0 = sbase + p.off_b + (uint32_t)which * (PREC == P2_COMP ? 2u : 1u) * p.kind_bytes;
+            const uint64_t dsc_hi = umma_smem_desc_kmajor_noswz(b0, 128, 256);
+            const uint64_t dsc_lo = umma_smem_desc_kmajor_noswz(b0 + p.kind_bytes, 128, 256);
+            const uint64_t dstep = (uint64_t)(p.unit_b_bytes >> 4);
+            const int units = p.units, a_slots = p.a_slots, acc_stages = p.acc_stages;
+            // A kinds: COMPENSATED s_hi @0, s_lo @8, d_hi @16, d_lo @24; single pass s @0, d @8
+            const uint32_t a_base = tmem_base + (uint32_t)p.a_col0 + (uint32_t)which * (PREC == P2_COMP ? 16u : 8u);
+            const uint32_t unit_cols = (uint32_t)p.unit_cols;
+            const uint32_t acc_cols = (uint32_t)p.acc_cols;
+            const uint32_t d_base = tmem_base + (uint32_t)which * (uint32_t)p.nb;
+            int aslot = 0, stage = 0;
+            uint32_t aph = 0, sph = 0;
+            bool basis_pending = true;
+            constexpr bool b_res = !STREAM;
+            const int b_slots = p.b_slots;
+            int bslot = 0;          // streamed basis: ring slot of the next K-step's slab (resident basis: slot = K-step)
+            uint32_t bph = 0;
+            for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+                TRACE(20);
+                mbar_wait(BAR(V_ACC_EMPTY + stage), sph ^ 1u);
+                TRACE(21);
+                const uint32_t d = d_base + (uint32_t)stage * acc_cols;
+                uint64_t du = 0;   // resident basis: descriptor offset of K-step u
+                for (int u = 0; u < units; u += 2, du += 2 * dstep) {
+                    const bool two = u + 1 < units;
+                    int aslot1 = aslot + 1;
+                    uint32_t aph1 = aph;
+                    if (aslot1 == a_slots) { aslot1 = 0; aph1 ^= 1u; }
+                    int bs0, bs1;
+                    uint32_t bp0 = 0, bp1 = 0;
+                    if (b_res) {
+                        bs0 = u; bs1 = u + 1;
+                    } else {
+                        bs0 = bslot; bp0 = bph;
+                        bs1 = bslot + 1; bp1 = bph;
+                        if (bs1 == b_slots) { bs1 = 0; bp1 ^= 1u; }
+                    }
+                    if (basis_pending || !b_res) {
+                        mbar_wait(BAR(V_B_FULL + bs0), bp0); mbar_wait_cluster(BAR(V_B_PEER + bs0), bp0);
+                        if (two) { mbar_wait(BAR(V_B_FULL + bs1), bp1); mbar_wait_cluster(BAR(V_B_PEER + bs1), bp1); }
+                    }
+                    mbar_wait(BAR(V_A_FULL + aslot), aph);
+                    if (two) mbar_wait(BAR(V_A_FULL + aslot1), aph1);
+                    TRACE(22);
+                    tc_fence_after();
+                    if (elect_one()) {
+                        const uint32_t a0 = a_base + (uint32_t)aslot * unit_cols, a1 = a_base + (uint32_t)aslot1 * unit_cols;
+                        const uint64_t du0 = b_res ? du : (uint64_t)bs0 * dstep, du1 = b_res ? du + dstep : (uint64_t)bs1 * dstep;
+                        const uint32_t acc = u > 0;
+                        if (PREC == P2_COMP) {
+                            umma2_ts_f16(d, a0, dsc_hi + du0, idesc, acc);          // hi . hi
+                            umma2_ts_f16(d, a0 + 8, dsc_hi + du0, idesc, 1);        // lo . hi
+                            umma2_ts_f16(d, a0, dsc_lo + du0, idesc, 1);            // hi . lo
+                        } else if (PREC == P2_TF32) {
+                            umma2_ts_tf32(d, a0, dsc_hi + du0, idesc, acc);
+                        } else {
+                            umma2_ts_f16(d, a0, dsc_hi + du0, idesc, acc);
+                        }
+                        tc_commit2(BAR(V_A_EMPTY + aslot), 3);
+                        if (!b_res) tc_commit2(BAR(V_B_EMPTY + bs0), 3);
+                        if (two) {
+                            if (PREC == P2_COMP) {
+                                umma2_ts_f16(d, a1, dsc_hi + du1, idesc, 1);
+                                umma2_ts_f16(d, a1 + 8, dsc_hi + du1, idesc, 1);
+                                umma2_ts_f16(d, a1, dsc_lo + du1, idesc, 1);
+                            } else if (PREC == P2_TF32) {
+                                umma2_ts_tf32(d, a1, dsc_hi + du1, idesc, 1);
+                            } else {
+                                umma2_ts_f16(d, a1, dsc_hi + du1, idesc, 1);
+                            }
+                            tc_commit2(BAR(V_A_EMPTY + aslot1), 3);
+                            if (!b_res) tc_commit2(BAR(V_B_EMPTY + bs1), 3);
+                        }
+                        if (u + 2 >= units) tc_commit2(BAR(V_ACC_FULL + stage), 3);
+                    }
+                    __syncwarp();
+                    TRACE(23);
+                    if (!b_res) {
+                        bslot = bs0; bph = bp0;
+                        const int adv = two ? 2 : 1;
+                        for (int k = 0; k < adv; ++k)
+                            if (++bslot == b_slots) { bslot = 0; bph ^= 1u; }
+                    }
+                    if (two) { aslot = aslot1; aph = aph1; }
+                    if (++aslot == a_slots) { aslot = 0; aph ^= 1u; }
+                }
+                basis_pending = false;
+                if (++stage == acc_stages) { stage = 0; sph ^= 1u; }
+            }
+            // Nobody waits for the last operand-slot releases (tcgen05.commit arrivals, multicast to both CTAs).  They must not
+            // land after a CTA has exited and the next grid -- which may start on this SM right away (programmatic dependent
+            // launch) -- has re-initialised the barriers at the same shared-memory addresses: one more commit, behind all the
+            // others, is awaited by both CTAs before they retire.
+            if (elect_one()) tc_commit2(BAR(V_DONE), 3);
+            __syncwarp();
+        }
+    } else if (MODE != 2 && warp >= W_EPI0 && warp < W_EPI0 + 4) {
+        // ============================================================== epilogue (thread = frame)
+        const int q = warp & 3;
+        const int row = q * 32 + lane;
+        const uint32_t lane_taddr = tmem_base + ((uint32_t)(q * 32) << 16);
+        const uint32_t acc_empty_remote = mapa_cluster(BAR(V_ACC_EMPTY), 0);
+        const float kLog10_2 = 0.30102999566398120f;
+        int stage = 0;
+        uint32_t sph = 0;
+        const bool fast_log = p.n_mfcc == 0 && !p.output_power && p.tap == nullptr;
+        bool dep_done = false;
+        for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+            Tile2 ti;
+            get_tile2<RAGGED>(p, tile, ti);
+            const int b = ti.clip;
+            const int t0 = ti.t0 + (int)rank * 128;
+            const long long T = ti.T;
+            const bool valid = (long long)(t0 + row) < T;
+            float *optr, *tptr;
+            long long cstride;
+            const int c_off = ti.pass * p.nb;                                   // first bin of this pass
+            const int nm = p.n_mels - c_off < p.nb ? p.n_mels - c_off : p.nb;   // bins of this pass
+            if (p.feature_major) {
+                optr = p.out + ((long long)b * p.n_ch + c_off) * T + t0 + row;
+                tptr = p.tap ? p.tap + ((long long)b * p.n_mels + c_off) * T + t0 + row : nullptr;
+                cstride = T;
+            } else {   // frame-major; ragged batches: packed, the clip starts at frame ti.f0
+                optr = p.out + (ti.f0 + t0 + row) * p.n_ch + c_off;
+                tptr = p.tap ? p.tap + (ti.f0 + t0 + row) * p.n_mels + c_off : nullptr;
+                cstride = 1;
+            }
+            TRACE(30);
+            mbar_wait(BAR(V_ACC_FULL + stage), sph);
+            if (!dep_done) { asm volatile("griddepcontrol.wait;" ::: "memory"); dep_done = true; }   // before the first global store
+            TRACE(31);
+            tc_fence_after();
+            const uint32_t t_r = lane_taddr + (uint32_t)stage * (uint32_t)p.acc_cols, t_i = t_r + (uint32_t)p.nb;
+            if (SHARE) {
+                // single accumulator stage, log-Mel: this warp drains every third 16-bin block, the two converter warps of the
+                // lane quarter the others
+                epi_fast_share(t_r, t_i, p.nb, nm, optr, cstride, valid, p.out_log10_offset, 0, DRAINERS);
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
+            } else if (fast_log) {
+                // log-Mel, no DCT, no tap: the common case.  Whole 16-bin blocks take predicated stores without per-element
+                // bounds tests; the tensor-memory loads of the next block are in flight while this one is computed and stored.
+                float *o = optr;
+                const float off = p.out_log10_offset;
+                const int n_whole = nm & ~15;
+                uint32_t vr[16], vi[16];
+                if (n_whole > 0) { tmem_ld16(t_r, vr); tmem_ld16(t_i, vi); }
+                for (int c0 = 0; c0 < n_whole; c0 += 16) {
+                    float v[16];
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int c = 0; c < 16; ++c) {
+                        const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                        v[c] = fmaf(r, r, im * im);                                                          // Eq. (4)
+                    }
+                    if (c0 + 16 < p.nb) { tmem_ld16(t_r + (uint32_t)(c0 + 16), vr); tmem_ld16(t_i + (uint32_t)(c0 + 16), vi); }
+                    if (valid) {
+#pragma unroll
+                        for (int c = 0; c < 16; ++c) {
+                            *o = fmaxf(fmaf(lg2_ftz(v[c]), kLog10_2, off), -10.f);                           // Eq. (8), contract form
+                            o += cstride;
+                        }
+                    }
+                }
+                if (n_whole < p.nb) {   // last, partial block (its loads were issued above, or here when it is the only one)
+                    if (n_whole == 0) { tmem_ld16(t_r, vr); tmem_ld16(t_i, vi); }
+                    tmem_wait_ld();
+                    const int nrem = nm - n_whole;
+#pragma unroll
+                    for (int c = 0; c < 16; ++c) {
+                        const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                        const float praw = fmaf(r, r, im * im);
+                        if (valid && c < nrem) *o = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, off), -10.f);
+                        o += cstride;
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
+            } else {
+                const uint32_t eb = acc_empty_remote + (uint32_t)stage * 8u;
+                if (p.n_mfcc == 0) epi_generic<0>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm);
+                else if (p.dct_pitch <= 16) epi_generic<4>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm);
+                else if (p.dct_pitch <= 40) epi_generic<10>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm);
+                else epi_generic<16>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm);
+            }
+            TRACE(32);
+            if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
+        }
+    } else if (warp >= CONV0) {
+        // ============================================================== converters (thread = frame; the groups take K-step pairs round-robin)
+        const int q = warp & 3, g = (warp - CONV0) >> 2;
+        const uint32_t lane_taddr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)p.a_col0;
+        const uint32_t a_full_remote = mapa_cluster(BAR(V_A_FULL), 0);
+        const uint32_t row_off = sbase + p.off_stg + (uint32_t)lane * (uint32_t)p.pitch_bytes;
+        const float S_in = p.in_scale;
+        int sslot = q;
+        uint32_t sph = 0;
+        int aslot = g % p.a_slots;               // ring position of unit counter ug = it * units + u, first u = g
+        uint32_t aph = (uint32_t)((g / p.a_slots) & 1);
+        // SHARE (single accumulator stage, log-Mel): this warp also drains its share of the previous tile's accumulator --
+        // after its second K-step of the next tile, so that the MMAs find operands waiting when the drain releases them.
+        int pend_tile = -1, dstage = 0;
+        uint32_t dph = 0;
+        bool dep_done = false;
+        const uint32_t acc_empty_remote = mapa_cluster(BAR(V_ACC_EMPTY), 0);
+#define DRAIN_PENDING()                                                                                          \
+        do {                                                                                                     \
+            Tile2 dt;                                                                                            \
+            get_tile2<RAGGED>(p, pend_tile, dt);                                                                 \
+            const int drow = q * 32 + lane, dt0 = dt.t0 + (int)rank * 128;                                       \
+            const bool dvalid = (long long)(dt0 + drow) < dt.T;                                                  \
+            const int dc_off = dt.pass * p.nb;                                                                   \
+            const int dnm = p.n_mels - dc_off < p.nb ? p.n_mels - dc_off : p.nb;                                 \
+            float *doptr = p.feature_major ? p.out + ((long long)dt.clip * p.n_ch + dc_off) * dt.T + dt0 + drow   \
+                                           : p.out + (dt.f0 + dt0 + drow) * p.n_ch + dc_off;                     \
+            mbar_wait(BAR(V_ACC_FULL + dstage), dph);                                                            \
+            if (!dep_done) { asm volatile("griddepcontrol.wait;" ::: "memory"); dep_done = true; }               \
+            tc_fence_after();                                                                                    \
+            const uint32_t dtr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)dstage * (uint32_t)p.acc_cols; \
+            epi_fast_share(dtr, dtr + (uint32_t)p.nb, p.nb, dnm, doptr, p.feature_major ? dt.T : 1, dvalid,      \
+                           p.out_log10_offset, DRAIN0 + g, DRAINERS);                                            \
+            tc_fence_before();                                                                                   \
+            __syncwarp();                                                                                        \
+            if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)dstage * 8u);                         \
+            if (++dstage == p.acc_stages) { dstage = 0; dph ^= 1u; }                                             \
+            pend_tile = -1;                                                                                      \
+        } while (0)
+        for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+            TRACE(40);
+            const char *gxb = nullptr;   // DIRECT: this thread's frame in global memory
+            if (DIRECT) {
+                Tile2 ti;
+                get_tile2<RAGGED>(p, tile, ti);
+                const long long trow = ti.t0 + (int)rank * 128 + q * 32 + lane;
+                gxb = reinterpret_cast<const char *>(p.x + ti.s0 + (trow < ti.T ? trow : 0) * p.hop);   // rows of no frame re-read frame 0
+            } else {
+                mbar_wait(BAR(V_STG_FULL + sslot), sph);
+            }
+            if (RAGGED) {   // a template parameter: the dense instantiation must not carry this call in its converter loop
+                // ragged: group 0's warp realigns its chunk (see the loader), the other groups wait for it
+                if (g == 0) {
+                    ragged_realign(p.offsets, p.tile_prefix, p.n_clips, tile,
+                                   reinterpret_cast<float *>(smem + p.off_stg + (size_t)sslot * p.slot_bytes),
+                                   p.rows_per_chunk * (p.pitch_bytes >> 2), lane);
+                    if (lane == 0) mbar_arrive(BAR(V_STG_READY + sslot));
+                } else {
+                    mbar_wait(BAR(V_STG_READY + sslot), sph);
+                }
+            }
+            TRACE(41);
+            const uint32_t fb = row_off + (uint32_t)sslot * (uint32_t)p.slot_bytes;
+            bool released = false;
+            // The staged chunk is handed back to the loader as soon as this warp's last K-step of the tile has been read and
+            // folded (its samples are in registers), not after the operand store and its hand-off.
+#define STG_RELEASE_IF_LAST()                                                                       \
+            do {                                                                                    \
+                if (!DIRECT && u + NG >= p.units) {                                                 \
+                    __syncwarp();                                                                   \
+                    if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));                           \
+                    released = true;                                                                \
+                }                                                                                   \
+            } while (0)
+            int u = g;   // this group's K-steps: g, g + NG, ...
+            while (u < p.units) {
+                if (SHARE && pend_tile >= 0 && u >= g + 2 * NG) DRAIN_PENDING();
+                // ---- loads: NQ forward quads, NQ mirrored quads (+ one single when the mirrored run starts at 1 mod 4)
+                TRACE(42);
+                const short *tb = p.tab[u];
+                float fw[KS], bw[KS];
+#pragma unroll
+                for (int i = 0; i < NQ; ++i) {
+                    const float4 f = DIRECT ? ldg128(gxb + (int)tb[i]) : lds128(fb + (uint32_t)(int)tb[i]);
+                    fw[4 * i + 0] = f.x; fw[4 * i + 1] = f.y; fw[4 * i + 2] = f.z; fw[4 * i + 3] = f.w;
+                }
+                // mirrored partner of pair e is the sample at position KS-1-e of the descending run
+                if (SIGMA == 0) {
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i) {
+                        const float4 f = DIRECT ? ldg128(gxb + (int)tb[4 + i]) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs+4i .. rs+4i+3
+                        bw[KS - 1 - (4 * i + 0)] = f.x; bw[KS - 1 - (4 * i + 1)] = f.y;
+                        bw[KS - 1 - (4 * i + 2)] = f.z; bw[KS - 1 - (4 * i + 3)] = f.w;
+                    }
+                } else {
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i) {
+                        const float4 f = DIRECT ? ldg128(gxb + (int)tb[4 + i]) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs-1+4i .. rs+2+4i
+                        if (i > 0) bw[KS - 1 - (4 * i - 1)] = f.x;                  // position 4i-1 of the run
+                        bw[KS - 1 - (4 * i + 0)] = f.y; bw[KS - 1 - (4 * i + 1)] = f.z; bw[KS - 1 - (4 * i + 2)] = f.w;
+                    }
+                    bw[0] = DIRECT ? ldg32(gxb + (int)tb[8]) : lds32(fb + (uint32_t)(int)tb[8]);   // position KS-1 of the run
+                }
+                const uint32_t dst = lane_taddr + (uint32_t)aslot * (uint32_t)p.unit_cols;
+                if (PREC == P2_COMP) {
+                    // packed fp32 arithmetic (FMUL2 / FADD2): two folded pairs per instruction.  The mirrored samples are
+                    // scaled one by one, which also puts them in pair order at no cost; scaling by 2^s is exact, so
+                    // t + b == fma(f, S, b).
+                    uint32_t vsh[8], vsl[8], vdh[8], vdl[8];
+                    const uint64_t S2 = f2_pack(S_in, S_in);
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        const uint64_t t = f2_mul(f2_pack(fw[2 * c], fw[2 * c + 1]), S2);
+                        const uint64_t b = f2_pack(bw[2 * c] * S_in, bw[2 * c + 1] * S_in);
+                        const uint64_t s = f2_add(t, b), d = f2_sub(t, b);
+                        const __half2 sh = f2_to_half2(s), dh = f2_to_half2(d);
+                        const uint64_t sr = f2_sub(s, half2_to_f2(sh)), dr = f2_sub(d, half2_to_f2(dh));
+                        const __half2 sl = f2_to_half2(sr), dl = f2_to_half2(dr);
+                        vsh[c] = *reinterpret_cast<const uint32_t *>(&sh);
+                        vsl[c] = *reinterpret_cast<const uint32_t *>(&sl);
+                        vdh[c] = *reinterpret_cast<const uint32_t *>(&dh);
+                        vdl[c] = *reinterpret_cast<const uint32_t *>(&dl);
+                    }
+                    TRACE(43);
+                    STG_RELEASE_IF_LAST();
+                    mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    TRACE(44);
+                    tc_fence_after();
+                    tmem_st8(dst, vsh);
+                    tmem_st8(dst + 8, vsl);
+                    tmem_st8(dst + 16, vdh);
+                    tmem_st8(dst + 24, vdl);
+                } else if (PREC == P2_BF16) {
+                    uint32_t v[16];
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        const __nv_bfloat162 sh = __floats2bfloat162_rn(fw[2 * c] + bw[2 * c], fw[2 * c + 1] + bw[2 * c + 1]);
+                        const __nv_bfloat162 dh = __floats2bfloat162_rn(fw[2 * c] - bw[2 * c], fw[2 * c + 1] - bw[2 * c + 1]);
+                        v[c] = *reinterpret_cast<const uint32_t *>(&sh);
+                        v[8 + c] = *reinterpret_cast<const uint32_t *>(&dh);
+                    }
+                    TRACE(43);
+                    STG_RELEASE_IF_LAST();
+                    mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    TRACE(44);
+                    tc_fence_after();
+                    tmem_st16(dst, v);
+                } else {
+                    uint32_t v[16];
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        v[c] = cvt_tf32_rna(fw[c] + bw[c]);
+                        v[8 + c] = cvt_tf32_rna(fw[c] - bw[c]);
+                    }
+                    TRACE(43);
+                    STG_RELEASE_IF_LAST();
+                    mbar_wait(BAR(V_A_EMPTY + aslot), aph ^ 1u);   // the operand is ready in registers before the slot is
+                    TRACE(44);
+                    tc_fence_after();
+                    tmem_st16(dst, v);
+                }
+                // hand the slot to the MMA issuers right away: a slot is held only from its store to the end of its MMAs
+                tmem_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_remote(a_full_remote + (uint32_t)aslot * 8u);
+                TRACE(45);
+                // advance to this group's next K-step (the next tile's first one after the last)
+                int du = NG;
+                if (u + NG >= p.units) du = p.units - u + g;   // ug(next tile, u = g) - ug(this tile, u)
+                u += NG;
+                aslot += du;
+                while (aslot >= p.a_slots) { aslot -= p.a_slots; aph ^= 1u; }
+            }
+            if (!DIRECT && !released) {   // a group without K-steps in this geometry
+                __syncwarp();
+                if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));
+            }
+            sslot += 4;
+            if (sslot >= S) { sslot -= S; sph ^= 1u; }
+            if (SHARE) {
+                if (pend_tile >= 0) DRAIN_PENDING();   // short windows: fewer than three K-steps per group
+                pend_tile = tile;
+            }
+        }
+        if (SHARE && pend_tile >= 0) DRAIN_PENDING();   // the last tile
+#undef STG_RELEASE_IF_LAST
+#undef DRAIN_PENDING
+    }
+
+    // ------------------------------------------------------------------ teardown
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync_all();
+    if (warp == W_BASIS) tmem_dealloc2(tmem_base, 512);
+    TRACE_CTA(1);
+}
+
+
+// ---------------------------------------------------------------------------------------------- launch (per precision TU)
+template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM, bool DIRECT>
+static int launch_one_s(const K2Params &kp, int grid, cudaStream_t stream) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE, STREAM, DIRECT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
+        attr_done = true;
+    }
+    // Programmatic dependent launch: when the previous operation in the stream is another forward of this library, the
+    // CTAs of this grid are dispatched as soon as SMs of the previous grid free up (its clusters finish at different
+    // times: 384 tiles on 74 pairs), instead of after its last CTA has retired and a fresh launch has ramped up.  The
+    // kernel orders itself behind the previous grid (griddepcontrol.wait) before its first global store; it reads only
+    // the caller's signal and the plan's tables before that.  Any other predecessor serialises as usual.
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid, 1, 1);
+    cfg.blockDim = dim3(V2_THREADS, 1, 1);
+    cfg.dynamicSmemBytes = kp.smem_bytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    static const bool no_pdl = getenv("MELT_NO_PDL") != nullptr;   // debug switch
+    cfg.attrs = attr;
+    cfg.numAttrs = (no_pdl || kp.offsets != nullptr) ? 0 : 1;   // ragged: the scan kernel's results are read at kernel entry
+    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE, STREAM, DIRECT>, kp));
+    return MELT_OK;
+}
+
+template <int PREC, int SIGMA, bool RAGGED, int MODE>
+static int launch_one_r(const K2Params &kp, int grid, cudaStream_t stream) {
+    if (kp.direct) {   // dense, streamed basis only (plan_build_v2)
+        if (RAGGED) return fail(MELT_ERR_UNSUPPORTED, "internal: direct mode is dense only");
+        return launch_one_s<PREC, SIGMA, false, MODE, true, true>(kp, grid, stream);
+    }
+    return kp.b_resident ? launch_one_s<PREC, SIGMA, RAGGED, MODE, false, false>(kp, grid, stream)
+                         : launch_one_s<PREC, SIGMA, RAGGED, MODE, true, false>(kp, grid, stream);
+}
+
+template <int PREC, int SIGMA>
+static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
+    // Plain log-Mel output: no dedicated epilogue warps, three converter groups that also drain (MODE 2); everything else keeps
+    // the four epilogue warps (MODE 0).  (MODE 1, epilogue + converter warps draining a single-stage accumulator, measured the
+    // same as MODE 2 on cfg2 and is not instantiated.)
+    static const int forced = getenv("MELT_V2_MODE") ? atoi(getenv("MELT_V2_MODE")) : -1;   // debug switch: 0 forces the epilogue warps
+    const bool plain = kp.n_mfcc == 0 && !kp.output_power && kp.tap == nullptr;
+    const int mode = (plain && forced != 0) ? 2 : 0;
+    if (kp.offsets) return mode == 2 ? launch_one_r<PREC, SIGMA, true, 2>(kp, grid, stream) : launch_one_r<PREC, SIGMA, true, 0>(kp, grid, stream);
+    return mode == 2 ? launch_one_r<PREC, SIGMA, false, 2>(kp, grid, stream) : launch_one_r<PREC, SIGMA, false, 0>(kp, grid, stream);
+}
+
+
+}  // namespace melt
