@@ -729,7 +729,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             if (RAGGED) {   // a template parameter: the dense instantiation must not carry this call in its converter loop
                 // ragged: group 0's warp realigns its chunk (see the loader), the other groups wait for it
                 if (g == 0) {
-                    ragged_realign(p.offsets, p.tile_prefix, p.n_clips, tile,
+                    ragged_realign(p.offsets, p.tile_prefix, p.n_clips, p.passes > 1 ? tile / p.passes : tile,
                                    reinterpret_cast<float *>(smem + p.off_stg + (size_t)sslot * p.slot_bytes),
                                    p.rows_per_chunk * (p.pitch_bytes >> 2), lane);
                     if (lane == 0) mbar_arrive(BAR(V_STG_READY + sslot));

@@ -388,3 +388,52 @@ def test_back_to_back_forwards_into_one_buffer_keep_stream_order():
         np.testing.assert_array_equal(out.cpu().numpy().transpose(0, 2, 1).astype(np.float64), want)
     finally:
         mb.melt_plan_destroy(plan)
+
+
+# ------------------------------------------------------------------------------------------- CTA-pair kernel variants
+@pytest.mark.parametrize("n_fft,hop,n_mels,layout,expect", [
+    (400, 160, 160, "frame_major", "basis=streamed"),     # > 128 bins: two passes over the bins, basis streamed
+    (400, 160, 160, "feature_major", "basis=streamed"),
+    (1024, 256, 128, "frame_major", "basis=streamed"),    # long window: basis streamed, chunks staged
+    (2048, 512, 200, "frame_major", "staging=0 x"),       # chunks do not fit: frames read straight from global memory, two passes
+    (2048, 512, 96, "feature_major", "staging=0 x"),
+])
+def test_pair_kernel_streamed_direct_and_bin_passes(n_fft, hop, n_mels, layout, expect):
+    """16-byte aligned dense batches of these geometries run on the CTA-pair kernel in its streamed-basis / direct-load /
+    several-passes-over-the-bins forms (checked through melt_plan_describe); log and power outputs against the oracle."""
+    from paper_2606_01009_b200 import binding as mb
+    rng = np.random.default_rng(n_fft + hop + n_mels)
+    fs = 22050.0
+    c = dict(name="pair(%d,%d,%d,%s)" % (n_fft, hop, n_mels, layout), fs=fs, n_fft=n_fft, hop=hop, window=0,
+             n_mels=n_mels, fmin=0.0, fmax=fs / 2, n_mfcc=0, layout=layout)
+    plan = pu.plan_for(c)
+    try:
+        desc = mb.melt_plan_describe(plan)
+    finally:
+        mb.melt_plan_destroy(plan)
+    assert desc.startswith("melt_b200 v2") and expect in desc, desc
+    L = n_fft + 300 * hop                                  # 301 frames per clip = two 256-frame tiles, the second ragged
+    t = np.arange(L) / fs
+    x = np.stack([(0.3 * np.sin(2 * np.pi * rng.uniform(100, 9000) * t + rng.uniform(0, 6)) + rng.normal(0, 0.01, L))
+                  for _ in range(3)]).astype(np.float32)
+    _check_dense(c, x, "compensated", n_expect_frames=301, p_bar=COMP_P_BAR)
+
+
+def test_pair_kernel_ragged_log_mel_with_bin_passes():
+    """Ragged batch, plain log-Mel, 160 bins: ragged tile lookup + realignment + two passes over the bins together."""
+    orc = _orc()
+    rng = np.random.default_rng(77)
+    fs = 16000.0
+    c = dict(name="ragged160", fs=fs, n_fft=400, hop=160, window=0, n_mels=160, fmin=0.0, fmax=8000.0, n_mfcc=0,
+             layout="frame_major")
+    lens = rng.integers(3000, 90000, 9)
+    lens[3] = 399                                          # too short for a frame
+    off = np.zeros(len(lens) + 1, np.int64)
+    off[1:] = np.cumsum(lens)
+    x = rng.normal(0, 0.1, int(off[-1])).astype(np.float32)
+    x += (0.2 * np.sin(2 * np.pi * 1234.5 * np.arange(x.size) / fs)).astype(np.float32)
+    L_gpu, fo = pu.gpu_ragged(c, x, off, "compensated")
+    ref = orc.forward_ragged(x, off, want=("P", "L"), **pu.oracle_kwargs(c))
+    np.testing.assert_array_equal(fo, ref["frame_offsets"])
+    assert L_gpu.shape == ref["L"].shape and np.isfinite(L_gpu).all()
+    assert pu.log_error(L_gpu, ref["L"], ref["P"]) <= pu.LOG_BAR
