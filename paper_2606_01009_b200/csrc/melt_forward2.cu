@@ -43,9 +43,11 @@ int plan_build_v2(melt_plan *p) {
     k.a_col0 = k.acc_stages * k.acc_cols;
     k.a_slots = std::min(V2_MAX_A_SLOTS, (512 - k.a_col0) / k.unit_cols);
     if (k.a_slots < 2) return MELT_OK;
-    k.rows_per_chunk = 32 + (N - 1) / H;
-    if (k.rows_per_chunk > 64) return MELT_OK;
     const int pitch_words = ((H / 4) & 1) ? H : H + 4;   // pitch / 4 odd: 8 consecutive rows hit 8 distinct 16-byte bank groups
+    // hop-rows a 32-frame chunk touches; one more when the rows carry no padding words: a ragged chunk is fetched from up to
+    // three samples below its start and shifted down, which needs those samples at the end of the last row
+    k.rows_per_chunk = 32 + (N - 1) / H + (pitch_words == H ? 1 : 0);
+    if (k.rows_per_chunk > 64) return MELT_OK;
     k.pitch_bytes = pitch_words * 4;
     k.slot_bytes = round_up2(k.rows_per_chunk * k.pitch_bytes, 128);   // tensor-map boxes land on 128-byte boundaries
     k.kind_bytes = (uint32_t)(k.nb / 2) * 32u;
@@ -58,19 +60,19 @@ int plan_build_v2(melt_plan *p) {
     // The basis half stays resident when that leaves room for at least five staging slots; otherwise (long windows) its
     // K-step slabs are streamed from L2 through the deepest ring (<= 8 slabs) that still leaves five slots.
     k.b_resident = 1; k.b_slots = k.units;
-    if (k.passes > 1) { k.b_resident = 0; k.b_slots = std::min(8, k.units - 1); }   // every pass needs other rows: streamed
+    if (k.passes > 1) { k.b_resident = 0; k.b_slots = std::min(8, k.units); }   // every pass needs other rows: streamed
     for (;;) {
         const uint32_t ring_bytes = (uint32_t)k.b_slots * k.unit_b_bytes;
         k.off_stg = (uint32_t)round_up2((int)ring_bytes, 128) + 128;  // 128-byte zero guard in front of the staging ring
         const long long room = (long long)SMEM_BUDGET - k.off_stg - 128 - dct_bytes - bar_bytes - 256;
         k.stg_slots = (int)std::min<long long>(room > 0 ? room / k.slot_bytes : 0, V2_MAX_STG);
         if (k.stg_slots >= 5) break;
-        if (k.b_resident) { k.b_resident = 0; k.b_slots = std::min(8, k.units - 1); }
+        if (k.b_resident) { k.b_resident = 0; k.b_slots = std::min(8, k.units); }
         else --k.b_slots;
-        if (k.b_slots < 3) {
+        if (k.b_slots < std::min(3, k.units)) {   // the issuers take two K-steps per iteration: two different slabs at least
             // not even a streamed basis leaves room for staged chunks (windows of thousands of samples): no staging at all,
             // the converter threads read their frames from global memory (L2 serves the 4x frame overlap)
-            k.direct = 1; k.b_slots = std::min(8, k.units - 1); k.stg_slots = 0;
+            k.direct = 1; k.b_slots = std::min(8, k.units); k.stg_slots = 0;
             k.off_stg = (uint32_t)round_up2((int)((uint32_t)k.b_slots * k.unit_b_bytes), 128) + 128;
             break;
         }

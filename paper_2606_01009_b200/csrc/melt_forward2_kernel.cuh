@@ -235,7 +235,8 @@ static __device__ __noinline__ void ragged_realign(const long long *offsets, con
     const int dlt = (int)(__ldg(offsets + lo) & 3);
     if (dlt) {
         const int n = n_words - dlt;
-        for (int i = lane; i < n; i += 128) {
+        for (int base = 0; base < n; base += 128) {   // warp-uniform trip count: the loop body synchronises the warp
+            const int i = base + lane;
             float v[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j) v[j] = (i + 32 * j < n) ? w[i + 32 * j + dlt] : 0.f;

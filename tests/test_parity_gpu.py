@@ -437,3 +437,29 @@ def test_pair_kernel_ragged_log_mel_with_bin_passes():
     np.testing.assert_array_equal(fo, ref["frame_offsets"])
     assert L_gpu.shape == ref["L"].shape and np.isfinite(L_gpu).all()
     assert pu.log_error(L_gpu, ref["L"], ref["P"]) <= pu.LOG_BAR
+
+
+@pytest.mark.parametrize("n_fft,hop,n_mels", [
+    (512, 128, 80),    # chunk of 35 x 132 words: the realignment loop's last round is partial (found by fuzzing: hang)
+    (800, 160, 23),
+    (16, 4, 128),      # rows without padding words: the shifted chunk needs one more hop-row (found by fuzzing)
+    (896, 128, 23),
+])
+def test_ragged_unaligned_clip_starts_other_geometries(n_fft, hop, n_mels):
+    """Ragged batches whose clips start at arbitrary samples (realignment in shared memory) for geometries other than
+    configs[3]'s; includes empty clips, a clip of exactly one frame and clips longer than a tile."""
+    orc = _orc()
+    rng = np.random.default_rng(n_fft * 7 + hop)
+    c = dict(name="rag(%d,%d,%d)" % (n_fft, hop, n_mels), fs=16000.0, n_fft=n_fft, hop=hop, window=1, n_mels=n_mels, fmin=0.0,
+             fmax=8000.0, n_mfcc=0, layout="frame_major")
+    lens = rng.integers(0, 40 * hop + n_fft, 9)
+    lens[2] = n_fft
+    lens[5] += 300 * hop + 1
+    off = np.zeros(len(lens) + 1, np.int64)
+    off[1:] = np.cumsum(lens)
+    x = rng.normal(0, 0.1, int(off[-1])).astype(np.float32)
+    L_gpu, fo = pu.gpu_ragged(c, x, off, "compensated")
+    ref = orc.forward_ragged(x, off, want=("P", "L"), **pu.oracle_kwargs(c))
+    np.testing.assert_array_equal(fo, ref["frame_offsets"])
+    assert np.isfinite(L_gpu).all()
+    assert pu.log_error(L_gpu, ref["L"], ref["P"]) <= pu.LOG_BAR
