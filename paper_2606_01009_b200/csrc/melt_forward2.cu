@@ -54,7 +54,10 @@ int plan_build_v2(melt_plan *p) {
     k.unit_b_bytes = (uint32_t)k.nk * k.kind_bytes;
     k.dct_pitch = k1.dct_pitch;
     const uint32_t b_bytes = (uint32_t)k.units * k.unit_b_bytes;
-    const uint32_t dct_bytes = p->n_mfcc > 0 ? (uint32_t)(M * k.dct_pitch * 4) : 0;
+    const uint32_t dct_only = p->n_mfcc > 0 ? (uint32_t)(M * k.dct_pitch * 4) : 0;
+    // MFCCT, frame-major: 4 epilogue warps x 32 frames x n_mfcc floats behind the DCT table (cepstra transposed for coalesced stores)
+    const uint32_t epi_bytes = (p->n_mfcc > 0 && p->layout == MELT_LAYOUT_FRAME_MAJOR) ? (uint32_t)(4 * 32 * p->n_mfcc * 4) : 0;
+    const uint32_t dct_bytes = dct_only + epi_bytes;
     const uint32_t bar_bytes = (uint32_t)round_up2(V_NBARS * 8 + 16, 128);
     k.off_b = 0;
     // The basis half stays resident when that leaves room for at least five staging slots; otherwise (long windows) its
@@ -78,6 +81,7 @@ int plan_build_v2(melt_plan *p) {
         }
     }
     k.off_dct = (uint32_t)round_up2((int)(k.off_stg + (uint32_t)k.stg_slots * k.slot_bytes + 128), 128);
+    k.off_epi = epi_bytes ? k.off_dct + dct_only : 0;
     k.off_bar = (uint32_t)round_up2((int)(k.off_dct + dct_bytes), 128);
     k.smem_bytes = k.off_bar + bar_bytes;
     if (k.smem_bytes > (uint32_t)SMEM_BUDGET) return MELT_OK;

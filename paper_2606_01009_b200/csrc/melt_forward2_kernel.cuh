@@ -143,7 +143,8 @@ __device__ __forceinline__ void epi_fast_share(uint32_t t_r, uint32_t t_i, int n
 // matrix, optional DCT-II with 4 * KQ accumulators (KQ = 0: no DCT).  Returns after handing the accumulator stage back.
 template <int KQ>
 __device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uint32_t t_i, const float *dct_s, float *optr, float *tptr,
-                                            long long cstride, bool valid, int lane, uint32_t acc_empty_bar, int nm) {
+                                            long long cstride, bool valid, int lane, uint32_t acc_empty_bar, int nm,
+                                            float *stage, float *warp_out, int nvalid) {
     const float kLog10_2 = 0.30102999566398120f;
     float cacc[KQ > 0 ? 4 * KQ : 1];
 #pragma unroll
@@ -182,7 +183,19 @@ __device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uin
     tc_fence_before();
     __syncwarp();
     if (lane == 0) mbar_arrive_remote(acc_empty_bar);
-    if (KQ > 0 && valid) {                                                                      // Eq. (9)
+    if (KQ > 0 && stage != nullptr) {                                                           // Eq. (9)
+        // frame-major cepstra: the 32 frames of this warp are 32 * n_mfcc consecutive floats of the output.  Every thread
+        // parks its row in shared memory, then the warp writes the block with consecutive lanes on consecutive addresses
+        // (a thread storing its own row touches n_mfcc scattered 4-byte pieces: 13x the sector traffic for 13 cepstra).
+        const int K = p.n_mfcc;
+#pragma unroll
+        for (int k = 0; k < 4 * KQ; ++k)
+            if (k < K) stage[lane * K + k] = cacc[k];
+        __syncwarp();
+        const int n_out = nvalid * K;
+        for (int w = lane; w < n_out; w += 32) warp_out[w] = stage[w];
+        __syncwarp();
+    } else if (KQ > 0 && valid) {
 #pragma unroll
         for (int k = 0; k < 4 * KQ; ++k)
             if (k < p.n_mfcc) optr[k * cstride] = cacc[k];
@@ -669,10 +682,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
             } else {
                 const uint32_t eb = acc_empty_remote + (uint32_t)stage * 8u;
-                if (p.n_mfcc == 0) epi_generic<0>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm);
-                else if (p.dct_pitch <= 16) epi_generic<4>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm);
-                else if (p.dct_pitch <= 40) epi_generic<10>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm);
-                else epi_generic<16>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm);
+                // frame-major MFCCT with a staging block: this warp's 32 frames start at row (t0 + 32 q) of the clip
+                float *estage = (p.off_epi && !p.feature_major) ? reinterpret_cast<float *>(smem + p.off_epi) + q * 32 * p.n_mfcc : nullptr;
+                float *ewout = p.out + (ti.f0 + t0 + q * 32) * p.n_ch;
+                const long long erem = T - (long long)(t0 + q * 32);
+                const int envalid = erem <= 0 ? 0 : (erem < 32 ? (int)erem : 32);
+                if (p.n_mfcc == 0) epi_generic<0>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
+                else if (p.dct_pitch <= 16) epi_generic<4>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
+                else if (p.dct_pitch <= 40) epi_generic<10>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
+                else epi_generic<16>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
             }
             TRACE(32);
             if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }

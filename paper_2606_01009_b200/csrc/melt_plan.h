@@ -71,6 +71,7 @@ struct K2Params {
     // ---- basis (this CTA's half: nb/2 rows per kind)
     uint32_t unit_b_bytes, kind_bytes;
     uint32_t off_b, off_stg, off_dct, off_bar, smem_bytes;
+    uint32_t off_epi;          // MFCCT, frame-major: per epilogue warp 32 x n_mfcc floats to transpose the cepstra for coalesced stores (0 = none)
     int dct_pitch;
     float in_scale, out_scale, out_log10_offset;
     int output_power, feature_major;
