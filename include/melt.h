@@ -79,8 +79,11 @@ typedef enum {
 
 typedef enum {
     MELT_PAD_NONE = 0,   /* T = floor((len - n_fft)/hop) + 1 frames per clip; tail samples ignored */
-    MELT_PAD_REFLECT = 1 /* the clip is virtually reflect-padded by n_fft/2 per side (edge sample not repeated);
-                            T = floor(len/hop) + 1 for even n_fft; needs len > n_fft/2 */
+    MELT_PAD_REFLECT = 1 /* the clip is reflect-padded by n_fft/2 per side (edge sample not repeated);
+                            T = floor(len/hop) + 1 for even n_fft; needs len > n_fft/2.  On the fast path the padded signal is
+                            written once into a plan-owned device copy (allocated at the first such forward call and re-allocated,
+                            after a stream synchronisation, only when a later call needs more room; forwards of one plan that
+                            use it must then be issued on one stream at a time) */
 } melt_pad;
 
 typedef enum {

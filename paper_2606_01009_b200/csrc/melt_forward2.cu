@@ -32,7 +32,8 @@ int plan_build_v2(melt_plan *p) {
     k.nb = round_up2((M + k.passes - 1) / k.passes, 16);
     if (k.nb < 32) k.nb = 32;
     // ---- what the kernel covers (everything else stays on the general v1 kernel)
-    if (k.units > V2_MAX_UNITS || (H & 3) || (k1.a0 & 3) || p->pad != MELT_PAD_NONE) return MELT_OK;
+    if (k.units > V2_MAX_UNITS || (H & 3) || (k1.a0 & 3)) return MELT_OK;
+    if (p->pad != MELT_PAD_NONE && (N & 7)) return MELT_OK;   // reflect padding: the padded copy keeps every clip start 16-byte aligned
     if (k.passes > 1 && p->n_mfcc > 0) return MELT_OK;             // the DCT needs all bins of a frame in one pass
     const int rs = k1.b0 - (k.kstep - 1);           // lowest sample of the mirrored run of unit 0
     const int sigma = ((rs % 4) + 4) % 4;
@@ -235,6 +236,44 @@ int v2_encode_tmap_ragged(K2Params &k) {
 
 bool v2_accepts(const melt_plan *p, const float *x, long long len) {
     return p->v2_ok && (((uintptr_t)x & 15) == 0) && ((len & 3) == 0);
+}
+
+// Reflect padding for the CTA-pair kernel: xp[b][i] = x[b][rho(i - pad)], rho(j) = -j for j < 0, 2 (len - 1) - j for j >= len
+// (edge sample not repeated), i in [0, len + 2 pad).  One pass over the signal into a plan-owned copy.
+__global__ void reflect_pad_kernel(const float *__restrict__ x, float *__restrict__ xp, long long len, int pad, long long plen, int vec) {
+    const long long b = blockIdx.y;
+    const float *xb = x + b * len;
+    float *pb = xp + b * plen;
+    const long long stride = (long long)gridDim.x * blockDim.x, t0 = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (vec) {   // interior as 16-byte copies (x, len and pad are all 16-byte aligned), the 2 * pad reflected samples one by one
+        const float4 *src = reinterpret_cast<const float4 *>(xb);
+        float4 *dst = reinterpret_cast<float4 *>(pb + pad);
+        for (long long i = t0; i < len / 4; i += stride) dst[i] = __ldg(src + i);
+        for (long long i = t0; i < 2LL * pad; i += stride) {
+            const long long ip = i < pad ? i : len + i;          // position in the padded clip
+            long long j = ip - pad;
+            if (j < 0) j = -j;
+            if (j >= len) j = 2 * (len - 1) - j;
+            pb[ip] = xb[j];
+        }
+        return;
+    }
+    for (long long i = t0; i < plen; i += stride) {
+        long long j = i - pad;
+        if (j < 0) j = -j;
+        if (j >= len) j = 2 * (len - 1) - j;
+        pb[i] = xb[j];
+    }
+}
+
+int launch_reflect_pad(const float *x, float *xp, int batch, long long len, int pad, cudaStream_t stream) {
+    const long long plen = len + 2LL * pad;
+    const int vec = (((uintptr_t)x & 15) == 0) && (len % 4 == 0) && (pad % 4 == 0);
+    const long long work = vec ? len / 4 : plen;
+    const int bx = (int)std::max<long long>(1, std::min<long long>((work + 511) / 512, 2048));
+    reflect_pad_kernel<<<dim3((unsigned)bx, (unsigned)batch), 256, 0, stream>>>(x, xp, len, pad, plen, vec);
+    MELT_CUDA(cudaGetLastError());
+    return MELT_OK;
 }
 
 int launch_forward2(const melt_plan *pl, const K2Params &kp, cudaStream_t stream) {

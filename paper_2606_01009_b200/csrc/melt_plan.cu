@@ -261,8 +261,29 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
         if (T == 0) return MELT_OK;
         const long long tpc = (T + TILE_M - 1) / TILE_M;
         if (tpc * n_clips > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
-        if (v2_accepts(p, x, len) && !(tap && ((uintptr_t)tap & 3))) {
+        // reflect padding: the padded copy is aligned whatever x is; it only needs a length that keeps the clip starts aligned
+        const bool v2_in = p->pad == MELT_PAD_REFLECT ? (p->v2_ok && ((len + p->n_fft) & 3) == 0 && !(p->n_fft & 1)) : v2_accepts(p, x, len);
+        if (v2_in && !(tap && ((uintptr_t)tap & 3))) {
             K2Params k2 = p->k2;
+            if (p->pad == MELT_PAD_REFLECT) {
+                // in-library reflect padding on the fast path: one pass writes the padded signal into a plan-owned copy (allocated
+                // on the first such call, re-allocated only for a bigger batch), the kernel then frames the copy
+                const int padn = p->n_fft / 2;
+                const long long plen = len + 2LL * padn;
+                const size_t need = (size_t)n_clips * (size_t)plen * sizeof(float);
+                melt_plan *mp = const_cast<melt_plan *>(p);
+                if (need > mp->ws_pad_bytes) {
+                    MELT_CUDA(cudaStreamSynchronize(st));
+                    cudaFree(mp->ws_pad);
+                    mp->ws_pad = nullptr; mp->ws_pad_bytes = 0;
+                    if (cudaMalloc(&mp->ws_pad, need) != cudaSuccess) { (void)cudaGetLastError(); return fail(MELT_ERR_ALLOC, "padded-signal workspace of %zu bytes", need); }
+                    mp->ws_pad_bytes = need;
+                }
+                rc = launch_reflect_pad(x, mp->ws_pad, n_clips, len, padn, st);
+                if (rc) return rc;
+                x = mp->ws_pad;
+                len = plen;
+            }
             const long long tpc2 = (T + 255) / 256;
             if (tpc2 * n_clips * std::max(1, p->k2.passes) > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
             k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = len; k2.frames_per_clip = T;
@@ -310,6 +331,7 @@ extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window
     p->d_bimg = nullptr; p->d_bimg2 = nullptr; p->v2_ok = false; p->v2_sigma = 0; p->d_tab = nullptr; p->d_dct = nullptr; p->d_tile_prefix = nullptr; p->d_frame_offsets_scratch = nullptr;
     memset(&p->kp, 0, sizeof(p->kp));
     p->ws_in = nullptr; p->ws_out = nullptr; p->ws_in_bytes = p->ws_out_bytes = 0;
+    p->ws_pad = nullptr; p->ws_pad_bytes = 0;
     // Eq. (1)-(2): M centres uniformly spaced in mel between fmin and fmax, endpoints excluded
     p->centres.resize(n_mels);
     const double mlo = hz_to_mel(fmin), mhi = hz_to_mel(fmax);
@@ -332,6 +354,7 @@ extern "C" void melt_plan_destroy(melt_plan *p) {
     cudaFree(p->d_tile_prefix);
     cudaFree(p->ws_in);
     cudaFree(p->ws_out);
+    cudaFree(p->ws_pad);
     delete p;
 }
 
