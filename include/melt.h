@@ -124,8 +124,9 @@ int melt_plan_get_centres(const melt_plan *plan, double *f_hz);
 
 /*
  * melt_forward -- the whole hot path on a dense batch.
- *   x    device, fp32, [batch, len] contiguous, 4-byte aligned (16-byte alignment of every clip start, i.e. of x
- *        and of len*4, enables the vectorised loader);
+ *   x    device, fp32, [batch, len] contiguous, 4-byte aligned.  When every clip start is 16-byte aligned (x and len*4)
+ *        the kernel frames x in place; otherwise one pass first copies the batch into a plan-owned buffer at an aligned
+ *        clip stride (allocated at the first such call, see MELT_PAD_REFLECT);
  *   out  device, fp32, batch * C * T floats, T = melt_num_frames(plan, len), layout per MELT_OPT_LAYOUT.
  * batch == 0 or T == 0 is a successful no-op.  Returns a melt_status.
  */

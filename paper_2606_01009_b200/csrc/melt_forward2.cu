@@ -249,11 +249,12 @@ __global__ void reflect_pad_kernel(const float *__restrict__ x, float *__restric
         const float4 *src = reinterpret_cast<const float4 *>(xb);
         float4 *dst = reinterpret_cast<float4 *>(pb + pad);
         for (long long i = t0; i < len / 4; i += stride) dst[i] = __ldg(src + i);
-        for (long long i = t0; i < 2LL * pad; i += stride) {
+        for (long long i = t0; i < plen - len; i += stride) {
             const long long ip = i < pad ? i : len + i;          // position in the padded clip
             long long j = ip - pad;
             if (j < 0) j = -j;
             if (j >= len) j = 2 * (len - 1) - j;
+            if (j < 0) j = 0;   // filler samples of very short clips (never read by a frame)
             pb[ip] = xb[j];
         }
         return;
@@ -262,12 +263,12 @@ __global__ void reflect_pad_kernel(const float *__restrict__ x, float *__restric
         long long j = i - pad;
         if (j < 0) j = -j;
         if (j >= len) j = 2 * (len - 1) - j;
+        if (j < 0) j = 0;
         pb[i] = xb[j];
     }
 }
 
-int launch_reflect_pad(const float *x, float *xp, int batch, long long len, int pad, cudaStream_t stream) {
-    const long long plen = len + 2LL * pad;
+int launch_reflect_pad(const float *x, float *xp, int batch, long long len, int pad, long long plen, cudaStream_t stream) {   // plen >= len + 2 pad
     const int vec = (((uintptr_t)x & 15) == 0) && (len % 4 == 0) && (pad % 4 == 0);
     const long long work = vec ? len / 4 : plen;
     const int bx = (int)std::max<long long>(1, std::min<long long>((work + 511) / 512, 2048));

@@ -262,14 +262,17 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
         const long long tpc = (T + TILE_M - 1) / TILE_M;
         if (tpc * n_clips > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
         // reflect padding: the padded copy is aligned whatever x is; it only needs a length that keeps the clip starts aligned
-        const bool v2_in = p->pad == MELT_PAD_REFLECT ? (p->v2_ok && ((len + p->n_fft) & 3) == 0 && !(p->n_fft & 1)) : v2_accepts(p, x, len);
+        // and a batch that is not 16-byte aligned (pointer or clip length) takes the same route with a pad of zero samples:
+        // one pass copies it into the plan-owned buffer at an aligned clip stride
+        const bool realign = p->pad == MELT_PAD_NONE && p->v2_ok && !v2_accepts(p, x, len);
+        const bool v2_in = p->pad == MELT_PAD_REFLECT ? (p->v2_ok && ((len + p->n_fft) & 3) == 0 && !(p->n_fft & 1)) : p->v2_ok;
         if (v2_in && !(tap && ((uintptr_t)tap & 3))) {
             K2Params k2 = p->k2;
-            if (p->pad == MELT_PAD_REFLECT) {
+            if (p->pad == MELT_PAD_REFLECT || realign) {
                 // in-library reflect padding on the fast path: one pass writes the padded signal into a plan-owned copy (allocated
                 // on the first such call, re-allocated only for a bigger batch), the kernel then frames the copy
-                const int padn = p->n_fft / 2;
-                const long long plen = len + 2LL * padn;
+                const int padn = realign ? 0 : p->n_fft / 2;
+                const long long plen = realign ? ((len + 3) & ~3LL) : len + 2LL * padn;   // realign: up to 3 filler samples no frame reads
                 const size_t need = (size_t)n_clips * (size_t)plen * sizeof(float);
                 melt_plan *mp = const_cast<melt_plan *>(p);
                 if (need > mp->ws_pad_bytes) {
@@ -279,7 +282,7 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
                     if (cudaMalloc(&mp->ws_pad, need) != cudaSuccess) { (void)cudaGetLastError(); return fail(MELT_ERR_ALLOC, "padded-signal workspace of %zu bytes", need); }
                     mp->ws_pad_bytes = need;
                 }
-                rc = launch_reflect_pad(x, mp->ws_pad, n_clips, len, padn, st);
+                rc = launch_reflect_pad(x, mp->ws_pad, n_clips, len, padn, plen, st);
                 if (rc) return rc;
                 x = mp->ws_pad;
                 len = plen;

@@ -133,7 +133,7 @@ int launch_forward(const melt_plan *p, const KParams &kp, cudaStream_t stream);
 int plan_build_v2(melt_plan *p);   // fills p->k2 / p->v2_ok (never fails the plan: v1 remains the general path)
 bool v2_accepts(const melt_plan *p, const float *x, long long len);
 int launch_forward2(const melt_plan *p, const K2Params &kp, cudaStream_t stream);
-int launch_reflect_pad(const float *x, float *xp, int batch, long long len, int pad, cudaStream_t stream);
+int launch_reflect_pad(const float *x, float *xp, int batch, long long len, int pad, long long plen, cudaStream_t stream);
 int v2_encode_tmap(K2Params &kp);
 int v2_encode_tmap_ragged(K2Params &kp);   // 2-D map over the packed buffer (any start sample, rows of `hop` samples)   // fills kp.tmap / kp.tma_rows for this call's (x, len, batch); never fails the call
 int launch_ragged_scan(const melt_plan *p, const long long *offsets, int n_clips, long long *frame_offsets, int tile_m, cudaStream_t stream);
