@@ -97,11 +97,13 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 // Optional event trace (development builds only, -DMELT_TRACE): lane 0 of every warp of cluster 0 appends (tag, clock) pairs.
 #ifdef MELT_TRACE
 extern __device__ long long *g_melt_trace;   // [2 ranks][16 warps][1024] events
+#define TRACE_PT(i) do { if (g_melt_trace && threadIdx.x == 0) g_melt_trace[2 * 16 * 1024 + 592 + blockIdx.x * 8 + (i)] = clock64(); } while (0)
 #define TRACE_DECL int tr_n = 0; long long *tr_buf = (g_melt_trace && cluster_id_x() == 0 && (threadIdx.x & 31) == 0) ? g_melt_trace + ((size_t)cluster_ctarank() * 16 + (threadIdx.x >> 5)) * 1024 : nullptr;
 #define TRACE(tag) do { if (tr_buf && tr_n < 1023) tr_buf[++tr_n] = ((long long)(tag) << 48) | (clock64() & 0xFFFFFFFFFFFFll); if (tr_buf) tr_buf[0] = tr_n; } while (0)
-#define TRACE_CTA(which) do { if (g_melt_trace && threadIdx.x == 0) g_melt_trace[2 * 16 * 1024 + blockIdx.x * 2 + (which)] = (long long)globaltimer_ns(); } while (0)
+#define TRACE_CTA(which) do { if (g_melt_trace && threadIdx.x == 0) { g_melt_trace[2 * 16 * 1024 + blockIdx.x * 2 + (which)] = (long long)globaltimer_ns(); g_melt_trace[2 * 16 * 1024 + 296 + blockIdx.x * 2 + (which)] = clock64(); } } while (0)
 #else
 #define TRACE_CTA(which) do { } while (0)
+#define TRACE_PT(i) do { } while (0)
 #define TRACE_DECL
 #define TRACE(tag) do { } while (0)
 #endif
@@ -263,6 +265,7 @@ static __device__ __noinline__ void ragged_realign(const long long *offsets, con
     __syncwarp();
 }
 
+static_assert(V_NBARS <= V2_THREADS, "one thread per barrier at set-up");
 template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM, bool DIRECT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
     extern __shared__ __align__(128) uint8_t smem[];
@@ -305,17 +308,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             }
         }
     }
-    if (tid == 0) {
-        for (int i = 0; i < V2_MAX_STG; ++i) { mbar_init(BAR(V_STG_FULL + i), 1); mbar_init(BAR(V_STG_EMPTY + i), NG); }
-        for (int i = 0; i < V2_MAX_A_SLOTS; ++i) { mbar_init(BAR(V_A_FULL + i), 8); mbar_init(BAR(V_A_EMPTY + i), 2); }   // both issuers commit
-        for (int i = 0; i < 2; ++i) { mbar_init(BAR(V_ACC_FULL + i), 2); mbar_init(BAR(V_ACC_EMPTY + i), SHARE ? 8 * DRAINERS : 8); }
-        for (int i = 0; i < p.b_slots; ++i) { mbar_init(BAR(V_B_FULL + i), 1); mbar_init(BAR(V_B_PEER + i), 1); }   // b_slots = units when resident
-        mbar_init(BAR(V_DONE), 2);   // both MMA issuers
-        if (STREAM)
-            for (int i = 0; i < 8; ++i) mbar_init(BAR(V_B_EMPTY + i), 2);   // streamed basis: both issuers release a slab
-        for (int i = 0; i < V2_MAX_STG; ++i) mbar_init(BAR(V_STG_READY + i), 1);
+    // every barrier of the block is set up by a thread of its own (one thread doing all of them costs ~2000 cycles per launch)
+    if (tid < V_NBARS) {
+        const int i = tid;
+        const uint32_t count = i < V_STG_EMPTY ? 1u : i < V_A_FULL ? (uint32_t)NG : i < V_A_EMPTY ? 8u
+                             : i < V_ACC_EMPTY ? 2u                                    // A_EMPTY, ACC_FULL: both issuers commit
+                             : i < V_B_FULL ? (uint32_t)(SHARE ? 8 * DRAINERS : 8)     // ACC_EMPTY
+                             : i < V_DONE ? 1u                                         // B_FULL, B_PEER
+                             : i == V_DONE ? 2u                                        // both MMA issuers
+                             : i < V_B_EMPTY ? 1u : 2u;                                // STG_READY; B_EMPTY: both issuers release a slab
+        mbar_init(BAR(i), count);
         fence_barrier_init();
     }
+    TRACE_PT(1);
     if (warp == W_BASIS) {
         tmem_alloc2(smem_u32(tmem_ptr_s), 512);
         tmem_relinquish2();
@@ -328,10 +333,18 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     }
     if (p.n_mfcc > 0)
         for (int i = tid; i < p.n_mels * p.dct_pitch; i += V2_THREADS) dct_s[i] = __ldg(p.dct + i);
+    TRACE_PT(2);
     fence_proxy_async_smem();  // the zero fill (generic proxy) is ordered before the bulk copies (async proxy) that follow
     tc_fence_before();
     __syncthreads();
+    TRACE_PT(3);
+#ifdef MELT_STRICT_CLUSTER_SYNC
     cluster_sync_all();
+#else
+    cluster_arrive_relaxed();   // barrier set-up is published by fence.mbarrier_init; everything else set up here is CTA-local
+    cluster_wait();
+#endif
+    TRACE_PT(4);
     tc_fence_after();
     const uint32_t tmem_base = *tmem_ptr_s;
     if (tid == 0) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the next forward may start filling freed SMs
@@ -595,6 +608,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             // others, is awaited by both CTAs before they retire.
             if (elect_one()) tc_commit2(BAR(V_DONE), 3);
             __syncwarp();
+            // Likewise the peer's last accumulator releases (remote arrivals on this CTA's barriers that no later tile waits
+            // for): this CTA takes them before it retires, so that the exit barrier below needs no memory ordering.
+            for (int k = 0; k < acc_stages; ++k) {
+                mbar_wait(BAR(V_ACC_EMPTY + stage), sph ^ 1u);
+                if (++stage == acc_stages) { stage = 0; sph ^= 1u; }
+            }
         }
     } else if (MODE != 2 && warp >= W_EPI0 && warp < W_EPI0 + 4) {
         // ============================================================== epilogue (thread = frame)
@@ -734,6 +753,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             if (++dstage == p.acc_stages) { dstage = 0; dph ^= 1u; }                                             \
             pend_tile = -1;                                                                                      \
         } while (0)
+        int u = g;
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             TRACE(40);
             const char *gxb = nullptr;   // DIRECT: this thread's frame in global memory
@@ -769,9 +789,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     released = true;                                                                \
                 }                                                                                   \
             } while (0)
-            int u = g;   // this group's K-steps: g, g + NG, ...
+            // this group's K-steps: every NG-th of the running count over the CTA's tiles (u carries over from the previous
+            // tile), so that a K-step count that NG does not divide is spread evenly over the groups
+            const int u0 = u;
             while (u < p.units) {
-                if (SHARE && pend_tile >= 0 && u >= g + 2 * NG) DRAIN_PENDING();
+                if (SHARE && pend_tile >= 0 && u >= u0 + 2 * NG) DRAIN_PENDING();
                 // ---- loads: NQ forward quads, NQ mirrored quads (+ one single when the mirrored run starts at 1 mod 4)
                 TRACE(42);
                 const short *tb = p.tab[u];
@@ -862,13 +884,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 __syncwarp();
                 if (lane == 0) mbar_arrive_remote(a_full_remote + (uint32_t)aslot * 8u);
                 TRACE(45);
-                // advance to this group's next K-step (the next tile's first one after the last)
-                int du = NG;
-                if (u + NG >= p.units) du = p.units - u + g;   // ug(next tile, u = g) - ug(this tile, u)
+                // advance to this group's next K-step
                 u += NG;
-                aslot += du;
+                aslot += NG;
                 while (aslot >= p.a_slots) { aslot -= p.a_slots; aph ^= 1u; }
             }
+            u -= p.units;   // position in the next tile
             if (!DIRECT && !released) {   // a group without K-steps in this geometry
                 __syncwarp();
                 if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));
@@ -886,9 +907,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     }
 
     // ------------------------------------------------------------------ teardown
+    TRACE_PT(5);
     tc_fence_before();
     __syncthreads();
+    TRACE_PT(6);
+#ifdef MELT_STRICT_CLUSTER_SYNC
     cluster_sync_all();
+#else
+    // execution barrier only: every cross-CTA arrival has been waited for (the DONE commit, the accumulator releases above);
+    // with release semantics the barrier would wait ~1500 cycles for this CTA's last output stores to be performed
+    cluster_arrive_relaxed();
+    cluster_wait();
+#endif
+    TRACE_PT(7);
     if (warp == W_BASIS) tmem_dealloc2(tmem_base, 512);
     TRACE_CTA(1);
 }

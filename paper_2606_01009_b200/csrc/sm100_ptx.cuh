@@ -203,6 +203,10 @@ __device__ __forceinline__ uint32_t cluster_nid_x() {
 __device__ __forceinline__ void cluster_sync_all() {  // every thread of every CTA of the cluster
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
+// the two halves of a cluster barrier without memory ordering (execution only): barrier set-up made visible by
+// fence.mbarrier_init, and exits that only have to wait for the peer to get there
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 // shared::cta address of this CTA -> shared::cluster address of the same offset in CTA `rank` of the cluster
 __device__ __forceinline__ uint32_t mapa_cluster(uint32_t smem_addr, uint32_t rank) {
     uint32_t r;
