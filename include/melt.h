@@ -187,6 +187,14 @@ int melt_selftest_umma(int kind, int n, int k, const float *a, const float *b, f
  */
 int melt_selftest_umma2(int kind, int n, int k, const float *a, const float *b, float *d);
 
+/*
+ * Test aid: fills the shared memory of every SM of the current device with NaN bit patterns (one resident block per SM
+ * with the largest opt-in dynamic allocation), on `stream` (a cudaStream_t; NULL = default stream), asynchronously.
+ * The forward kernels must not depend on what earlier kernels left in shared memory (staging
+ * ring); tests call this before a forward.  Returns a melt_status.
+ */
+int melt_selftest_poison_smem(void *stream);
+
 #ifdef __cplusplus
 }
 #endif

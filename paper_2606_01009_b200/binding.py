@@ -23,7 +23,7 @@ MELT_OUTPUT_LOG, MELT_OUTPUT_POWER = 0, 1
 SYMBOLS = [
     "melt_plan_create", "melt_plan_destroy", "melt_plan_set_option", "melt_num_frames", "melt_num_channels",
     "melt_plan_get_centres", "melt_forward", "melt_forward_host", "melt_forward_ragged", "melt_forward_tap", "melt_last_error",
-    "melt_plan_describe", "melt_selftest_umma", "melt_selftest_umma2",
+    "melt_plan_describe", "melt_selftest_umma", "melt_selftest_umma2", "melt_selftest_poison_smem",
 ]
 
 _lib = None
@@ -67,6 +67,7 @@ def lib():
     L.melt_plan_describe.argtypes = [vp]
     L.melt_selftest_umma.argtypes = [ip, ip, ip, vp, vp, vp]
     L.melt_selftest_umma2.argtypes = [ip, ip, ip, vp, vp, vp]
+    L.melt_selftest_poison_smem.argtypes = [vp]
     _lib = L
     return L
 
@@ -167,3 +168,8 @@ def melt_selftest_umma2(kind, a, b):
     d = np.empty((256, n), np.float32)
     _check(lib().melt_selftest_umma2(int(kind), n, k, a.ctypes.data, b.ctypes.data, d.ctypes.data))
     return d
+
+
+def melt_selftest_poison_smem(stream=0):
+    """Fill every SM's shared memory with NaN bit patterns (test aid: forwards must not depend on stale shared memory)."""
+    _check(lib().melt_selftest_poison_smem(stream or None))

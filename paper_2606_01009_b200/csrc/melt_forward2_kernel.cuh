@@ -325,11 +325,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         tmem_alloc2(smem_u32(tmem_ptr_s), 512);
         tmem_relinquish2();
     }
-    {   // staging ring (and its guard bands) starts finite: stale rows are multiplied by zero basis entries or belong to
-        // frames that are never stored, but must never be NaN / Inf bit patterns
-        float4 *z = reinterpret_cast<float4 *>(smem + p.off_stg - 128);
-        const int n16 = (S * p.slot_bytes + 256) / 16;
-        for (int i = tid; i < n16; i += V2_THREADS) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    {   // What a frame of zero-weighted (padded) folded pairs may read must be finite, never a stale NaN / Inf bit pattern: up to
+        // 128 bytes before its chunk's slot and after it (the load table is checked against that).  A full-chunk box writes
+        // its whole slot, the clipped form below clears its slot first; what is left to clear at start-up is the 128 bytes
+        // on either side of every slot boundary, plus the slot tails (< 128 bytes) no copy writes.  (Clearing the whole ring
+        // cost ~1300 cycles per launch, shared-memory store bandwidth.)
+        const int s = tid / 24, j = tid - s * 24;
+        if (s <= S && (s > 0 || j >= 8))
+            *reinterpret_cast<float4 *>(smem + p.off_stg + (size_t)s * p.slot_bytes - 256 + 16 * j) = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     if (p.n_mfcc > 0)
         for (int i = tid; i < p.n_mels * p.dct_pitch; i += V2_THREADS) dct_s[i] = __ldg(p.dct + i);
@@ -418,6 +421,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     TRACE(12);
                     if (++slot == S) { slot = 0; ph ^= 1u; }
                     continue;
+                }
+                if (!by_tma && n_rows > 0) {
+                    // the clipped form writes only the samples the clip has: the rest of the slot is cleared first (see set-up)
+                    float4 *z = reinterpret_cast<float4 *>(smem + p.off_stg + (size_t)slot * p.slot_bytes);
+                    for (int i = lane; i < p.slot_bytes / 16; i += 32) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    fence_proxy_async_smem();   // generic-proxy stores before the bulk copies (async proxy) into the same slot
+                    __syncwarp();
                 }
                 if (elect_one()) {
                     const uint32_t full = BAR(V_STG_FULL + slot);

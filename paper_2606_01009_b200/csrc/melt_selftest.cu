@@ -271,3 +271,23 @@ extern "C" int melt_selftest_umma2(int kind, int n, int k, const float *a, const
     cudaFree(dimg);
     return MELT_OK;
 }
+
+// ---------------------------------------------------------------------------------------------- shared-memory poison
+__global__ void __launch_bounds__(256, 1) poison_smem_kernel(int n16) {
+    extern __shared__ __align__(16) unsigned char ps[];
+    uint4 *z = reinterpret_cast<uint4 *>(ps);
+    for (int i = threadIdx.x; i < n16; i += 256) z[i] = make_uint4(0x7fc00000u, 0xffc00000u, 0x7f800001u, 0x7fc00000u);
+}
+
+extern "C" int melt_selftest_poison_smem(void *stream) {
+    int dev = 0, sms = 0, smem = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
+        return melt::fail(MELT_ERR_CUDA, "melt_selftest_poison_smem: device query failed");
+    if (cudaFuncSetAttribute(poison_smem_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess)
+        return melt::fail(MELT_ERR_CUDA, "melt_selftest_poison_smem: cannot opt in to %d bytes of shared memory", smem);
+    poison_smem_kernel<<<4 * sms, 256, smem, (cudaStream_t)stream>>>(smem / 16);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return melt::fail(MELT_ERR_CUDA, "melt_selftest_poison_smem: %s", cudaGetErrorString(e));
+    return MELT_OK;
+}

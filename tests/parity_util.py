@@ -42,6 +42,7 @@ def gpu_dense(c, x_host, precision="compensated", layout=None, pad=None, drop_la
         shape = (B, C, T) if lay == "feature_major" else (B, T, C)
         out = torch.full(shape, float("nan"), device="cuda")
         stream = torch.cuda.current_stream().cuda_stream
+        mb.melt_selftest_poison_smem(stream)   # the forward must not depend on what is left in shared memory
         if tap:
             tshape = (B, M, T) if lay == "feature_major" else (B, T, M)
             lm = torch.full(tshape, float("nan"), device="cuda")
@@ -77,6 +78,7 @@ def gpu_ragged(c, x_host, offsets, precision="compensated", tap=False):
         out = torch.full((max(total, 1), C), float("nan"), device="cuda")
         fo = torch.full((n + 1,), -1, dtype=torch.int64, device="cuda")
         stream = torch.cuda.current_stream().cuda_stream
+        mb.melt_selftest_poison_smem(stream)   # the forward must not depend on what is left in shared memory
         lm = None
         if tap:
             lm = torch.full((max(total, 1), M), float("nan"), device="cuda")
