@@ -4,10 +4,6 @@
 
 namespace melt {
 
-#ifdef MELT_TRACE
-__device__ long long *g_melt_trace = nullptr;   // [2 ranks][16 warps][1024] events
-#endif
-
 int launch_forward2_comp(const K2Params &kp, int grid, int sigma, cudaStream_t stream);
 int launch_forward2_tf32(const K2Params &kp, int grid, int sigma, cudaStream_t stream);
 int launch_forward2_bf16(const K2Params &kp, int grid, int sigma, cudaStream_t stream);
@@ -291,9 +287,3 @@ int launch_forward2(const melt_plan *pl, const K2Params &kp, cudaStream_t stream
 }
 
 }  // namespace melt
-
-#ifdef MELT_TRACE
-extern "C" int melt_debug_set_trace(long long *buf) {
-    return (int)cudaMemcpyToSymbol(melt::g_melt_trace, &buf, sizeof(buf));
-}
-#endif

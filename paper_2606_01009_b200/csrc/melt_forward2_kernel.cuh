@@ -96,7 +96,7 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 
 // Optional event trace (development builds only, -DMELT_TRACE): lane 0 of every warp of cluster 0 appends (tag, clock) pairs.
 #ifdef MELT_TRACE
-extern __device__ long long *g_melt_trace;   // [2 ranks][16 warps][1024] events
+static __device__ long long *g_melt_trace = nullptr;   // [2 ranks][16 warps][1024] events; one copy per translation unit (set by melt_debug_set_trace in melt_forward2_comp.cu)
 #define TRACE_PT(i) do { if (g_melt_trace && threadIdx.x == 0) g_melt_trace[2 * 16 * 1024 + 592 + blockIdx.x * 8 + (i)] = clock64(); } while (0)
 #define TRACE_DECL int tr_n = 0; long long *tr_buf = (g_melt_trace && cluster_id_x() == 0 && (threadIdx.x & 31) == 0) ? g_melt_trace + ((size_t)cluster_ctarank() * 16 + (threadIdx.x >> 5)) * 1024 : nullptr;
 #define TRACE(tag) do { if (tr_buf && tr_n < 1023) tr_buf[++tr_n] = ((long long)(tag) << 48) | (clock64() & 0xFFFFFFFFFFFFll); if (tr_buf) tr_buf[0] = tr_n; } while (0)

@@ -10,6 +10,14 @@ P_BAR = {"compensated": 1e-3, "tf32": 1e-3, "bf16": 3e-2}
 LOG_BAR = 5e-3
 MASK_FLOOR = 1e-6
 
+# CUDA result against the CPU emulation of ITS OWN operand scheme (oracle/melt_emul.py: operands rounded exactly as the
+# kernel rounds them, products summed in fp64): what is left is the tensor cores' fp32 accumulation, ~2^-24 of the larger
+# terms of a sum.  Derivation: |dR| <~ 2^-23 sum_j |a_j b_j| <~ 1e-6 R_max, so |dS| / S_max <~ 4e-6 on
+# the loudest bins; a bin at the mask floor (S = 1e-6 S_max, |R| = 1e-3 R_max) then has |dS| / S <~ 2e-3, |dlog10| <~ 1e-3.
+ACC_P_BAR = 1e-5      # max |S_gpu - S_emul| / frame max
+ACC_LOG_BAR = 1.5e-3  # max |L_gpu - log10(max(S_emul, 1e-10))| where S_ref >= 1e-6 frame max
+EMUL_SCHEME = {"compensated": "f16x3", "tf32": "tf32", "bf16": "bf16"}
+
 
 def plan_for(c, precision="compensated", layout=None, pad=None, drop_last=None, output="log", n_mfcc=None):
     """Create a plan for config dict c (workloads.CONFIGS entry or look-alike) with the given options."""
@@ -114,3 +122,19 @@ def log_error(L_gpu, L_ref, P_ref):
     if not mask.any():
         return 0.0
     return float(np.abs(L_gpu - L_ref)[mask].max())
+
+
+def emulated_power(c, x, precision, pad=None, drop_last=None):
+    """S [B, T, M] of the dense batch x under the operand scheme of `precision` in the kernels' folded operand layout, products
+    summed in fp64 on the CPU (oracle/melt_emul.py)."""
+    from oracle import melt_emul as em
+    return em.emulate_power_batch(x, fs=c["fs"], n_fft=c["n_fft"], hop=c["hop"], window_kind=c["window"], n_mels=c["n_mels"],
+                                  fmin=c["fmin"], fmax=c["fmax"], scheme=EMUL_SCHEME[precision], layout="folded",
+                                  pad=int(bool(pad)), drop_last=bool(c.get("drop_last", False) if drop_last is None else drop_last))
+
+
+def single_pass_bars(precision, perr_emul, lerr_emul):
+    """Bars of a CUDA result against the ORACLE for a mode whose operand rounding alone (emulated error perr_emul /
+    lerr_emul against the oracle, exact summation) may exceed the north-star bar: the north-star bar where the arithmetic
+    meets it, otherwise 1.25 x what the arithmetic gives plus the accumulation allowance -- never unbounded."""
+    return max(P_BAR[precision], 1.25 * perr_emul + ACC_P_BAR), max(LOG_BAR, 1.25 * lerr_emul + ACC_LOG_BAR)
