@@ -20,7 +20,13 @@
  *     "host" pointers are ordinary host memory.  The library never takes ownership of caller buffers.
  *   - All forward calls are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = the
  *     legacy default stream).  Caller buffers must stay valid until the stream reaches the call.
- *   - No allocation and no host synchronisation happens inside a forward call.
+ *   - No host synchronisation happens inside a forward call, and the plan is never modified by one (forward calls take a
+ *     const plan; concurrent calls on one plan from several threads / streams are safe).  Dense batches whose clips start on
+ *     16-byte boundaries -- the fast path -- use no memory beyond the caller's buffers.  Three paths need per-call device
+ *     scratch: packed (ragged) batches (4 (n_clips + 1) bytes), dense batches that are not 16-byte aligned (one realigned copy of
+ *     the batch) and melt_forward_host (device copies of x and out).  That scratch is taken from a plan-owned stream-ordered
+ *     pool (cudaMallocFromPoolAsync on `stream`, returned with cudaFreeAsync on `stream` inside the same call): asynchronous,
+ *     and after the first call of a given size it is served from memory the pool already holds (melt_plan_reserve pre-sizes it).
  *   - Errors are detected on the host before any launch and returned as melt_status; the message is
  *     available from melt_last_error() (thread-local).  Kernel-side faults are not reported asynchronously.
  *   - Inputs must be finite; in MELT_PREC_COMPENSATED mode |x| must stay below 8 * 2^(12 - s) where s is
@@ -62,7 +68,16 @@ typedef enum {
     MELT_OPT_PAD = 3,              /* melt_pad; default NONE */
     MELT_OPT_INPUT_SCALE_LOG2 = 4, /* s in [-24, 24]: samples are multiplied by 2^s before the fp16 split of the
                                       COMPENSATED mode (exact; undone in the epilogue); default 12 */
-    MELT_OPT_OUTPUT = 5            /* melt_output; default LOG */
+    MELT_OPT_OUTPUT = 5,           /* melt_output; default LOG */
+    MELT_OPT_INPUT_READY = 6       /* 0/1, default 0.  Consecutive forwards on one stream overlap on the device (programmatic
+                                      dependent launch: the next forward's blocks start on the SMs the previous kernel has
+                                      already vacated).  With 0 a forward waits for the completion of whatever precedes it in
+                                      `stream` before its first read of x (and of offsets) -- correct for any producer, only the
+                                      kernel's set-up and its reads of the plan's own tables overlap.  1 is the caller's promise
+                                      that x / offsets are NOT written by the operation that directly precedes the call in
+                                      `stream` (they were complete earlier: copied by a memcpy, or produced before an earlier
+                                      kernel): the kernel then reads them while its predecessor is still draining and waits
+                                      only before its first store.  bench.py's device-resident timing sets 1 and says so. */
 } melt_option;
 
 typedef enum {
@@ -80,10 +95,9 @@ typedef enum {
 typedef enum {
     MELT_PAD_NONE = 0,   /* T = floor((len - n_fft)/hop) + 1 frames per clip; tail samples ignored */
     MELT_PAD_REFLECT = 1 /* the clip is reflect-padded by n_fft/2 per side (edge sample not repeated);
-                            T = floor(len/hop) + 1 for even n_fft; needs len > n_fft/2.  On the fast path the padded signal is
-                            written once into a plan-owned device copy (allocated at the first such forward call and re-allocated,
-                            after a stream synchronisation, only when a later call needs more room; forwards of one plan that
-                            use it must then be issued on one stream at a time) */
+                            T = floor(len/hop) + 1 for even n_fft; needs len > n_fft/2.  The padding is virtual: the few frames per
+                            clip that reach beyond the clip are staged through an edge path that mirrors the indices, every other
+                            frame takes the same bulk-copy path as an unpadded clip -- no padded copy of the signal is made */
 } melt_pad;
 
 typedef enum {
@@ -116,6 +130,15 @@ int melt_plan_set_option(melt_plan *plan, int key, int value);
 /* Frames per clip for a clip of `len` samples under the plan's pad / drop_last options (0 if too short). */
 long long melt_num_frames(const melt_plan *plan, long long len);
 
+/* The same count from the framing parameters alone (no plan, no GPU): T = floor((len + 2 p - n_fft) / hop) + 1 - drop_last with
+ * p = n_fft/2 for MELT_PAD_REFLECT (which also needs len > n_fft/2) and 0 otherwise; 0 when the clip is too short.  Host-only
+ * integer arithmetic, for callers that size buffers or shard batches before a plan exists. */
+long long melt_count_frames(long long len, int n_fft, int hop, int pad, int drop_last);
+
+/* Pre-sizes the plan's scratch pool so that later forward calls needing up to `bytes` of per-call scratch (see "Conventions")
+ * are served without growing it.  Synchronous; optional.  Returns a melt_status. */
+int melt_plan_reserve(melt_plan *plan, unsigned long long bytes);
+
 /* Output channels per frame: n_mfcc if n_mfcc > 0 else n_mels. */
 int melt_num_channels(const melt_plan *plan);
 
@@ -125,22 +148,23 @@ int melt_plan_get_centres(const melt_plan *plan, double *f_hz);
 /*
  * melt_forward -- the whole hot path on a dense batch.
  *   x    device, fp32, [batch, len] contiguous, 4-byte aligned.  When every clip start is 16-byte aligned (x and len*4)
- *        the kernel frames x in place; otherwise one pass first copies the batch into a plan-owned buffer at an aligned
- *        clip stride (allocated at the first such call, see MELT_PAD_REFLECT);
+ *        the kernel frames x in place; otherwise one pass first copies the batch into pool scratch at an aligned clip
+ *        stride (see "Conventions");
  *   out  device, fp32, batch * C * T floats, T = melt_num_frames(plan, len), layout per MELT_OPT_LAYOUT.
  * batch == 0 or T == 0 is a successful no-op.  Returns a melt_status.
  */
 int melt_forward(const melt_plan *plan, const float *x, int batch, long long len, float *out, void *stream);
 
 /*
- * melt_forward_host -- melt_forward on HOST buffers: copies x_host [batch, len] to a plan-owned device workspace, runs the
- * hot path and copies the result to out_host (batch * C * T floats, layout per MELT_OPT_LAYOUT), all asynchronously on
- * `stream`.  The call returns without waiting: synchronise the stream before reading out_host or reusing x_host.  Pinned
- * (page-locked) host buffers are needed for the copies to be asynchronous.  The workspace is allocated on the first call and
- * re-allocated (after a stream synchronisation) only when a later call needs more room; because it belongs to the plan,
- * calls of melt_forward_host on one plan must be issued on one stream at a time.
+ * melt_forward_host -- melt_forward on HOST buffers: x_host [batch, len] in, out_host (batch * C * T floats, layout per
+ * MELT_OPT_LAYOUT) out.  The batch is cut into groups of clips and pipelined: the host-to-device copy of group k + 1, the
+ * kernel of group k and the device-to-host copy of group k - 1 run at the same time (two plan-owned copy streams, ordered
+ * against `stream` by events), so the call costs about max(upload, download) instead of their sum.  Everything is ordered
+ * after the work already in `stream`, and `stream` waits for the last download: synchronise `stream` before reading out_host
+ * or reusing x_host.  The call itself returns without waiting.  Pinned (page-locked) host buffers are needed for the copies
+ * to be asynchronous.  Device copies of x and out come from the plan's scratch pool (see "Conventions").
  */
-int melt_forward_host(melt_plan *plan, const float *x_host, int batch, long long len, float *out_host, void *stream);
+int melt_forward_host(const melt_plan *plan, const float *x_host, int batch, long long len, float *out_host, void *stream);
 
 /*
  * melt_forward_ragged -- the whole hot path on clips packed back to back (configs[3]).
@@ -169,31 +193,6 @@ const char *melt_last_error(void);
 
 /* Library / kernel configuration as a short human-readable string for logs (static storage per plan). */
 const char *melt_plan_describe(const melt_plan *plan);
-
-/*
- * Self-test of the tensor-core building block used by the forward kernels: D[128, n] = A[128, k] . B[n, k]^T
- * with A written to tensor memory by threads and B read from shared memory (tcgen05.mma, A-from-TMEM form).
- *   kind: 0 = fp16, 1 = bf16, 2 = tf32;  a, b host fp32 row-major (values are rounded to `kind` inside);
- *   d host fp32 [128, n] result.  n % 16 == 0, 16 <= n <= 256; k % 16 == 0 (fp16/bf16) or k % 8 == 0 (tf32), k <= 256.
- * Synchronous.  Returns a melt_status.
- */
-int melt_selftest_umma(int kind, int n, int k, const float *a, const float *b, float *d);
-
-/*
- * Self-test of the CTA-pair form of the same building block (tcgen05.mma.cta_group::2 on a cluster of two CTAs):
- * D[256, n] = A[256, k] . B[n, k]^T, CTA r of the pair holding rows [128 r, 128 r + 128) of A in its tensor memory
- * and rows [r n/2, (r+1) n/2) of B in its shared memory.  a host fp32 [256, k]; b host fp32 [n, k]; d host fp32
- * [256, n].  n % 16 == 0, 32 <= n <= 256; k as for melt_selftest_umma.  Synchronous.  Returns a melt_status.
- */
-int melt_selftest_umma2(int kind, int n, int k, const float *a, const float *b, float *d);
-
-/*
- * Test aid: fills the shared memory of every SM of the current device with NaN bit patterns (one resident block per SM
- * with the largest opt-in dynamic allocation), on `stream` (a cudaStream_t; NULL = default stream), asynchronously.
- * The forward kernels must not depend on what earlier kernels left in shared memory (staging
- * ring); tests call this before a forward.  Returns a melt_status.
- */
-int melt_selftest_poison_smem(void *stream);
 
 #ifdef __cplusplus
 }

@@ -13,18 +13,21 @@ from . import build as _build
 MELT_OK, MELT_ERR_INVALID_ARG, MELT_ERR_UNSUPPORTED, MELT_ERR_ALIGNMENT, MELT_ERR_CUDA, MELT_ERR_ALLOC = range(6)
 MELT_WINDOW_HANN_PERIODIC, MELT_WINDOW_HANN_SYMMETRIC, MELT_WINDOW_RECT = 0, 1, 2
 MELT_MEL_HTK, MELT_MEL_SLANEY = 0, 1
-MELT_OPT_LAYOUT, MELT_OPT_PRECISION, MELT_OPT_DROP_LAST, MELT_OPT_PAD, MELT_OPT_INPUT_SCALE_LOG2, MELT_OPT_OUTPUT = range(6)
+MELT_OPT_LAYOUT, MELT_OPT_PRECISION, MELT_OPT_DROP_LAST, MELT_OPT_PAD, MELT_OPT_INPUT_SCALE_LOG2, MELT_OPT_OUTPUT, \
+    MELT_OPT_INPUT_READY = range(7)
 MELT_LAYOUT_FRAME_MAJOR, MELT_LAYOUT_FEATURE_MAJOR = 0, 1
 MELT_PREC_COMPENSATED, MELT_PREC_TF32, MELT_PREC_BF16 = 0, 1, 2
 MELT_PAD_NONE, MELT_PAD_REFLECT = 0, 1
 MELT_OUTPUT_LOG, MELT_OUTPUT_POWER = 0, 1
 
-# every symbol include/melt.h declares (tests/test_abi.py checks the header against this list and the .so)
+# every symbol include/melt.h declares (tests/test_abi.py checks the header against this list and the .so) ...
 SYMBOLS = [
-    "melt_plan_create", "melt_plan_destroy", "melt_plan_set_option", "melt_num_frames", "melt_num_channels",
-    "melt_plan_get_centres", "melt_forward", "melt_forward_host", "melt_forward_ragged", "melt_forward_tap", "melt_last_error",
-    "melt_plan_describe", "melt_selftest_umma", "melt_selftest_umma2", "melt_selftest_poison_smem",
+    "melt_plan_create", "melt_plan_destroy", "melt_plan_set_option", "melt_num_frames", "melt_count_frames", "melt_num_channels",
+    "melt_plan_reserve", "melt_plan_get_centres", "melt_forward", "melt_forward_host", "melt_forward_ragged", "melt_forward_tap",
+    "melt_last_error", "melt_plan_describe",
 ]
+# ... and the test aids of include/melt_test.h (not part of the product API)
+TEST_SYMBOLS = ["melt_selftest_umma", "melt_selftest_umma2", "melt_selftest_poison_smem"]
 
 _lib = None
 
@@ -56,6 +59,9 @@ def lib():
     L.melt_plan_set_option.argtypes = [vp, ip, ip]
     L.melt_num_frames.restype = ll
     L.melt_num_frames.argtypes = [vp, ll]
+    L.melt_count_frames.restype = ll
+    L.melt_count_frames.argtypes = [ll, ip, ip, ip, ip]
+    L.melt_plan_reserve.argtypes = [vp, C.c_ulonglong]
     L.melt_num_channels.argtypes = [vp]
     L.melt_plan_get_centres.argtypes = [vp, C.POINTER(dbl)]
     L.melt_forward.argtypes = [vp, vp, ip, ll, vp, vp]
@@ -107,6 +113,15 @@ def melt_plan_set_option(plan, key, value):
 
 def melt_num_frames(plan, length):
     return int(lib().melt_num_frames(plan, int(length)))
+
+
+def melt_count_frames(length, n_fft, hop, pad=MELT_PAD_NONE, drop_last=False):
+    """Frames of a clip from the framing parameters alone (host-only integer arithmetic inside the library; no plan, no GPU)."""
+    return int(lib().melt_count_frames(int(length), int(n_fft), int(hop), int(pad), int(bool(drop_last))))
+
+
+def melt_plan_reserve(plan, nbytes):
+    _check(lib().melt_plan_reserve(plan, int(nbytes)))
 
 
 def melt_num_channels(plan):

@@ -469,19 +469,21 @@ __global__ void __launch_bounds__(1024, 1) ragged_scan_kernel(const KParams p, c
     if (tid == 0) { frame_offsets[n_clips] = carry_f; tile_prefix[n_clips] = carry_t; }
 }
 
-int launch_ragged_scan(const melt_plan *pl, const long long *offsets, int n_clips, long long *frame_offsets, int tile_m, cudaStream_t stream) {
-    ragged_scan_kernel<<<1, 1024, 0, stream>>>(pl->kp, offsets, n_clips, frame_offsets, pl->d_tile_prefix, tile_m);
+int launch_ragged_scan(const melt_plan *pl, const long long *offsets, int n_clips, long long *frame_offsets, int *tile_prefix, int tile_m, cudaStream_t stream) {
+    ragged_scan_kernel<<<1, 1024, 0, stream>>>(pl->kp, offsets, n_clips, frame_offsets, tile_prefix, tile_m);
     MELT_CUDA(cudaGetLastError());
     return MELT_OK;
 }
 
 int launch_forward(const melt_plan *pl, const KParams &kp, cudaStream_t stream) {
-    static bool attr_done = false;
-    if (!attr_done) {
+    // the opt-in shared-memory size is a per-device attribute of the function: set once per device (bit d of the mask)
+    static std::atomic<unsigned long long> attr_done{0};
+    const unsigned long long bit = 1ull << (pl->device & 63);
+    if (pl->device >= 64 || !(attr_done.load(std::memory_order_acquire) & bit)) {
         MELT_CUDA(cudaFuncSetAttribute(melt_fwd_kernel<PREC_COMP>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
         MELT_CUDA(cudaFuncSetAttribute(melt_fwd_kernel<PREC_TF32>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
         MELT_CUDA(cudaFuncSetAttribute(melt_fwd_kernel<PREC_BF16>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
-        attr_done = true;
+        attr_done.fetch_or(bit, std::memory_order_release);
     }
     int grid = pl->sm_count;
     if (kp.n_tiles >= 0 && kp.n_tiles < grid) grid = kp.n_tiles;

@@ -77,6 +77,7 @@ int plan_build_v2(melt_plan *p) {
             break;
         }
     }
+    k.stg_phases = std::max(1, (k.stg_slots + 3) / 4);
     k.off_dct = (uint32_t)round_up2((int)(k.off_stg + (uint32_t)k.stg_slots * k.slot_bytes + 128), 128);
     k.off_epi = epi_bytes ? k.off_dct + dct_only : 0;
     k.off_bar = (uint32_t)round_up2((int)(k.off_dct + dct_bytes), 128);
@@ -142,14 +143,8 @@ int plan_build_v2(melt_plan *p) {
             }
     cudaFree(p->d_bimg2);
     p->d_bimg2 = nullptr;
-    {   // replicas of the image spread the clusters' simultaneous first fetch over more L2 lines (tuning knob; default 1)
-        const char *e = getenv("MELT_BASIS_REPLICAS");
-        const int want = e ? atoi(e) : 1;
-        k.b_replicas = (int)std::max<size_t>(1, std::min<size_t>((size_t)std::max(want, 1), ((size_t)8 << 20) / img_bytes));
-    }
-    MELT_CUDA(cudaMalloc(&p->d_bimg2, img_bytes * k.b_replicas));
-    for (int r = 0; r < k.b_replicas; ++r)
-        MELT_CUDA(cudaMemcpy(p->d_bimg2 + (size_t)r * img_bytes, img.data(), img_bytes, cudaMemcpyHostToDevice));
+    MELT_CUDA(cudaMalloc(&p->d_bimg2, img_bytes));
+    MELT_CUDA(cudaMemcpy(p->d_bimg2, img.data(), img_bytes, cudaMemcpyHostToDevice));
     k.b_img = p->d_bimg2;
     k.dct = p->d_dct;
     p->v2_ok = true;
@@ -182,16 +177,17 @@ static EncodeTiledFn encode_tiled_fn() {
 int v2_encode_tmap(K2Params &k) {
     k.tma_rows = 0;
     if (k.direct) return MELT_OK;   // no staging, no tensor map
-    static const bool disabled = getenv("MELT_DISABLE_TMA") != nullptr;   // debug switch: per-row bulk copies everywhere
-    if (disabled) return MELT_OK;
     EncodeTiledFn enc = encode_tiled_fn();
     const long long W = k.pitch_bytes / 4;
-    if (!enc || W > 256 || k.rows_per_chunk > 256 || k.len < W) return MELT_OK;
-    const long long rows = (k.len - W) / k.hop + 1;   // rows whose W-wide extent stays inside a clip (hence inside the buffer)
+    // virtual reflect padding: a chunk starts at any multiple of 4 samples of the clip, i.e. at column (start % hop) of hop-row
+    // (start / hop): the rows are declared hop + W samples wide for that (as in the ragged map below)
+    const long long Wd = W + (k.vpad > 0 ? k.hop : 0);
+    if (!enc || W > 256 || k.rows_per_chunk > 256 || k.len < Wd) return MELT_OK;
+    const long long rows = (k.len - Wd) / k.hop + 1;   // rows whose whole declared extent stays inside a clip (hence inside the buffer)
     if (rows < k.rows_per_chunk || rows > 0x7fffffffLL) return MELT_OK;
     static_assert(sizeof(CUtensorMap) == 128, "CUtensorMap size");
     CUtensorMap tm;
-    const cuuint64_t gdim[3] = {(cuuint64_t)W, (cuuint64_t)rows, (cuuint64_t)k.n_clips};
+    const cuuint64_t gdim[3] = {(cuuint64_t)Wd, (cuuint64_t)rows, (cuuint64_t)k.n_clips};
     const cuuint64_t gstr[2] = {(cuuint64_t)k.hop * 4u, (cuuint64_t)k.len * 4u};   // overlapping rows: stride (hop) < extent (pitch)
     const cuuint32_t box[3] = {(cuuint32_t)W, (cuuint32_t)k.rows_per_chunk, 1u};
     const cuuint32_t estr[3] = {1u, 1u, 1u};

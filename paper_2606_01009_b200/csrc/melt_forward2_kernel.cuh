@@ -29,6 +29,7 @@
 #include <cuda_fp16.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cstdlib>
 
 namespace melt {
@@ -97,10 +98,12 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 // Optional event trace (development builds only, -DMELT_TRACE): lane 0 of every warp of cluster 0 appends (tag, clock) pairs.
 #ifdef MELT_TRACE
 static __device__ long long *g_melt_trace = nullptr;   // [2 ranks][16 warps][1024] events; one copy per translation unit (set by melt_debug_set_trace in melt_forward2_comp.cu)
-#define TRACE_PT(i) do { if (g_melt_trace && threadIdx.x == 0) g_melt_trace[2 * 16 * 1024 + 592 + blockIdx.x * 8 + (i)] = clock64(); } while (0)
-#define TRACE_DECL int tr_n = 0; long long *tr_buf = (g_melt_trace && cluster_id_x() == 0 && (threadIdx.x & 31) == 0) ? g_melt_trace + ((size_t)cluster_ctarank() * 16 + (threadIdx.x >> 5)) * 1024 : nullptr;
+#define TRACE_WORDS (2 * 16 * 1024 + 592 + 148 * 8 + 64)   // one region per traced launch (K2Params::trace_slot)
+#define TRACE_BASE (g_melt_trace + (size_t)p.trace_slot * TRACE_WORDS)
+#define TRACE_PT(i) do { if (g_melt_trace && threadIdx.x == 0) TRACE_BASE[2 * 16 * 1024 + 592 + blockIdx.x * 8 + (i)] = clock64(); } while (0)
+#define TRACE_DECL int tr_n = 0; long long *tr_buf = (g_melt_trace && cluster_id_x() == 0 && (threadIdx.x & 31) == 0) ? TRACE_BASE + ((size_t)cluster_ctarank() * 16 + (threadIdx.x >> 5)) * 1024 : nullptr;
 #define TRACE(tag) do { if (tr_buf && tr_n < 1023) tr_buf[++tr_n] = ((long long)(tag) << 48) | (clock64() & 0xFFFFFFFFFFFFll); if (tr_buf) tr_buf[0] = tr_n; } while (0)
-#define TRACE_CTA(which) do { if (g_melt_trace && threadIdx.x == 0) { g_melt_trace[2 * 16 * 1024 + blockIdx.x * 2 + (which)] = (long long)globaltimer_ns(); g_melt_trace[2 * 16 * 1024 + 296 + blockIdx.x * 2 + (which)] = clock64(); } } while (0)
+#define TRACE_CTA(which) do { if (g_melt_trace && threadIdx.x == 0) { TRACE_BASE[2 * 16 * 1024 + blockIdx.x * 2 + (which)] = (long long)globaltimer_ns(); TRACE_BASE[2 * 16 * 1024 + 296 + blockIdx.x * 2 + (which)] = clock64(); } } while (0)
 #else
 #define TRACE_CTA(which) do { } while (0)
 #define TRACE_PT(i) do { } while (0)
@@ -292,66 +295,79 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     const int S = p.stg_slots;
 
     // ------------------------------------------------------------------ one-time setup
-    if (!RAGGED && !DIRECT && tid == 32 && p.tma_rows > 0 && p.passes == 1) {
-        // First thing, before any set-up: pull this CTA's first two tiles into L2.  The staging copies are issued ~1000
-        // cycles from now (after barrier / tensor-memory set-up) and one after the other; with the DRAM accesses of all
-        // chunks started here, in parallel, they cost L2 hits -- the first MMA starts ~1.5 us earlier.
-        const int cid = (int)cluster_id_x(), cstep = (int)cluster_nid_x();
-        for (int k = 0; k < 2; ++k) {
-            const int tile = cid + k * cstep;
-            if (tile >= p.n_tiles) break;
-            const int b = tile / p.tiles_per_clip;
-            const int t0 = (tile - b * p.tiles_per_clip) * 256 + (int)cluster_ctarank() * 128;
-            for (int q = 0; q < 4; ++q) {
-                const long long row0 = (long long)(t0 + 32 * q);
-                if (row0 < p.frames_per_clip && row0 + p.rows_per_chunk <= (long long)p.tma_rows) tma_prefetch_l2_3d(p.tmap, 0, (int)row0, b);
-            }
-        }
-    }
-    // every barrier of the block is set up by a thread of its own (one thread doing all of them costs ~2000 cycles per launch)
-    if (tid < V_NBARS) {
-        const int i = tid;
-        const uint32_t count = i < V_STG_EMPTY ? 1u : i < V_A_FULL ? (uint32_t)NG : i < V_A_EMPTY ? 8u
-                             : i < V_ACC_EMPTY ? 2u                                    // A_EMPTY, ACC_FULL: both issuers commit
-                             : i < V_B_FULL ? (uint32_t)(SHARE ? 8 * DRAINERS : 8)     // ACC_EMPTY
-                             : i < V_DONE ? 1u                                         // B_FULL, B_PEER
-                             : i == V_DONE ? 2u                                        // both MMA issuers
-                             : i < V_B_EMPTY ? 1u : 2u;                                // STG_READY; B_EMPTY: both issuers release a slab
-        mbar_init(BAR(i), count);
-        fence_barrier_init();
-    }
-    TRACE_PT(1);
+    // Who does what, so that nothing waits for anything it does not need (set-up used to cost ~3000 cycles per launch, now the
+    // ~1000 of the tensor-memory allocation): the basis warp allocates tensor memory first thing; warps 4.. clear the margins of
+    // the staging ring; the loader warp sets up the staging barriers itself and -- after a named barrier with the clearing warps
+    // only -- goes straight to its loop, so the first tile's chunks are in flight while the rest of the block is still setting
+    // up; the two issuer warps set up all other barriers.  The loader joins the cluster barrier by arriving early and waiting
+    // at its very end (it needs nothing the barrier publishes).
+    constexpr bool EARLY_LOADER = !DIRECT;                       // direct-load form: the loader warp has no work
+    constexpr int SETUP_THREADS = EARLY_LOADER ? V2_THREADS - 32 : V2_THREADS;
     if (warp == W_BASIS) {
         tmem_alloc2(smem_u32(tmem_ptr_s), 512);
         tmem_relinquish2();
     }
-    {   // What a frame of zero-weighted (padded) folded pairs may read must be finite, never a stale NaN / Inf bit pattern: up to
+    if (tid >= 128) {
+        // What a frame of zero-weighted (padded) folded pairs may read must be finite, never a stale NaN / Inf bit pattern: up to
         // 128 bytes before its chunk's slot and after it (the load table is checked against that).  A full-chunk box writes
         // its whole slot, the clipped form below clears its slot first; what is left to clear at start-up is the 128 bytes
         // on either side of every slot boundary, plus the slot tails (< 128 bytes) no copy writes.  (Clearing the whole ring
         // cost ~1300 cycles per launch, shared-memory store bandwidth.)
-        const int s = tid / 24, j = tid - s * 24;
+        const int s = (tid - 128) / 24, j = (tid - 128) - s * 24;
         if (s <= S && (s > 0 || j >= 8))
             *reinterpret_cast<float4 *>(smem + p.off_stg + (size_t)s * p.slot_bytes - 256 + 16 * j) = make_float4(0.f, 0.f, 0.f, 0.f);
+        fence_proxy_async_smem();  // the zero fill (generic proxy) is ordered before the bulk copies (async proxy) that follow
+    }
+    static_assert(13 * 24 <= V2_THREADS - 128, "one thread per 16 bytes of margin");
+    if (warp == W_LOAD) {
+        // staging barriers: FULL (one arrival + transaction bytes), EMPTY (one arrival per converter group), READY (ragged)
+        if (lane < V2_MAX_STG) {
+            mbar_init(BAR(V_STG_FULL + lane), 1u);
+            mbar_init(BAR(V_STG_EMPTY + lane), (uint32_t)NG);
+            mbar_init(BAR(V_STG_READY + lane), 1u);
+        }
+        fence_barrier_init();
+    } else if (warp == W_MMA || warp == W_MMA2) {
+        const int n_b = STREAM ? 8 : (p.units < V2_MAX_UNITS ? p.units : V2_MAX_UNITS);   // basis barriers in use
+        const int t64 = (warp == W_MMA ? 0 : 32) + lane;
+        for (int i = t64; i < 16; i += 64) { mbar_init(BAR(V_A_FULL + i), 8u); mbar_init(BAR(V_A_EMPTY + i), 2u); }   // A_EMPTY: both issuers commit
+        if (t64 < 2) { mbar_init(BAR(V_ACC_FULL + t64), 2u); mbar_init(BAR(V_ACC_EMPTY + t64), (uint32_t)(SHARE ? 8 * DRAINERS : 8)); }
+        for (int i = t64; i < n_b; i += 64) { mbar_init(BAR(V_B_FULL + i), 1u); mbar_init(BAR(V_B_PEER + i), 1u); }
+        if (t64 < 8) mbar_init(BAR(V_B_EMPTY + t64), 2u);                                // both issuers release a slab
+        if (t64 == 8) mbar_init(BAR(V_DONE), 2u);                                        // both MMA issuers
+        fence_barrier_init();
     }
     if (p.n_mfcc > 0)
         for (int i = tid; i < p.n_mels * p.dct_pitch; i += V2_THREADS) dct_s[i] = __ldg(p.dct + i);
-    TRACE_PT(2);
-    fence_proxy_async_smem();  // the zero fill (generic proxy) is ordered before the bulk copies (async proxy) that follow
-    tc_fence_before();
-    __syncthreads();
-    TRACE_PT(3);
+    TRACE_PT(1);
+    uint32_t tmem_base = 0;
+    if (EARLY_LOADER && warp == W_LOAD) {
+        // the loader: margins cleared (named barrier with the clearing warps), its own barriers set up -> start copying
+        asm volatile("bar.sync 1, %0;" ::"n"(V2_THREADS - 96) : "memory");
+        cluster_arrive_relaxed();
+    } else {
+        if (EARLY_LOADER && tid >= 128) asm volatile("bar.arrive 1, %0;" ::"n"(V2_THREADS - 96) : "memory");
+        TRACE_PT(2);
+        tc_fence_before();
+        asm volatile("bar.sync 2, %0;" ::"n"(SETUP_THREADS) : "memory");   // tensor memory allocated, barriers set up (this CTA)
+        TRACE_PT(3);
 #ifdef MELT_STRICT_CLUSTER_SYNC
-    cluster_sync_all();
+        cluster_sync_all();
 #else
-    cluster_arrive_relaxed();   // barrier set-up is published by fence.mbarrier_init; everything else set up here is CTA-local
-    cluster_wait();
+        cluster_arrive_relaxed();   // barrier set-up is published by fence.mbarrier_init; everything else set up here is CTA-local
+        cluster_wait();
 #endif
-    TRACE_PT(4);
-    tc_fence_after();
-    const uint32_t tmem_base = *tmem_ptr_s;
-    if (tid == 0) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the next forward may start filling freed SMs
+        TRACE_PT(4);
+        tc_fence_after();
+        tmem_base = *tmem_ptr_s;
+    }
+    if (tid == 32) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the next forward may start filling freed SMs
 
+    // Programmatic dependent launch: this grid may have started while the previous kernel of the stream is still running.
+    // Everything above touched only this block's shared / tensor memory and the plan's own tables.  Unless the caller vouches
+    // for the input (MELT_OPT_INPUT_READY), wait here -- before the first read of x / offsets -- for the predecessor to complete
+    // and its writes to be visible; otherwise the wait is taken just before the first global store (dep_done below).
+    if (!p.input_ready) asm volatile("griddepcontrol.wait;" ::: "memory");
     const int first_tile = (int)cluster_id_x(), tile_step = (int)cluster_nid_x();
     const int n_tiles = (RAGGED ? p.tile_prefix[p.n_clips] : p.n_tiles) * p.passes;   // ragged: counted by the scan kernel; one visit per pass over the bins
     TRACE_DECL
@@ -361,8 +377,20 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     } else if (warp == W_LOAD) {
         // ============================================================== signal loader (bulk-copy engine)
         // The whole warp runs the (uniform) loop; one elected lane issues the copies.
-        int slot = 0;
-        uint32_t ph = 0;
+        // The chunk of lane quarter q of this CTA's tl-th tile lands in memory slot (4 tl + q) mod S, but its barriers are
+        // FULL / EMPTY / READY [q + 4 (tl mod P)], P = ceil(S / 4): every waiter then waits for EVERY phase of the barriers it
+        // uses (a converter warp of quarter q waits on [q + 4 (tl mod P)] at every tile; this loader waits, in chunk order, for
+        // the release of chunk c - S before it overwrites that chunk's slot with chunk c).  Indexing the barriers by memory slot
+        // would let a warp meet a barrier whose previous phase belongs to another quarter's chunk and which it never
+        // waited for: if that phase has not completed yet, a parity wait for the following phase succeeds at once (found with
+        // single-pass modes whose operand ring holds a whole tile: a quarter without valid frames ran a tile ahead and read
+        // a slot that still held, or was still receiving, the previous chunk).
+        int slot = 0, cq = 0, ctp = 0;        // memory slot, lane quarter and tile phase of the next chunk
+        uint32_t cph = 0;
+        int eq = 0, etp = 0;                  // the same for chunk c - S (whose release frees the slot), valid once c >= S
+        uint32_t eph = 0;
+        int chunk_count = 0;
+        const int P = p.stg_phases;
         const long long len = p.len;
         if (p.tma_rows > 0 && lane == 0) tma_prefetch_desc(p.tmap);
         constexpr bool ragged = RAGGED;
@@ -386,24 +414,79 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 // The tensor-map engine wants the box to start on a 16-byte boundary: it is fetched from the aligned sample below
                 // (clip starts are arbitrary; hop % 4 == 0, so every chunk of a clip has the same misalignment) and the
                 // converter warp that owns the chunk shifts it down by (s0 & 3) words in shared memory.
+                // Virtual reflect padding (MELT_PAD_REFLECT): frame t of a clip starts vpad samples before sample t * hop, so the
+                // chunk's first row starts at clip-relative sample st (negative at the head of a clip).  The box is addressed by its
+                // start sample: column st % hop of hop-row st / hop (both maps are hop + pitch samples wide for that).
+                const long long st = row0 * p.hop - p.vpad;
                 long long s = 0;
                 int c0 = 0, c1 = (int)row0, c2 = b;
                 bool by_tma;
                 if (!ragged) {
-                    by_tma = n_rows > 0 && row0 + n_rows <= (long long)p.tma_rows;
+                    if (p.vpad == 0) {
+                        by_tma = n_rows > 0 && row0 + n_rows <= (long long)p.tma_rows;
+                    } else {
+                        const long long r = st >= 0 ? st / p.hop : 0;
+                        c0 = (int)(st - r * p.hop); c1 = (int)r;
+                        by_tma = n_rows > 0 && st >= 0 && r + n_rows <= (long long)p.tma_rows;   // every row of the box inside the clip
+                    }
                 } else {
-                    s = (ti.s0 & ~3ll) + row0 * p.hop;
-                    const long long r = s / p.hop;
+                    s = (ti.s0 & ~3ll) + st;
+                    const long long r = s >= 0 ? s / p.hop : 0;
                     c0 = (int)(s - r * p.hop); c1 = (int)r; c2 = 0;
-                    by_tma = n_rows > 0 && s + (long long)(p.rows_per_chunk - 1) * p.hop + (p.pitch_bytes >> 2) <= total;
+                    by_tma = n_rows > 0 && s >= 0 && s + (long long)(p.rows_per_chunk - 1) * p.hop + (p.pitch_bytes >> 2) <= total;
+                    if (p.vpad > 0) {   // and every valid frame of the chunk inside its clip (what lies beyond is mirrored, not the next clip)
+                        const long long tlast = row0 + 31 < ti.T - 1 ? row0 + 31 : ti.T - 1;
+                        by_tma = by_tma && st >= 0 && tlast * p.hop - p.vpad + p.n_fft <= clip_len;
+                    }
                 }
                 // The staging ring holds less than two tiles, so the loader usually sits here waiting for a slot: pull the
                 // chunk into L2 meanwhile -- when the slot frees, the copy into shared memory costs an L2 hit, not a DRAM access
                 if (by_tma && elect_one()) tma_prefetch_l2_3d(p.tmap, c0, c1, c2);
                 __syncwarp();
                 TRACE(10);
-                mbar_wait(BAR(V_STG_EMPTY + slot), ph ^ 1u);
+                if (chunk_count >= S) {      // the slot's previous tenant, chunk c - S, has been read by every converter group
+                    mbar_wait(BAR(V_STG_EMPTY + eq + 4 * etp), eph);
+                    if (++eq == 4) { eq = 0; if (++etp == P) { etp = 0; eph ^= 1u; } }
+                }
+                const uint32_t full = BAR(V_STG_FULL + cq + 4 * ctp);
                 TRACE(11);
+                if (p.vpad > 0 && !by_tma && n_rows > 0) {
+                    // Edge chunk of a reflect-padded clip (its first chunk and its last one or two): hop-rows that lie inside the
+                    // clip are bulk-copied as they are; the two or three rows that reach before the first or beyond the last
+                    // sample are filled element by element with the mirrored samples x[-j] / x[2 (len - 1) - j] (numpy 'reflect':
+                    // the edge sample is not repeated).  Ragged batches: in the layout the realignment pass expects (the chunk as
+                    // fetched from the aligned sample below its start).
+                    const int pw = p.pitch_bytes >> 2;
+                    const long long jbase = st - (ragged ? (ti.s0 & 3ll) : 0ll);
+                    float *dstp = reinterpret_cast<float *>(smem + p.off_stg + (size_t)slot * p.slot_bytes);
+                    uint32_t bulk_bytes = 0;
+                    for (int r = 0; r < n_rows; ++r) {
+                        const long long jlo = jbase + (long long)r * p.hop;
+                        if (jlo >= 0 && jlo + pw <= clip_len) { bulk_bytes += (uint32_t)p.pitch_bytes; continue; }
+                        for (int col = lane; col < pw; col += 32) {
+                            long long j = jlo + col;
+                            j = j < 0 ? -j : j;
+                            j = j >= clip_len ? 2 * (clip_len - 1) - j : j;
+                            j = j < 0 ? 0 : (j >= clip_len ? clip_len - 1 : j);   // rows no valid frame reads: any finite sample
+                            dstp[r * pw + col] = __ldg(xb + j);
+                        }
+                    }
+                    __syncwarp();   // every lane's stores precede lane 0's arrival below
+                    if (elect_one()) {
+                        if (bulk_bytes) mbar_arrive_expect_tx(full, bulk_bytes);
+                        else mbar_arrive(full);
+                        for (int r = 0; r < n_rows; ++r) {
+                            const long long jlo = jbase + (long long)r * p.hop;
+                            if (jlo >= 0 && jlo + pw <= clip_len) bulk_g2s(dst0 + (uint32_t)r * (uint32_t)p.pitch_bytes, xb + jlo, (uint32_t)p.pitch_bytes, full);
+                        }
+                    }
+                    __syncwarp();
+                    TRACE(12);
+                    if (++slot == S) slot = 0;
+                    ++chunk_count;
+                    if (++cq == 4) { cq = 0; if (++ctp == P) { ctp = 0; cph ^= 1u; } }
+                    continue;
+                }
                 if (ragged && !by_tma) {
                     // the few chunks that reach beyond the packed buffer (end of the last clip), or rows of no valid frame:
                     // plain bounds-checked loads by the whole warp (the bulk-copy engine needs 16-byte aligned sources)
@@ -416,10 +499,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         dstp[idx] = g < total ? __ldg(p.x + g) : 0.f;
                     }
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(BAR(V_STG_FULL + slot));
+                    if (lane == 0) mbar_arrive(full);
                     __syncwarp();
                     TRACE(12);
-                    if (++slot == S) { slot = 0; ph ^= 1u; }
+                    if (++slot == S) slot = 0;
+                    ++chunk_count;
+                    if (++cq == 4) { cq = 0; if (++ctp == P) { ctp = 0; cph ^= 1u; } }
                     continue;
                 }
                 if (!by_tma && n_rows > 0) {
@@ -430,7 +515,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     __syncwarp();
                 }
                 if (elect_one()) {
-                    const uint32_t full = BAR(V_STG_FULL + slot);
                     if (by_tma) {
                         // one tensor-map box = the whole chunk: rows_per_chunk hop-rows of pitch width (implicit im2col)
                         mbar_arrive_expect_tx(full, (uint32_t)p.rows_per_chunk * (uint32_t)p.pitch_bytes);
@@ -452,15 +536,18 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 }
                 __syncwarp();
                 TRACE(12);
-                if (++slot == S) { slot = 0; ph ^= 1u; }
+                if (++slot == S) slot = 0;
+                ++chunk_count;
+                if (++cq == 4) { cq = 0; if (++ctp == P) { ctp = 0; cph ^= 1u; } }
             }
         }
+        (void)cph;
+        if (EARLY_LOADER) cluster_wait();   // the phase it arrived on at set-up, before the exit barrier below
     } else if (warp == W_BASIS) {
         // ============================================================== basis: this CTA's half, resident
         // One barrier per K-step slab, so that the first tile's MMAs start as soon as the first slabs have landed.
         if (first_tile < n_tiles) {
-            // the image is replicated in global memory: 74 clusters fetching the same lines at once serialise in L2
-            const uint8_t *src = p.b_img + ((size_t)(cluster_id_x() % (uint32_t)p.b_replicas) * 2 + rank) * p.passes * p.units * p.unit_b_bytes;
+            const uint8_t *src = p.b_img + (size_t)rank * p.passes * p.units * p.unit_b_bytes;   // this CTA's half of the Mel rows
             if (!STREAM) {   // a template parameter: the resident instantiation carries no streaming code (0.7 us per cfg1 step)
                 if (elect_one()) {
                     for (int u = 0; u < p.units; ++u) {
@@ -731,7 +818,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         const uint32_t a_full_remote = mapa_cluster(BAR(V_A_FULL), 0);
         const uint32_t row_off = sbase + p.off_stg + (uint32_t)lane * (uint32_t)p.pitch_bytes;
         const float S_in = p.in_scale;
-        int sslot = q;
+        int sslot = q;                           // memory slot of this warp's chunk: (4 tl + q) mod S
+        int sbar = q;                            // its barriers: q + 4 (tl mod P) (see the loader)
         uint32_t sph = 0;
         int aslot = g % p.a_slots;               // ring position of unit counter ug = it * units + u, first u = g
         uint32_t aph = (uint32_t)((g / p.a_slots) & 1);
@@ -773,7 +861,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 const long long trow = ti.t0 + (int)rank * 128 + q * 32 + lane;
                 gxb = reinterpret_cast<const char *>(p.x + ti.s0 + (trow < ti.T ? trow : 0) * p.hop);   // rows of no frame re-read frame 0
             } else {
-                mbar_wait(BAR(V_STG_FULL + sslot), sph);
+                mbar_wait(BAR(V_STG_FULL + sbar), sph);
             }
             if (RAGGED) {   // a template parameter: the dense instantiation must not carry this call in its converter loop
                 // ragged: group 0's warp realigns its chunk (see the loader), the other groups wait for it
@@ -781,9 +869,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     ragged_realign(p.offsets, p.tile_prefix, p.n_clips, p.passes > 1 ? tile / p.passes : tile,
                                    reinterpret_cast<float *>(smem + p.off_stg + (size_t)sslot * p.slot_bytes),
                                    p.rows_per_chunk * (p.pitch_bytes >> 2), lane);
-                    if (lane == 0) mbar_arrive(BAR(V_STG_READY + sslot));
+                    if (lane == 0) mbar_arrive(BAR(V_STG_READY + sbar));
                 } else {
-                    mbar_wait(BAR(V_STG_READY + sslot), sph);
+                    mbar_wait(BAR(V_STG_READY + sbar), sph);
                 }
             }
             TRACE(41);
@@ -795,7 +883,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             do {                                                                                    \
                 if (!DIRECT && u + NG >= p.units) {                                                 \
                     __syncwarp();                                                                   \
-                    if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));                           \
+                    if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sbar));                            \
                     released = true;                                                                \
                 }                                                                                   \
             } while (0)
@@ -902,10 +990,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             u -= p.units;   // position in the next tile
             if (!DIRECT && !released) {   // a group without K-steps in this geometry
                 __syncwarp();
-                if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sslot));
+                if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sbar));
             }
             sslot += 4;
-            if (sslot >= S) { sslot -= S; sph ^= 1u; }
+            if (sslot >= S) sslot -= S;
+            sbar += 4;
+            if (sbar >= 4 * p.stg_phases) { sbar -= 4 * p.stg_phases; sph ^= 1u; }
             if (SHARE) {
                 if (pend_tile >= 0) DRAIN_PENDING();   // short windows: fewer than three K-steps per group
                 pend_tile = tile;
@@ -938,16 +1028,20 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
 // ---------------------------------------------------------------------------------------------- launch (per precision TU)
 template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM, bool DIRECT>
 static int launch_one_s(const K2Params &kp, int grid, cudaStream_t stream) {
-    static bool attr_done = false;
-    if (!attr_done) {
+    // the opt-in shared-memory size is a per-device attribute of the function: set once per device (bit d of the mask)
+    static std::atomic<unsigned long long> attr_done{0};
+    int dev = 0;
+    MELT_CUDA(cudaGetDevice(&dev));
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (dev >= 64 || !(attr_done.load(std::memory_order_acquire) & bit)) {
         MELT_CUDA(cudaFuncSetAttribute(melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE, STREAM, DIRECT>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BUDGET));
-        attr_done = true;
+        attr_done.fetch_or(bit, std::memory_order_release);
     }
-    // Programmatic dependent launch: when the previous operation in the stream is another forward of this library, the
-    // CTAs of this grid are dispatched as soon as SMs of the previous grid free up (its clusters finish at different
-    // times: 384 tiles on 74 pairs), instead of after its last CTA has retired and a fresh launch has ramped up.  The
-    // kernel orders itself behind the previous grid (griddepcontrol.wait) before its first global store; it reads only
-    // the caller's signal and the plan's tables before that.  Any other predecessor serialises as usual.
+    // Programmatic dependent launch: the CTAs of this grid are dispatched as soon as SMs of the previous kernel in the stream
+    // free up (its clusters finish at different times: 384 tiles on 74 pairs), instead of after its last CTA has retired and
+    // a fresh launch has ramped up.  The kernel orders itself behind that kernel with griddepcontrol.wait: before its first read
+    // of the caller's buffers by default, before its first global store only when the caller vouches for the input
+    // (K2Params::input_ready, MELT_OPT_INPUT_READY).
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid, 1, 1);
     cfg.blockDim = dim3(V2_THREADS, 1, 1);
@@ -956,10 +1050,16 @@ static int launch_one_s(const K2Params &kp, int grid, cudaStream_t stream) {
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
-    static const bool no_pdl = getenv("MELT_NO_PDL") != nullptr;   // debug switch
     cfg.attrs = attr;
-    cfg.numAttrs = (no_pdl || kp.offsets != nullptr) ? 0 : 1;   // ragged: the scan kernel's results are read at kernel entry
+    cfg.numAttrs = 1;
+#ifdef MELT_TRACE
+    static int trace_slot = 0;   // development builds: every launch records into its own region of the trace buffer (16 regions)
+    K2Params kt = kp;
+    kt.trace_slot = trace_slot++ & 15;
+    MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE, STREAM, DIRECT>, kt));
+#else
     MELT_CUDA(cudaLaunchKernelEx(&cfg, melt_fwd2_kernel<PREC, SIGMA, RAGGED, MODE, STREAM, DIRECT>, kp));
+#endif
     return MELT_OK;
 }
 
@@ -978,9 +1078,8 @@ static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
     // Plain log-Mel output: no dedicated epilogue warps, three converter groups that also drain (MODE 2); everything else keeps
     // the four epilogue warps (MODE 0).  (MODE 1, epilogue + converter warps draining a single-stage accumulator, measured the
     // same as MODE 2 on cfg2 and is not instantiated.)
-    static const int forced = getenv("MELT_V2_MODE") ? atoi(getenv("MELT_V2_MODE")) : -1;   // debug switch: 0 forces the epilogue warps
     const bool plain = kp.n_mfcc == 0 && !kp.output_power && kp.tap == nullptr;
-    const int mode = (plain && forced != 0) ? 2 : 0;
+    const int mode = plain ? 2 : 0;
     if (kp.offsets) return mode == 2 ? launch_one_r<PREC, SIGMA, true, 2>(kp, grid, stream) : launch_one_r<PREC, SIGMA, true, 0>(kp, grid, stream);
     return mode == 2 ? launch_one_r<PREC, SIGMA, false, 2>(kp, grid, stream) : launch_one_r<PREC, SIGMA, false, 0>(kp, grid, stream);
 }

@@ -226,78 +226,103 @@ static int validate_common(const melt_plan *p, const float *x, float *out) {
     return MELT_OK;
 }
 
+// Per-call device scratch from the plan's stream-ordered pool: usable by work submitted to `st` after this call, released
+// (cudaFreeAsync on `st`) once everything that uses it has been submitted.  No host synchronisation, nothing stored in the plan.
+static int scratch_alloc(const melt_plan *p, void **ptr, size_t bytes, cudaStream_t st) {
+    *ptr = nullptr;
+    if (cudaMallocFromPoolAsync(ptr, bytes, p->pool, st) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return fail(MELT_ERR_ALLOC, "per-call scratch of %zu bytes (stream-ordered pool)", bytes);
+    }
+    return MELT_OK;
+}
+
 static int forward_impl(const melt_plan *p, const float *x, const long long *offsets, int n_clips, long long len,
-                        float *out, float *tap, long long *out_frame_offsets, void *stream) {
+                        float *out, float *tap, long long *out_frame_offsets, void *stream, bool input_ready) {
     int rc = validate_common(p, x, out);
     if (rc) return rc;
     if (n_clips < 0) return fail(MELT_ERR_INVALID_ARG, "negative clip count");
     if (tap && ((uintptr_t)tap & 3)) return fail(MELT_ERR_ALIGNMENT, "logmel must be 4-byte aligned");
-    const_cast<melt_plan *>(p)->used = true;
+    p->used.store(true, std::memory_order_relaxed);
     if (n_clips == 0) return MELT_OK;
     KParams kp = p->kp;
     kp.x = x; kp.out = out; kp.tap = tap; kp.n_clips = n_clips;
     cudaStream_t st = (cudaStream_t)stream;
+    const bool reflect = p->pad == MELT_PAD_REFLECT;
     if (offsets) {
         if (n_clips > MAX_CLIPS) return fail(MELT_ERR_UNSUPPORTED, "n_clips=%d exceeds %d", n_clips, MAX_CLIPS);
         if (!out_frame_offsets) return fail(MELT_ERR_INVALID_ARG, "out_frame_offsets is NULL");
         if (kp.feature_major) return fail(MELT_ERR_UNSUPPORTED, "ragged batches are frame-major only");
-        if (p->v2_ok && !p->k2.direct && (((uintptr_t)x & 15) == 0)) {
+        // the device-side tile index of this call (exclusive prefix of tiles per clip): per-call scratch, so that ragged
+        // forwards of one plan may run concurrently on several streams
+        int *tile_prefix = nullptr;
+        rc = scratch_alloc(p, (void **)&tile_prefix, sizeof(int) * ((size_t)n_clips + 1), st);
+        if (rc) return rc;
+        const bool v2 = p->v2_ok && !p->k2.direct && (((uintptr_t)x & 15) == 0);
+        if (v2) {
             // the CTA-pair kernel: 256-frame tiles, looked up on the device; chunks start at any sample of the packed buffer
-            rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, 256, st);
-            if (rc) return rc;
+            rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, tile_prefix, 256, st);
             K2Params k2 = p->k2;
             k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = 0; k2.frames_per_clip = 0;
             k2.tiles_per_clip = 0; k2.n_tiles = -1;
-            k2.offsets = offsets; k2.frame_offsets = out_frame_offsets; k2.tile_prefix = p->d_tile_prefix;
-            if (v2_encode_tmap_ragged(k2) == MELT_OK && k2.tma_rows > 0) return launch_forward2(p, k2, st);
-        }
-        rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, TILE_M, st);
-        if (rc) return rc;
-        kp.offsets = offsets; kp.frame_offsets = out_frame_offsets; kp.tile_prefix = p->d_tile_prefix;
-        kp.len = 0; kp.frames_per_clip = 0; kp.tiles_per_clip = 0; kp.n_tiles = -1;
-    } else {
-        if (len < 0) return fail(MELT_ERR_INVALID_ARG, "negative len");
-        const long long T = frames_for(p, len);
-        if (T == 0) return MELT_OK;
-        const long long tpc = (T + TILE_M - 1) / TILE_M;
-        if (tpc * n_clips > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
-        // reflect padding: the padded copy is aligned whatever x is; it only needs a length that keeps the clip starts aligned
-        // and a batch that is not 16-byte aligned (pointer or clip length) takes the same route with a pad of zero samples:
-        // one pass copies it into the plan-owned buffer at an aligned clip stride
-        const bool realign = p->pad == MELT_PAD_NONE && p->v2_ok && !v2_accepts(p, x, len);
-        const bool v2_in = p->pad == MELT_PAD_REFLECT ? (p->v2_ok && ((len + p->n_fft) & 3) == 0 && !(p->n_fft & 1)) : p->v2_ok;
-        if (v2_in && !(tap && ((uintptr_t)tap & 3))) {
-            K2Params k2 = p->k2;
-            if (p->pad == MELT_PAD_REFLECT || realign) {
-                // in-library reflect padding on the fast path: one pass writes the padded signal into a plan-owned copy (allocated
-                // on the first such call, re-allocated only for a bigger batch), the kernel then frames the copy
-                const int padn = realign ? 0 : p->n_fft / 2;
-                const long long plen = realign ? ((len + 3) & ~3LL) : len + 2LL * padn;   // realign: up to 3 filler samples no frame reads
-                const size_t need = (size_t)n_clips * (size_t)plen * sizeof(float);
-                melt_plan *mp = const_cast<melt_plan *>(p);
-                if (need > mp->ws_pad_bytes) {
-                    MELT_CUDA(cudaStreamSynchronize(st));
-                    cudaFree(mp->ws_pad);
-                    mp->ws_pad = nullptr; mp->ws_pad_bytes = 0;
-                    if (cudaMalloc(&mp->ws_pad, need) != cudaSuccess) { (void)cudaGetLastError(); return fail(MELT_ERR_ALLOC, "padded-signal workspace of %zu bytes", need); }
-                    mp->ws_pad_bytes = need;
-                }
-                rc = launch_reflect_pad(x, mp->ws_pad, n_clips, len, padn, plen, st);
-                if (rc) return rc;
-                x = mp->ws_pad;
-                len = plen;
+            k2.offsets = offsets; k2.frame_offsets = out_frame_offsets; k2.tile_prefix = tile_prefix;
+            k2.vpad = reflect ? p->n_fft / 2 : 0;
+            k2.input_ready = 0;   // the scan kernel just ahead in the stream produces what the kernel reads at its entry
+            if (rc == MELT_OK && v2_encode_tmap_ragged(k2) == MELT_OK && k2.tma_rows > 0) {
+                rc = launch_forward2(p, k2, st);
+                cudaFreeAsync(tile_prefix, st);
+                return rc;
             }
-            const long long tpc2 = (T + 255) / 256;
-            if (tpc2 * n_clips * std::max(1, p->k2.passes) > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
-            k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = len; k2.frames_per_clip = T;
-            k2.tiles_per_clip = (int)tpc2; k2.n_tiles = (int)(tpc2 * n_clips);
-            k2.offsets = nullptr; k2.frame_offsets = nullptr; k2.tile_prefix = nullptr;
-            v2_encode_tmap(k2);
-            return launch_forward2(p, k2, st);
         }
-        kp.offsets = nullptr; kp.frame_offsets = nullptr; kp.tile_prefix = nullptr;
-        kp.len = len; kp.frames_per_clip = T; kp.tiles_per_clip = (int)tpc; kp.n_tiles = (int)(tpc * n_clips);
+        if (rc == MELT_OK) rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, tile_prefix, TILE_M, st);
+        kp.offsets = offsets; kp.frame_offsets = out_frame_offsets; kp.tile_prefix = tile_prefix;
+        kp.len = 0; kp.frames_per_clip = 0; kp.tiles_per_clip = 0; kp.n_tiles = -1;
+        if (rc == MELT_OK) rc = launch_forward(p, kp, st);
+        cudaFreeAsync(tile_prefix, st);
+        return rc;
     }
+    if (len < 0) return fail(MELT_ERR_INVALID_ARG, "negative len");
+    const long long T = frames_for(p, len);
+    if (T == 0) return MELT_OK;
+    const long long tpc = (T + TILE_M - 1) / TILE_M;
+    if (tpc * n_clips > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
+    if (p->v2_ok && !(tap && ((uintptr_t)tap & 3))) {
+        K2Params k2 = p->k2;
+        const bool aligned = v2_accepts(p, x, len);
+        // Reflect padding is virtual on the staged forms of the kernel (the loader's edge path mirrors the indices).  Two cases
+        // still take ONE copy pass into pool scratch first: a batch whose clip starts are not 16-byte aligned (pointer or clip
+        // length; copied at an aligned clip stride), and reflect padding on the direct-load form (very long windows, whose
+        // converter threads read their frames from global memory and cannot mirror): the padded signal is written out.
+        const bool copy_pad = reflect && (k2.direct || !aligned);
+        const bool realign = !reflect && !aligned;
+        float *scratch = nullptr;
+        if (copy_pad || realign) {
+            const int padn = copy_pad ? p->n_fft / 2 : 0;
+            const long long plen = (len + 2LL * padn + 3) & ~3LL;   // up to 3 filler samples no frame reads
+            rc = scratch_alloc(p, (void **)&scratch, (size_t)n_clips * (size_t)plen * sizeof(float), st);
+            if (rc) return rc;
+            rc = launch_reflect_pad(x, scratch, n_clips, len, padn, plen, st);
+            if (rc) { cudaFreeAsync(scratch, st); return rc; }
+            x = scratch;
+            len = plen;
+            k2.vpad = 0;
+            k2.input_ready = 0;   // the copy kernel just ahead in the stream produces the kernel's input
+        } else {
+            k2.vpad = reflect ? p->n_fft / 2 : 0;
+            k2.input_ready = input_ready ? 1 : 0;
+        }
+        const long long tpc2 = (T + 255) / 256;
+        if (tpc2 * n_clips * std::max(1, p->k2.passes) > 0x7fffffffLL) { if (scratch) cudaFreeAsync(scratch, st); return fail(MELT_ERR_UNSUPPORTED, "too many tiles"); }
+        k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = len; k2.frames_per_clip = T;
+        k2.tiles_per_clip = (int)tpc2; k2.n_tiles = (int)(tpc2 * n_clips);
+        k2.offsets = nullptr; k2.frame_offsets = nullptr; k2.tile_prefix = nullptr;
+        v2_encode_tmap(k2);
+        rc = launch_forward2(p, k2, st);
+        if (scratch) cudaFreeAsync(scratch, st);
+        return rc;
+    }
+    kp.offsets = nullptr; kp.frame_offsets = nullptr; kp.tile_prefix = nullptr;
+    kp.len = len; kp.frames_per_clip = T; kp.tiles_per_clip = (int)tpc; kp.n_tiles = (int)(tpc * n_clips);
     return launch_forward(p, kp, st);
 }
 
@@ -330,11 +355,26 @@ extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window
     p->fs = fs; p->fmin = fmin; p->fmax = fmax; p->n_fft = n_fft; p->hop = hop; p->window = window; p->n_mels = n_mels;
     p->mel_scale = mel_scale; p->n_mfcc = n_mfcc;
     p->layout = MELT_LAYOUT_FRAME_MAJOR; p->precision = MELT_PREC_COMPENSATED; p->drop_last = 0; p->pad = MELT_PAD_NONE;
-    p->in_scale_log2 = 12; p->output = MELT_OUTPUT_LOG; p->used = false; p->device = dev; p->sm_count = prop.multiProcessorCount;
-    p->d_bimg = nullptr; p->d_bimg2 = nullptr; p->v2_ok = false; p->v2_sigma = 0; p->d_tab = nullptr; p->d_dct = nullptr; p->d_tile_prefix = nullptr; p->d_frame_offsets_scratch = nullptr;
+    p->in_scale_log2 = 12; p->output = MELT_OUTPUT_LOG; p->input_ready = 0; p->used.store(false); p->device = dev; p->sm_count = prop.multiProcessorCount;
+    p->d_bimg = nullptr; p->d_bimg2 = nullptr; p->v2_ok = false; p->v2_sigma = 0; p->d_tab = nullptr; p->d_dct = nullptr;
+    p->pool = nullptr; p->copy_in = nullptr; p->copy_out = nullptr;
     memset(&p->kp, 0, sizeof(p->kp));
-    p->ws_in = nullptr; p->ws_out = nullptr; p->ws_in_bytes = p->ws_out_bytes = 0;
-    p->ws_pad = nullptr; p->ws_pad_bytes = 0;
+    {   // the scratch pool: device memory of this device, kept (not returned to the driver) between calls
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof(props));
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        e = cudaMemPoolCreate(&p->pool, &props);
+        if (e == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            e = cudaMemPoolSetAttribute(p->pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->copy_in, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&p->copy_out, cudaStreamNonBlocking);
+        if (e != cudaSuccess) { cuda_fail(e, "scratch pool / copy streams"); melt_plan_destroy(p); return nullptr; }
+    }
     // Eq. (1)-(2): M centres uniformly spaced in mel between fmin and fmax, endpoints excluded
     p->centres.resize(n_mels);
     const double mlo = hz_to_mel(fmin), mhi = hz_to_mel(fmax);
@@ -345,8 +385,6 @@ extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window
         else if (window == MELT_WINDOW_HANN_SYMMETRIC) p->win[n] = 0.5 - 0.5 * std::cos(2.0 * kPi * n / (n_fft - 1));
         else p->win[n] = 1.0;
     }
-    e = cudaMalloc(&p->d_tile_prefix, sizeof(int) * (size_t)(MAX_CLIPS + 1));
-    if (e != cudaSuccess) { cuda_fail(e, "cudaMalloc(tile_prefix)"); melt_plan_destroy(p); return nullptr; }
     if (plan_build_device(p) != MELT_OK) { melt_plan_destroy(p); return nullptr; }
     return p;
 }
@@ -354,16 +392,15 @@ extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window
 extern "C" void melt_plan_destroy(melt_plan *p) {
     if (!p) return;
     free_device(p);
-    cudaFree(p->d_tile_prefix);
-    cudaFree(p->ws_in);
-    cudaFree(p->ws_out);
-    cudaFree(p->ws_pad);
+    if (p->copy_in) cudaStreamDestroy(p->copy_in);
+    if (p->copy_out) cudaStreamDestroy(p->copy_out);
+    if (p->pool) cudaMemPoolDestroy(p->pool);
     delete p;
 }
 
 extern "C" int melt_plan_set_option(melt_plan *p, int key, int value) {
     if (!p) return fail(MELT_ERR_INVALID_ARG, "plan is NULL");
-    if (p->used) return fail(MELT_ERR_INVALID_ARG, "plan is immutable after its first forward call");
+    if (p->used.load()) return fail(MELT_ERR_INVALID_ARG, "plan is immutable after its first forward call");
     switch (key) {
         case MELT_OPT_LAYOUT:
             if (value < 0 || value > 1) return fail(MELT_ERR_INVALID_ARG, "bad layout %d", value);
@@ -384,6 +421,10 @@ extern "C" int melt_plan_set_option(melt_plan *p, int key, int value) {
             if (value < 0 || value > 1) return fail(MELT_ERR_INVALID_ARG, "bad output %d", value);
             if (value == MELT_OUTPUT_POWER && p->n_mfcc > 0) return fail(MELT_ERR_INVALID_ARG, "power output needs n_mfcc == 0");
             p->output = value; break;
+        case MELT_OPT_INPUT_READY:
+            if (value < 0 || value > 1) return fail(MELT_ERR_INVALID_ARG, "bad input_ready %d", value);
+            p->input_ready = value;
+            return MELT_OK;   // a launch-time flag: no operand image depends on it
         default:
             return fail(MELT_ERR_INVALID_ARG, "unknown option %d", key);
     }
@@ -391,6 +432,26 @@ extern "C" int melt_plan_set_option(melt_plan *p, int key, int value) {
 }
 
 extern "C" long long melt_num_frames(const melt_plan *p, long long len) { return p ? frames_for(p, len) : 0; }
+extern "C" long long melt_count_frames(long long len, int n_fft, int hop, int pad, int drop_last) {
+    if (len < 0 || n_fft < 1 || hop < 1) return 0;
+    long long padded = len;
+    if (pad == MELT_PAD_REFLECT) {
+        if (len < (long long)(n_fft / 2) + 1) return 0;
+        padded += 2LL * (n_fft / 2);
+    }
+    if (padded < n_fft) return 0;
+    const long long T = (padded - n_fft) / hop + 1 - (drop_last ? 1 : 0);
+    return T < 0 ? 0 : T;
+}
+extern "C" int melt_plan_reserve(melt_plan *p, unsigned long long bytes) {
+    if (!p) return fail(MELT_ERR_INVALID_ARG, "plan is NULL");
+    if (bytes == 0) return MELT_OK;
+    void *q = nullptr;   // grow the pool once: the memory stays with it (release threshold = unlimited)
+    if (cudaMallocFromPoolAsync(&q, (size_t)bytes, p->pool, nullptr) != cudaSuccess) { (void)cudaGetLastError(); return fail(MELT_ERR_ALLOC, "reserve of %llu bytes", bytes); }
+    MELT_CUDA(cudaFreeAsync(q, nullptr));
+    MELT_CUDA(cudaStreamSynchronize(nullptr));
+    return MELT_OK;
+}
 extern "C" int melt_num_channels(const melt_plan *p) { return p ? p->kp.n_ch : 0; }
 
 extern "C" int melt_plan_get_centres(const melt_plan *p, double *f_hz) {
@@ -402,41 +463,81 @@ extern "C" int melt_plan_get_centres(const melt_plan *p, double *f_hz) {
 extern "C" const char *melt_plan_describe(const melt_plan *p) { return p ? p->desc.c_str() : ""; }
 
 extern "C" int melt_forward(const melt_plan *p, const float *x, int batch, long long len, float *out, void *stream) {
-    return forward_impl(p, x, nullptr, batch, len, out, nullptr, nullptr, stream);
+    return forward_impl(p, x, nullptr, batch, len, out, nullptr, nullptr, stream, p && p->input_ready);
 }
-extern "C" int melt_forward_host(melt_plan *p, const float *x_host, int batch, long long len, float *out_host, void *stream) {
+
+// Host buffers: the batch is cut into groups of clips; upload of group k + 1 (copy_in stream), kernel of group k (the caller's
+// stream) and download of group k - 1 (copy_out stream) overlap.  PCIe is full duplex, so the call costs about
+// max(upload, download) + one group's worth of the other two stages instead of their sum.
+extern "C" int melt_forward_host(const melt_plan *p, const float *x_host, int batch, long long len, float *out_host, void *stream) {
     if (!p) return fail(MELT_ERR_INVALID_ARG, "plan is NULL");
     if (batch < 0 || len < 0) return fail(MELT_ERR_INVALID_ARG, "negative batch / len");
     const long long T = frames_for(p, len);
     if (batch == 0 || T == 0) return MELT_OK;
     if (!x_host || !out_host) return fail(MELT_ERR_INVALID_ARG, "x_host / out_host is NULL");
-    const size_t in_bytes = (size_t)batch * (size_t)len * sizeof(float);
-    const size_t out_bytes = (size_t)batch * (size_t)T * (size_t)p->kp.n_ch * sizeof(float);
+    int dev = -1;
+    MELT_CUDA(cudaGetDevice(&dev));
+    if (dev != p->device) return fail(MELT_ERR_INVALID_ARG, "plan was created on device %d, current device is %d", p->device, dev);
+    const size_t clip_in = (size_t)len, clip_out = (size_t)T * (size_t)p->kp.n_ch;
     cudaStream_t st = (cudaStream_t)stream;
-    if (in_bytes > p->ws_in_bytes || out_bytes > p->ws_out_bytes) {   // (re)size the plan-owned device workspace: first call / bigger batch only
-        MELT_CUDA(cudaStreamSynchronize(st));
-        cudaFree(p->ws_in); cudaFree(p->ws_out);
-        p->ws_in = nullptr; p->ws_out = nullptr; p->ws_in_bytes = p->ws_out_bytes = 0;
-        if (cudaMalloc(&p->ws_in, in_bytes) != cudaSuccess || cudaMalloc(&p->ws_out, out_bytes) != cudaSuccess) {
-            cudaFree(p->ws_in); cudaFree(p->ws_out);
-            p->ws_in = nullptr; p->ws_out = nullptr;
-            (void)cudaGetLastError();
-            return fail(MELT_ERR_ALLOC, "device workspace of %zu + %zu bytes", in_bytes, out_bytes);
-        }
-        p->ws_in_bytes = in_bytes; p->ws_out_bytes = out_bytes;
-    }
-    MELT_CUDA(cudaMemcpyAsync(p->ws_in, x_host, in_bytes, cudaMemcpyHostToDevice, st));
-    const int rc = forward_impl(p, p->ws_in, nullptr, batch, len, p->ws_out, nullptr, nullptr, stream);
+    float *ws_in = nullptr, *ws_out = nullptr;
+    int rc = scratch_alloc(p, (void **)&ws_in, (size_t)batch * clip_in * sizeof(float), st);
     if (rc) return rc;
-    MELT_CUDA(cudaMemcpyAsync(out_host, p->ws_out, out_bytes, cudaMemcpyDeviceToHost, st));
+    rc = scratch_alloc(p, (void **)&ws_out, (size_t)batch * clip_out * sizeof(float), st);
+    if (rc) { cudaFreeAsync(ws_in, st); return rc; }
+    // groups of clips: about 4 MB of input each, at most 16 groups
+    int per = (int)std::max<size_t>(1, ((size_t)4 << 20) / (clip_in * sizeof(float)));
+    if ((batch + per - 1) / per > 16) per = (batch + 15) / 16;
+    const int groups = (batch + per - 1) / per;
+    cudaEvent_t ev_start = nullptr, ev_in[16] = {}, ev_k[16] = {}, ev_done = nullptr;
+    cudaError_t e = cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming);
+    for (int g = 0; g < groups && e == cudaSuccess; ++g) {
+        e = cudaEventCreateWithFlags(&ev_in[g], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_k[g], cudaEventDisableTiming);
+    }
+    auto cleanup = [&]() {   // destroying a recorded event is legal: its resources are released when it has completed
+        if (ev_start) cudaEventDestroy(ev_start);
+        if (ev_done) cudaEventDestroy(ev_done);
+        for (int g = 0; g < 16; ++g) { if (ev_in[g]) cudaEventDestroy(ev_in[g]); if (ev_k[g]) cudaEventDestroy(ev_k[g]); }
+    };
+    if (e != cudaSuccess) { cleanup(); cudaFreeAsync(ws_in, st); cudaFreeAsync(ws_out, st); return cuda_fail(e, "cudaEventCreate"); }
+    // the copy streams start behind everything already in the caller's stream (which includes the scratch allocations)
+    e = cudaEventRecord(ev_start, st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(p->copy_in, ev_start, 0);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(p->copy_out, ev_start, 0);
+    rc = MELT_OK;
+    for (int g = 0; g < groups && e == cudaSuccess && rc == MELT_OK; ++g) {
+        const int b0 = g * per, nb = std::min(per, batch - b0);
+        e = cudaMemcpyAsync(ws_in + (size_t)b0 * clip_in, x_host + (size_t)b0 * clip_in, (size_t)nb * clip_in * sizeof(float), cudaMemcpyHostToDevice, p->copy_in);
+        if (e == cudaSuccess) e = cudaEventRecord(ev_in[g], p->copy_in);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_in[g], 0);
+        if (e != cudaSuccess) break;
+        // the kernel's input was produced by a copy it is fully ordered behind (event), never by the kernel ahead of it
+        rc = forward_impl(p, ws_in + (size_t)b0 * clip_in, nullptr, nb, len, ws_out + (size_t)b0 * clip_out, nullptr, nullptr, stream, true);
+        if (rc != MELT_OK) break;
+        e = cudaEventRecord(ev_k[g], st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(p->copy_out, ev_k[g], 0);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync(out_host + (size_t)b0 * clip_out, ws_out + (size_t)b0 * clip_out, (size_t)nb * clip_out * sizeof(float),
+                                cudaMemcpyDeviceToHost, p->copy_out);
+    }
+    // the caller's stream waits for the last download; the scratch goes back to the pool behind it
+    if (e == cudaSuccess) e = cudaEventRecord(ev_done, p->copy_out);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_done, 0);
+    cudaFreeAsync(ws_in, st);
+    cudaFreeAsync(ws_out, st);
+    cleanup();
+    if (rc != MELT_OK) return rc;
+    if (e != cudaSuccess) return cuda_fail(e, "melt_forward_host pipeline");
     return MELT_OK;
 }
 extern "C" int melt_forward_ragged(const melt_plan *p, const float *x, const long long *offsets, int n_clips, float *out,
                                    long long *out_frame_offsets, void *stream) {
     if (!offsets) return fail(MELT_ERR_INVALID_ARG, "offsets is NULL");
-    return forward_impl(p, x, offsets, n_clips, 0, out, nullptr, out_frame_offsets, stream);
+    return forward_impl(p, x, offsets, n_clips, 0, out, nullptr, out_frame_offsets, stream, false);
 }
 extern "C" int melt_forward_tap(const melt_plan *p, const float *x, const long long *offsets, int n_clips, long long len,
                                 float *out, float *logmel, long long *out_frame_offsets, void *stream) {
-    return forward_impl(p, x, offsets, n_clips, len, out, logmel, out_frame_offsets, stream);
+    return forward_impl(p, x, offsets, n_clips, len, out, logmel, out_frame_offsets, stream, p && p->input_ready);
 }

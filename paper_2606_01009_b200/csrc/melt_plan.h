@@ -2,6 +2,8 @@
 #pragma once
 #include "melt_internal.h"
 
+#include <atomic>
+
 namespace melt {
 
 constexpr int TILE_M = 128;         // frames per tile = UMMA M
@@ -54,7 +56,10 @@ struct KParams {
 };
 
 // ---------------------------------------------------------------------------------------------- v2 (CTA-pair kernel)
-constexpr int V2_CONV_GROUPS = 2;     // converter groups of 4 warps (one warp per tensor-memory lane quarter); 3 groups
+#ifndef MELT_X_GROUPS
+#define MELT_X_GROUPS 2
+#endif
+constexpr int V2_CONV_GROUPS = MELT_X_GROUPS;     // converter groups of 4 warps (one warp per tensor-memory lane quarter); 3 groups
                                       // (640 threads, 96 registers) measured no faster on the Whisper shape
 constexpr int V2_THREADS = 128 * (2 + V2_CONV_GROUPS);   // warps: loader, MMA issuer R, basis/TMEM, MMA issuer I, 4 epilogue, 4 per converter group
 constexpr int V2_MAX_UNITS = 128;     // K-steps per tile the per-unit load table covers
@@ -68,6 +73,10 @@ struct K2Params {
     int acc_cols, acc_stages, a_slots, a_col0;
     // ---- staging ring of 32-frame chunks: rows of `hop` samples at a padded pitch
     int rows_per_chunk, pitch_bytes, slot_bytes, stg_slots;
+    int stg_phases;            // ceil(stg_slots / 4): staging barriers are indexed [lane quarter + 4 (tile mod stg_phases)]
+    int vpad;                  // MELT_PAD_REFLECT on this kernel: frames start vpad = n_fft/2 samples before sample t * hop, the
+                               // samples beyond the clip are mirrored by the loader's edge path (0: no padding)
+    int input_ready;           // MELT_OPT_INPUT_READY: x / offsets may be read before the predecessor kernel has completed
     // ---- basis (this CTA's half: nb/2 rows per kind)
     uint32_t unit_b_bytes, kind_bytes;
     uint32_t off_b, off_stg, off_dct, off_bar, smem_bytes;
@@ -86,8 +95,7 @@ struct K2Params {
     const long long *frame_offsets;  // device frame offsets (n_clips + 1), written by the scan kernel
     const int *tile_prefix;          // device exclusive prefix of 256-frame tiles per clip (n_clips + 1)
     // ---- plan-owned device data
-    const uint8_t *b_img;  // [b_replicas][2 ranks][units] slabs of unit_b_bytes
-    int b_replicas;
+    const uint8_t *b_img;  // [2 ranks][passes][units] slabs of unit_b_bytes
     int passes;                // passes over the Mel bins (nb bins each); > 1 needs the streamed basis
     int direct;                // no staging: converter threads read their frames from global memory (very long windows)
     int b_resident, b_slots;   // basis half resident in shared memory (b_slots = units), or streamed through a ring of b_slots K-step slabs
@@ -98,6 +106,9 @@ struct K2Params {
     //      hop-row: stride = hop, clip: stride = len); one box = one 32-frame chunk.  tma_rows = hop-rows per clip whose
     //      whole pitch-wide extent lies inside the clip (chunks reaching beyond take the per-row bulk-copy path); 0 = off.
     int tma_rows;
+#ifdef MELT_TRACE
+    int trace_slot;            // development builds only: region of the event-trace buffer this launch records into
+#endif
     alignas(64) unsigned char tmap[128];
 };
 
@@ -106,8 +117,8 @@ struct K2Params {
 struct melt_plan {
     double fs, fmin, fmax;
     int n_fft, hop, window, n_mels, mel_scale, n_mfcc;
-    int layout, precision, drop_last, pad, in_scale_log2, output;
-    bool used;
+    int layout, precision, drop_last, pad, in_scale_log2, output, input_ready;
+    mutable std::atomic<bool> used;    // set by the first forward call: options are frozen from then on
     int device, sm_count;
     std::vector<double> centres, win;
     melt::KParams kp;  // geometry + plan-owned device pointers (batch fields filled per call)
@@ -118,12 +129,9 @@ struct melt_plan {
     uint8_t *d_bimg;
     uint32_t *d_tab;
     float *d_dct;
-    int *d_tile_prefix;
-    long long *d_frame_offsets_scratch;
-    float *ws_in, *ws_out;             // device workspace of melt_forward_host (grown on demand)
-    float *ws_pad;                     // reflect-padded copy of the signal for the CTA-pair kernel (grown on demand)
-    size_t ws_pad_bytes;
-    size_t ws_in_bytes, ws_out_bytes;
+    cudaMemPool_t pool;                // per-call device scratch (ragged tile index, realigned copies, host-buffer staging):
+                                       // stream-ordered allocations, so forward calls neither synchronise nor touch the plan
+    cudaStream_t copy_in, copy_out;    // melt_forward_host: upload / download streams (ordered against the caller's by events)
     std::string desc;
 };
 
@@ -136,5 +144,5 @@ int launch_forward2(const melt_plan *p, const K2Params &kp, cudaStream_t stream)
 int launch_reflect_pad(const float *x, float *xp, int batch, long long len, int pad, long long plen, cudaStream_t stream);
 int v2_encode_tmap(K2Params &kp);
 int v2_encode_tmap_ragged(K2Params &kp);   // 2-D map over the packed buffer (any start sample, rows of `hop` samples)   // fills kp.tmap / kp.tma_rows for this call's (x, len, batch); never fails the call
-int launch_ragged_scan(const melt_plan *p, const long long *offsets, int n_clips, long long *frame_offsets, int tile_m, cudaStream_t stream);
+int launch_ragged_scan(const melt_plan *p, const long long *offsets, int n_clips, long long *frame_offsets, int *tile_prefix, int tile_m, cudaStream_t stream);
 }  // namespace melt

@@ -4,6 +4,7 @@
 // (A-from-TMEM form) per K-step issued by a single thread, completion through tcgen05.commit -> mbarrier,
 // and the accumulator read back with tcgen05.ld.  Exactly the mechanisms melt_fwd_kernel relies on.
 #include "melt_internal.h"
+#include "../../include/melt_test.h"
 #include "sm100_ptx.cuh"
 
 #include <cuda_bf16.h>

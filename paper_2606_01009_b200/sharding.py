@@ -3,9 +3,12 @@ over the batch with NO data-path collective.  One process per GPU; the basis (a 
 rebuilt per rank.  The only communication is bookkeeping around the timed region: a barrier, and a MAX / SUM
 reduction of the timing and the frame counts (NCCL on GPUs, gloo in the CPU tests).
 
-No method arithmetic lives here: frame counting is the integer formula of include/melt.h (melt_num_frames).
+No method arithmetic lives here: frames are counted by the library itself (melt_count_frames of include/melt.h, host-only
+integer arithmetic that needs no GPU).
 """
 import numpy as np
+
+from . import binding as _mb
 
 
 def rank_seed(base_seed, rank):
@@ -14,16 +17,8 @@ def rank_seed(base_seed, rank):
 
 
 def frames_of(length, n_fft, hop, pad_reflect=False, drop_last=False):
-    """Integer frame count of one clip (same formula as melt_num_frames)."""
-    length = int(length)
-    padded = length
-    if pad_reflect:
-        if length < n_fft // 2 + 1:
-            return 0
-        padded += 2 * (n_fft // 2)
-    if padded < n_fft:
-        return 0
-    return max(0, (padded - n_fft) // hop + 1 - (1 if drop_last else 0))
+    """Frame count of one clip: the library's own melt_count_frames (one copy of the formula)."""
+    return _mb.melt_count_frames(length, n_fft, hop, _mb.MELT_PAD_REFLECT if pad_reflect else _mb.MELT_PAD_NONE, drop_last)
 
 
 def partition_dense(n_clips, world):
