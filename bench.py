@@ -160,6 +160,210 @@ def torch_context(cfg, c, x_dev, steps=20):
     return out
 
 
+def make_plan(mb, c, precision, input_ready=True):
+    plan = mb.melt_plan_create(*wl.plan_args(c))
+    mb.melt_plan_set_option(plan, mb.MELT_OPT_PRECISION, PREC_NAMES[precision])
+    mb.melt_plan_set_option(plan, mb.MELT_OPT_DROP_LAST, int(c["drop_last"]))
+    mb.melt_plan_set_option(plan, mb.MELT_OPT_LAYOUT, int(c["layout"] == "feature_major"))
+    # the inputs are resident in HBM long before the timed region: consecutive forwards may read x while the previous kernel
+    # drains (MELT_OPT_INPUT_READY, include/melt.h); input_ready=False is the library's default, fully ordered form
+    mb.melt_plan_set_option(plan, mb.MELT_OPT_INPUT_READY, int(bool(input_ready)))
+    return plan
+
+
+def time_back_to_back(torch, step, steps, first=0):
+    """K forwards back to back on the current stream, ONE event on each side (ms per step)."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for i in range(steps):
+        step(first + i)
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / steps
+
+
+def time_isolated(torch, step, n):
+    """Every launch bracketed by its own events: durations (ms) of launches that cannot overlap their neighbours."""
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(n + 1)]
+    torch.cuda.synchronize()
+    evs[0].record()
+    for i in range(n):
+        step(i)
+        evs[i + 1].record()
+    torch.cuda.synchronize()
+    return [evs[i].elapsed_time(evs[i + 1]) for i in range(n)]
+
+
+def measure_tf32_peak(torch, n=8192, reps=10):
+    """cuBLAS TF32 GEMM n^3 through torch.matmul (allow_tf32), best of `reps` (burst figure, like MEASURED_PEAKS.json's bf16)."""
+    old = torch.backends.cuda.matmul.allow_tf32
+    torch.backends.cuda.matmul.allow_tf32 = True
+    try:
+        a = torch.randn((n, n), device="cuda")
+        b = torch.randn((n, n), device="cuda")
+        for _ in range(2):
+            a @ b
+        best = 1e9
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            a @ b
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        del a, b
+        torch.cuda.empty_cache()
+        return 2.0 * n ** 3 / (best * 1e-3) / 1e12
+    finally:
+        torch.backends.cuda.matmul.allow_tf32 = old
+
+
+def roofline_of(nums, ms, peaks, dtype, tf32_tflops):
+    """bound / achieved / peak / frac of one step of `ms` milliseconds."""
+    tensor_peak = tf32_tflops if dtype == "tf32" else peaks["bf16_tflops"]
+    nbytes = nums["bytes_in"] + nums["bytes_out"]
+    t_hbm = nbytes / (peaks["hbm_gbs"] * 1e9)
+    t_tensor = nums["flops"] / (tensor_peak * 1e12)
+    if t_hbm >= t_tensor:
+        ach = nbytes / (ms * 1e-3) / 1e9
+        r = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
+    else:
+        ach = nums["flops"] / (ms * 1e-3) / 1e12
+        r = {"bound": "tensor", "achieved": ach, "peak": tensor_peak, "unit": "TFLOP/s"}
+    r["frac"] = r["achieved"] / r["peak"]
+    r["t_hbm_us"], r["t_tensor_us"] = t_hbm * 1e6, t_tensor * 1e6
+    return r
+
+
+PER_WORKLOAD = [("cfg0", "compensated"), ("cfg2", "compensated"), ("cfg2", "tf32"), ("cfg2", "bf16"), ("cfg3", "compensated"),
+                ("cfg4a", "compensated"), ("cfg4a", "tf32"), ("cfg4a", "bf16"), ("cfg4b", "compensated"), ("cfg4c", "compensated"),
+                ("cfg4d", "compensated"), ("cfg4d", "tf32"), ("cfg4d", "bf16")]
+
+
+def bench_other_workloads(torch, mb, peaks, tf32_tflops, launches=20):
+    """Every other config of BASELINE.json under the same clock: `launches` back-to-back forwards (after 3 warm-ups) and the
+    median of 10 isolated ones.  Shapes, lengths and options are the configs'; the sample VALUES are device-side Gaussian noise
+    (timing does not depend on them; parity at these sizes is tests/test_parity_gpu.py's job).  Buffers are larger than L2 or
+    rotated so that HBM is measured."""
+    out = []
+    l2 = torch.cuda.get_device_properties(0).L2_cache_size
+    stream = torch.cuda.current_stream()
+    cache = {}
+    for cfg, prec in PER_WORKLOAD:
+        c = wl.CONFIGS[cfg]
+        ragged = bool(c.get("ragged"))
+        plan = make_plan(mb, c, prec)
+        try:
+            C = mb.melt_num_channels(plan)
+            N, H, M, K = c["n_fft"], c["hop"], c["n_mels"], c["n_mfcc"]
+            if ragged:
+                rng = np.random.default_rng(c["seed"])   # same length law as workloads.speaker_ragged
+                lens = rng.integers(c["min_len"], c["max_len"] + 1, size=c["n_clips"]).astype(np.int64)
+                offs = np.zeros(c["n_clips"] + 1, np.int64)
+                offs[1:] = np.cumsum(lens)
+                frames = int(sum(mb.melt_count_frames(int(v), N, H) for v in lens))
+                B, L, n_in = c["n_clips"], 0, int(offs[-1])
+                off_dev = torch.from_numpy(offs).cuda()
+                audio_s = float(lens.sum()) / c["fs"]
+                out_shape = (frames, C)
+            else:
+                B = c["n_clips"]
+                L = c["clip_len"] + (2 * (N // 2) if c["pad_reflect"] else 0)
+                T = mb.melt_num_frames(plan, L)
+                frames, n_in, audio_s = B * T, B * L, B * c["clip_len"] / c["fs"]
+                out_shape = (B, C, T) if c["layout"] == "feature_major" else (B, T, C)
+            nums = dict(frames=frames, flops=2.0 * frames * 2 * M * N + 2.0 * frames * M * K,
+                        bytes_in=4.0 * (n_in if ragged else B * c["clip_len"]), bytes_out=4.0 * frames * C)
+            set_bytes = 4 * n_in + 4 * frames * C
+            nsets = max(1, int(np.ceil(2.2 * l2 / set_bytes)))
+            key = (cfg, nsets)
+            if key not in cache:
+                cache.clear()
+                torch.cuda.empty_cache()
+                cache[key] = ([0.1 * torch.randn(n_in, device="cuda") for _ in range(nsets)],
+                              [torch.empty(out_shape, device="cuda") for _ in range(nsets)])
+            xs, outs = cache[key]
+            fo = torch.empty(B + 1, dtype=torch.int64, device="cuda") if ragged else None
+
+            def step(i, plan=plan, xs=xs, outs=outs, fo=fo):
+                if ragged:
+                    mb.melt_forward_ragged(plan, xs[i % nsets], off_dev, B, outs[i % nsets], fo, stream.cuda_stream)
+                else:
+                    mb.melt_forward(plan, xs[i % nsets], B, L, outs[i % nsets], stream.cuda_stream)
+
+            for i in range(3):
+                step(i)
+            ms = time_back_to_back(torch, step, launches)
+            iso = time_isolated(torch, step, 10)
+            dtype = PREC_DTYPE[prec]
+            roof = roofline_of(nums, ms, peaks, dtype, tf32_tflops)
+            row = {"workload": cfg, "precision": prec, "us_per_step": 1e3 * ms, "us_isolated_median": 1e3 * statistics.median(iso),
+                   "frames_per_step": frames, "frames_per_s": frames / (ms * 1e-3), "audio_s_per_s": audio_s / (ms * 1e-3),
+                   "bound": roof["bound"], "frac": roof["frac"], "frac_isolated": roof["frac"] * ms / statistics.median(iso),
+                   "t_hbm_us": roof["t_hbm_us"], "t_tensor_us": roof["t_tensor_us"], "launches": launches,
+                   "gpu_launches_per_step": 2 if ragged else 1,
+                   "kernel": mb.melt_plan_describe(plan).split(" | ")[0]}
+            if cfg == "cfg0":
+                # latency-bound single clip: also one forward captured in a CUDA graph and replayed (launch cost amortised)
+                g = torch.cuda.CUDAGraph()
+                side = torch.cuda.Stream()
+                side.wait_stream(torch.cuda.current_stream())
+                with torch.cuda.stream(side):
+                    mb.melt_forward(plan, xs[0], B, L, outs[0], side.cuda_stream)
+                    side.synchronize()
+                    with torch.cuda.graph(g, stream=side):
+                        mb.melt_forward(plan, xs[0], B, L, outs[0], side.cuda_stream)
+                    for _ in range(5):
+                        g.replay()
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record()
+                    for _ in range(200):
+                        g.replay()
+                    e1.record()
+                    side.synchronize()
+                    row["us_cuda_graph_replay"] = 1e3 * e0.elapsed_time(e1) / 200
+                row["note"] = "launch-latency bound: no roofline claim; us_isolated_median is the latency of one call"
+            out.append(row)
+        finally:
+            torch.cuda.synchronize()
+            mb.melt_plan_destroy(plan)
+    cache.clear()
+    torch.cuda.empty_cache()
+    return out
+
+
+def measure_energy(torch, step, ms_per_step, seconds=3.0):
+    """Energy per call with the NVML total-energy counter (section IV-B: a window of >= 30 counter quanta):
+    the counter is read around `seconds` of back-to-back forwards (>= 30 updates of a ~100 ms counter at 3 s) and around an
+    idle window of the same length; active energy = total - idle power x time."""
+    try:
+        import pynvml
+        pynvml.nvmlInit()
+        h = pynvml.nvmlDeviceGetHandleByIndex(torch.cuda.current_device())
+        read = lambda: pynvml.nvmlDeviceGetTotalEnergyConsumption(h)   # millijoules since driver load
+        torch.cuda.synchronize()
+        time.sleep(0.5)
+        e0, t0 = read(), time.perf_counter()
+        time.sleep(seconds)
+        e1, t1 = read(), time.perf_counter()
+        idle_w = (e1 - e0) * 1e-3 / (t1 - t0)
+        n = max(100, int(seconds / (ms_per_step * 1e-3)))
+        torch.cuda.synchronize()
+        e0, t0 = read(), time.perf_counter()
+        for i in range(n):
+            step(i)
+        torch.cuda.synchronize()
+        e1, t1 = read(), time.perf_counter()
+        tot_mj = float(e1 - e0)
+        dt = t1 - t0
+        return {"calls": n, "window_s": dt, "mj_per_call_total": tot_mj / n, "mj_per_call_active": (tot_mj - idle_w * dt * 1e3) / n,
+                "avg_power_w": tot_mj * 1e-3 / dt, "idle_power_w": idle_w,
+                "method": "nvmlDeviceGetTotalEnergyConsumption around %d back-to-back calls (%.1f s) minus idle power x time" % (n, dt)}
+    except Exception as e:  # noqa: BLE001
+        return {"unavailable": str(e)[:120]}
+
+
 def time_oracle(cfg, n_clips_sample, reps):
     """The fp64 oracle as it stands on the host cores, on a bounded sample of the workload (frames/s)."""
     from oracle import melt_oracle as orc
@@ -220,8 +424,12 @@ def main():
     ap.add_argument("--cpu-clips", type=int, default=8, help="clips in the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-context", action="store_true", help="skip the same-box torch.stft / unfold-matmul context timings")
+    ap.add_argument("--no-per-workload", action="store_true", help="skip the short pass over the other configs")
+    ap.add_argument("--no-energy", action="store_true", help="skip the NVML energy-per-call window")
+    ap.add_argument("--sustained-steps", type=int, default=3000, help="launches of the sustained-rate pass (0 = skip)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "cuda":
+        print("bench.py: --warmup %d raised to 3 (timing rule: at least 3 warm-up steps)" % args.warmup, file=sys.stderr)
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
@@ -249,12 +457,7 @@ def main():
     peaks = load_peaks()
 
     # ---- plan
-    plan = mb.melt_plan_create(*wl.plan_args(c))
-    mb.melt_plan_set_option(plan, mb.MELT_OPT_PRECISION, PREC_NAMES[args.precision])
-    mb.melt_plan_set_option(plan, mb.MELT_OPT_DROP_LAST, int(c["drop_last"]))
-    mb.melt_plan_set_option(plan, mb.MELT_OPT_LAYOUT, int(c["layout"] == "feature_major"))
-    # the inputs are resident in HBM long before the timed region: consecutive forwards may read x while the previous kernel drains
-    mb.melt_plan_set_option(plan, mb.MELT_OPT_INPUT_READY, 1)
+    plan = make_plan(mb, c, args.precision, input_ready=True)
     desc = mb.melt_plan_describe(plan)
 
     # ---- inputs: same per-clip streams on every rank but rank-shifted seed (weak scaling: every rank owns a full batch)
@@ -329,6 +532,23 @@ def main():
         evs[i + 1].record()
     barrier()
     per_ms = [evs[i].elapsed_time(evs[i + 1]) for i in range(iso_n)]
+    # Third pass: the sustained rate (>= 50 ms of back-to-back launches), the step-count curve that shows how much of the
+    # headline is launch overlap (1 launch = isolated ... 1000 = steady state), and the library's default, fully ordered form
+    # (MELT_OPT_INPUT_READY = 0: no read of x before the previous kernel has completed).
+    sustained_ms = time_back_to_back(torch, step, args.sustained_steps) if args.sustained_steps > 0 else None
+    overlap_curve = {str(k): 1e3 * min(time_back_to_back(torch, step, k) for _ in range(3 if k >= 200 else 10))
+                     for k in (1, 2, 5, 20, 200, 1000)} if rank == 0 else None
+    plan_ord = make_plan(mb, c, args.precision, input_ready=False)
+
+    def step_ord(i):
+        if ragged:
+            mb.melt_forward_ragged(plan_ord, xs[i % nsets], off_dev, B, outs[i % nsets], fo, stream.cuda_stream)
+        else:
+            mb.melt_forward(plan_ord, xs[i % nsets], B, L, outs[i % nsets], stream.cuda_stream)
+    for i in range(10):
+        step_ord(i)
+    ordered_ms = time_back_to_back(torch, step_ord, min(args.steps, 1000))
+    mb.melt_plan_destroy(plan_ord)
     if dist is not None:
         t = torch.tensor([total_ms], device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -376,30 +596,40 @@ def main():
     kernel_ms = ms_per_step                      # one launch per step: average launch duration over the timed region
     kernel_ms_median = statistics.median(per_ms)  # isolated launches (second pass, an event between every two launches)
     dtype = PREC_DTYPE[args.precision]
-    tensor_peak = peaks["bf16_tflops"] * (0.5 if dtype == "tf32" else 1.0)      # burst: the kernel is timed alone
-    t_hbm = (nums["bytes_in"] + nums["bytes_out"]) / (peaks["hbm_gbs"] * 1e9)
-    t_tensor = nums["flops"] / (tensor_peak * 1e12)
-    if t_hbm >= t_tensor:
-        achieved = (nums["bytes_in"] + nums["bytes_out"]) / (kernel_ms * 1e-3) / 1e9
-        roof = {"bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
-    else:
-        achieved = nums["flops"] / (kernel_ms * 1e-3) / 1e12
-        roof = {"bound": "tensor", "achieved": achieved, "peak": tensor_peak, "unit": "TFLOP/s"}
-    roof["frac"] = roof["achieved"] / roof["peak"]
+    tf32_tflops = measure_tf32_peak(torch)       # cuBLAS TF32 on this GPU, this run (MEASURED_PEAKS.json has bf16 only)
+    roof = roofline_of(nums, kernel_ms, peaks, dtype, tf32_tflops)
+    t_ref = max(roof["t_hbm_us"], roof["t_tensor_us"]) * 1e-3          # roofline time of one step, ms
     roof["traffic"] = None
     roof.update({"peaks": peaks["_source"], "kernel_ms": kernel_ms, "kernel_ms_median": kernel_ms_median,
-                 "kernel_ms_isolated_mean": statistics.mean(per_ms), "kernel_ms_min": min(per_ms), "t_hbm_us": t_hbm * 1e6, "t_tensor_us": t_tensor * 1e6,
-                 "tensor_peak_dtype": dtype, "algorithmic_bytes": nums["bytes_in"] + nums["bytes_out"],
-                 "algorithmic_flops": nums["flops"],
-                 "frac_vs_tf32_roofline": max(t_hbm, nums["flops"] / (peaks["bf16_tflops"] * 0.5e12)) / (kernel_ms * 1e-3)})
+                 "kernel_ms_isolated_mean": statistics.mean(per_ms), "kernel_ms_min": min(per_ms),
+                 "frac_isolated": t_ref / kernel_ms_median,
+                 "frac_sustained": (t_ref / sustained_ms) if sustained_ms else None,
+                 "sustained": {"launches": args.sustained_steps, "ms_per_step": sustained_ms},
+                 "frac_ordered": t_ref / ordered_ms,
+                 "ordered": {"ms_per_step": ordered_ms, "note": "MELT_OPT_INPUT_READY=0, the library default: no read of x before the "
+                             "previous kernel in the stream has completed (only set-up overlaps)"},
+                 "overlap_curve_us_per_step": overlap_curve,
+                 "tensor_peak_dtype": dtype, "tf32_tflops_measured": tf32_tflops,
+                 "algorithmic_bytes": nums["bytes_in"] + nums["bytes_out"], "algorithmic_flops": nums["flops"],
+                 "frac_vs_tf32_roofline": max(roof["t_hbm_us"] * 1e-6, nums["flops"] / (tf32_tflops * 1e12)) / (kernel_ms * 1e-3)})
     prof = os.path.join(ROOT, "profiles", "traffic_%s_%s.json" % (cfg, args.precision))
     if os.path.exists(prof):
         with open(prof) as fh:
             roof["traffic"] = json.load(fh).get("dram_bytes_per_launch")
+        roof["traffic_source"] = "constant from profiles/%s (one ncu --set full capture of this kernel), not measured in this run" % os.path.basename(prof)
 
+    energy = None
+    if not args.no_energy:
+        energy = measure_energy(torch, step, ms_per_step)
     context = None
     if not ragged and not args.no_context:
         context = torch_context(cfg, c, xs[0])
+    per_workload = None
+    if not args.no_per_workload and world == 1:
+        xs.clear()
+        outs.clear()
+        torch.cuda.empty_cache()
+        per_workload = bench_other_workloads(torch, mb, peaks, tf32_tflops)
     cpu = None
     if not args.no_cpu_baseline:
         fps, dt, cores, frames = time_oracle(cfg, args.cpu_clips, 1)      # calibration pass (also warms the OpenMP pool)
@@ -418,12 +648,16 @@ def main():
                    "precision": args.precision, "parallelism": "dp%d (independent shards, no collective)" % world,
                    "l2_policy": "rotating %d input/output buffer sets, %.0f MB total > 2x L2 (%.0f MB)" % (
                        nsets, nsets * set_bytes / 1e6, l2_bytes / 1e6),
+                   "input_ready": "MELT_OPT_INPUT_READY=1 (inputs resident before the timed region; consecutive forwards overlap); "
+                                  "roofline.ordered has the default form",
                    "kernel": desc},
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "frames/s", "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(x_pin.numel() * 4),
                 "d2h_bytes_per_step": int(out_pin.numel() * 4)},
         "gpu_launches": args.steps * (2 if ragged else 1),   # ragged: frame-offset scan + forward kernel
         "roofline": roof,
+        "per_workload": per_workload,
+        "energy": energy,
         "cpu_baseline": cpu,
         "context": context,
     }
