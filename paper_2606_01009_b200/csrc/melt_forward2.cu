@@ -43,7 +43,8 @@ int plan_build_v2(melt_plan *p) {
     const int pitch_words = ((H / 4) & 1) ? H : H + 4;   // pitch / 4 odd: 8 consecutive rows hit 8 distinct 16-byte bank groups
     // hop-rows a 32-frame chunk touches; one more when the rows carry no padding words: a ragged chunk is fetched from up to
     // three samples below its start and shifted down, which needs those samples at the end of the last row
-    k.rows_per_chunk = 32 + (N - 1) / H + (pitch_words == H ? 1 : 0);
+    // (+3 samples: in a ragged batch a chunk sits up to three words further into its rows, see load_shifted in the kernel)
+    k.rows_per_chunk = 32 + (N - 1 + 3) / H + (pitch_words == H ? 1 : 0);
     if (k.rows_per_chunk > 64) return MELT_OK;
     k.pitch_bytes = pitch_words * 4;
     k.slot_bytes = round_up2(k.rows_per_chunk * k.pitch_bytes, 128);   // tensor-map boxes land on 128-byte boundaries
@@ -55,7 +56,7 @@ int plan_build_v2(melt_plan *p) {
     // MFCCT, frame-major: 4 epilogue warps x 32 frames x n_mfcc floats behind the DCT table (cepstra transposed for coalesced stores)
     const uint32_t epi_bytes = (p->n_mfcc > 0 && p->layout == MELT_LAYOUT_FRAME_MAJOR) ? (uint32_t)(4 * 32 * p->n_mfcc * 4) : 0;
     const uint32_t dct_bytes = dct_only + epi_bytes;
-    const uint32_t bar_bytes = (uint32_t)round_up2(V_NBARS * 8 + 16, 128);
+    const uint32_t bar_bytes = (uint32_t)round_up2(V_NBARS * 8 + 16 + 32 * 16, 128);   // barriers, tensor-memory address, chunk records of ragged batches (32 x 16 B)
     k.off_b = 0;
     // The basis half stays resident when that leaves room for at least five staging slots; otherwise (long windows) its
     // K-step slabs are streamed from L2 through the deepest ring (<= 8 slabs) that still leaves five slots.
@@ -98,6 +99,8 @@ int plan_build_v2(melt_plan *p) {
         const int run = k1.b0 - k.kstep * u - (k.kstep - 1);   // lowest sample of the mirrored run
         for (int i = 0; i < nq; ++i) k.tab[u][4 + i] = (short)off_of(run - sigma + 4 * i);
         k.tab[u][8] = (short)off_of(run + k.kstep - 1);
+        k.tab[u][9] = (short)off_of(k1.a0 + k.kstep * u + k.kstep);     // the quads after the two runs (ragged batches: shifted chunks)
+        k.tab[u][10] = (short)off_of(run - sigma + k.kstep);
         for (int i = 0; i < V2_TAB; ++i)
             if (k.direct) {   // every read must stay inside the frame: [0, N) samples
                 const bool quad = i < nq || (i >= 4 && i < 4 + nq), single = i == 8 && sigma == 1;

@@ -38,7 +38,7 @@ enum { P2_COMP = 0, P2_TF32 = 1, P2_BF16 = 2 };
 // barrier indices (8 bytes each)
 enum {
     V_STG_FULL = 0, V_STG_EMPTY = V2_MAX_STG, V_A_FULL = 2 * V2_MAX_STG, V_A_EMPTY = V_A_FULL + 16, V_ACC_FULL = V_A_EMPTY + 16,
-    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_DONE = V_B_PEER + V2_MAX_UNITS, V_STG_READY = V_DONE + 1, V_B_EMPTY = V_STG_READY + V2_MAX_STG, V_NBARS = V_B_EMPTY + 8
+    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_DONE = V_B_PEER + V2_MAX_UNITS, V_STG_READY = V_DONE + 1, V_B_EMPTY = V_STG_READY + V2_MAX_STG, V_INFO = V_B_EMPTY + 8, V_NBARS = V_INFO + 32
 };
 constexpr int V2_MAX_A_SLOTS = 16;
 constexpr int W_LOAD = 0, W_MMA = 1, W_BASIS = 2, W_MMA2 = 3, W_EPI0 = 4, W_CONV0 = 8;
@@ -215,57 +215,55 @@ struct Tile2 {
     long long f0;      // index of the clip's first frame in the (packed or dense) frame order
     int pass;          // pass over the Mel bins (more than 128 bins: every tile is visited once per pass)
 };
+// Dense batches: a tile is 256 consecutive frames of one clip, found by division.  Ragged batches: the clips are cut into
+// 32-frame CHUNKS (the unit one converter / epilogue warp works on) and a tile is any 8 consecutive chunks of the packed
+// chunk order -- the four lane quarters of a CTA may belong to different clips, so the tail of a clip wastes at most 31 rows
+// instead of up to 255.  Only the loader looks chunks up (chunk_prefix, written by the scan kernel, is the exclusive prefix
+// of chunks per clip); it hands what the other warps need to them in shared memory (ChunkInfo).
+struct ChunkInfo {
+    long long row0;   // index of the chunk's first frame in the packed output
+    int nvalid;       // frames of the chunk that exist (0 .. 32)
+    int dlt;          // words by which the staged chunk sits further into its rows than the load table says (clip offset & 3)
+};
 template <bool RAGGED>
 __device__ __forceinline__ void get_tile2(const K2Params &p, int vtile, Tile2 &ti) {
+    static_assert(!RAGGED, "ragged batches: the loader tracks the clip of every chunk itself");
     int tile = vtile;
     ti.pass = 0;
     if (p.passes > 1) { tile = vtile / p.passes; ti.pass = vtile - tile * p.passes; }
-    if (!RAGGED) {
-        const int b = tile / p.tiles_per_clip;
-        ti.clip = b;
-        ti.t0 = (tile - b * p.tiles_per_clip) * 256;
-        ti.T = p.frames_per_clip;
-        ti.s0 = (long long)b * p.len;
-        ti.f0 = (long long)b * p.frames_per_clip;
-    } else {
-        int lo = 0, hi = p.n_clips;   // largest i with tile_prefix[i] <= tile
-        while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if (__ldg(p.tile_prefix + mid) <= tile) lo = mid; else hi = mid;
-        }
-        ti.clip = lo;
-        ti.t0 = (tile - __ldg(p.tile_prefix + lo)) * 256;
-        ti.f0 = p.frame_offsets[lo];
-        ti.T = p.frame_offsets[lo + 1] - ti.f0;
-        ti.s0 = __ldg(p.offsets + lo);
-    }
+    const int b = tile / p.tiles_per_clip;
+    ti.clip = b;
+    ti.t0 = (tile - b * p.tiles_per_clip) * 256;
+    ti.T = p.frames_per_clip;
+    ti.s0 = (long long)b * p.len;
+    ti.f0 = (long long)b * p.frames_per_clip;
 }
 
-// Ragged batches: shifts a staged chunk down by (clip offset & 3) words (see the loader).  Out of line on purpose: it runs
-// once per chunk on ragged batches only and must not take registers from the converter loop it is called from.
-static __device__ __noinline__ void ragged_realign(const long long *offsets, const int *tile_prefix, int n_clips, int tile, float *w,
-                                            int n_words, int lane) {
-    int lo = 0, hi = n_clips;   // largest i with tile_prefix[i] <= tile
-    while (hi - lo > 1) {
-        const int mid = (lo + hi) >> 1;
-        if (__ldg(tile_prefix + mid) <= tile) lo = mid; else hi = mid;
-    }
-    const int dlt = (int)(__ldg(offsets + lo) & 3);
-    if (dlt) {
-        const int n = n_words - dlt;
-        for (int base = 0; base < n; base += 128) {   // warp-uniform trip count: the loop body synchronises the warp
-            const int i = base + lane;
-            float v[4];
+// Ragged batches: a clip starts at any sample of the packed buffer, but the copy engines want 16-byte aligned sources, so a
+// chunk is fetched from the aligned sample below its start: frame sample n then sits dlt = (clip offset & 3) words further
+// into the staged rows than the load table says.  The converter reads the aligned quads around it (one more per direction)
+// and picks its 2 KS samples with offsets that are compile-time constants of the instantiation <DLT>: no pass over the chunk
+// in shared memory (an earlier version shifted every chunk down by dlt words first: ~2600 cycles per tile).
+//   forward run  : table quads tb[0 .. NQ) (samples n0 + 4 i ..) and the quad after them, tb[9]
+//   mirrored run : table quads tb[4 .. 4 + NQ) (samples run - SIGMA + 4 i ..) and the quad after them, tb[10]
+// Rows overlap by their padding words (a staged row is hop + 4 samples of the signal), so the words after a quad that ends a
+// row are the first samples of the next row: reading dlt words past a table quad never leaves the signal.
+template <int KS, int SIGMA, int DLT>
+__device__ __forceinline__ void load_shifted(uint32_t fb, const short *tb, float (&fw)[KS], float (&bw)[KS]) {
+    constexpr int NQ = KS / 4, BS = SIGMA + DLT;
+    float wf[KS + 4], wb[KS + 4];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) v[j] = (i + 32 * j < n) ? w[i + 32 * j + dlt] : 0.f;
-            __syncwarp();   // every lane has read before any lane overwrites (lane l writes what lane l - dlt read)
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-                if (i + 32 * j < n) w[i + 32 * j] = v[j];
-            __syncwarp();
-        }
+    for (int i = 0; i <= NQ; ++i) {
+        const float4 f = lds128(fb + (uint32_t)(int)tb[i < NQ ? i : 9]);
+        wf[4 * i + 0] = f.x; wf[4 * i + 1] = f.y; wf[4 * i + 2] = f.z; wf[4 * i + 3] = f.w;
+        const float4 g = lds128(fb + (uint32_t)(int)tb[i < NQ ? 4 + i : 10]);
+        wb[4 * i + 0] = g.x; wb[4 * i + 1] = g.y; wb[4 * i + 2] = g.z; wb[4 * i + 3] = g.w;
     }
-    __syncwarp();
+#pragma unroll
+    for (int e = 0; e < KS; ++e) {
+        fw[e] = wf[e + DLT];
+        bw[KS - 1 - e] = wb[BS + e];   // sample `run + e` of the descending run is the partner of pair KS - 1 - e
+    }
 }
 
 static_assert(V_NBARS <= V2_THREADS, "one thread per barrier at set-up");
@@ -287,6 +285,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     const uint32_t bar0 = sbase + p.off_bar;
     auto BAR = [&](int idx) -> uint32_t { return bar0 + (uint32_t)idx * 8u; };
     uint32_t *tmem_ptr_s = reinterpret_cast<uint32_t *>(smem + p.off_bar + V_NBARS * 8);
+    // ragged batches: what the loader found out about each chunk (a ring over the last 8 tiles x 4 lane quarters, entry
+    // [q + 4 (tl & 7)] for the chunk of quarter q of this CTA's tl-th tile): the converter warps need its misalignment, whoever
+    // drains the accumulators its first output row and its number of valid frames -- nobody else has to search the clip table
+    ChunkInfo *chunk_info = reinterpret_cast<ChunkInfo *>(smem + p.off_bar + V_NBARS * 8 + 16);
     float *dct_s = reinterpret_cast<float *>(smem + p.off_dct);
 
     const int tid = threadIdx.x, lane = tid & 31;
@@ -326,6 +328,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             mbar_init(BAR(V_STG_EMPTY + lane), (uint32_t)NG);
             mbar_init(BAR(V_STG_READY + lane), 1u);
         }
+        mbar_init(BAR(V_INFO + lane), 1u);   // 32 = 8 tile phases x 4 lane quarters: chunk info published (ragged batches)
         fence_barrier_init();
     } else if (warp == W_MMA || warp == W_MMA2) {
         const int n_b = STREAM ? 8 : (p.units < V2_MAX_UNITS ? p.units : V2_MAX_UNITS);   // basis barriers in use
@@ -369,7 +372,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     // and its writes to be visible; otherwise the wait is taken just before the first global store (dep_done below).
     if (!p.input_ready) asm volatile("griddepcontrol.wait;" ::: "memory");
     const int first_tile = (int)cluster_id_x(), tile_step = (int)cluster_nid_x();
-    const int n_tiles = (RAGGED ? p.tile_prefix[p.n_clips] : p.n_tiles) * p.passes;   // ragged: counted by the scan kernel; one visit per pass over the bins
+    const int n_tiles = (RAGGED ? (p.tile_prefix[p.n_clips] + 7) / 8 : p.n_tiles) * p.passes;   // ragged: 8 chunks per tile, counted by the scan kernel; one visit per pass over the bins
     TRACE_DECL
     TRACE(1);
     if (warp == W_LOAD && DIRECT) {
@@ -395,15 +398,50 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         if (p.tma_rows > 0 && lane == 0) tma_prefetch_desc(p.tmap);
         constexpr bool ragged = RAGGED;
         const long long total = ragged ? p.offsets[p.n_clips] : 0;   // samples in the packed buffer
+        // ragged: the clip the last chunk belonged to.  Chunk indices only grow, so the next clip is found by probing the 32
+        // prefix entries after the current one at once (one load latency; a tile step is ~25 clips on the speaker-style batch)
+        const int total_chunks = ragged ? p.tile_prefix[p.n_clips] : 0;
+        int rg_clip = 0, rg_lo = 0, rg_hi = ragged ? p.tile_prefix[1] : 0;
+        long long rg_f0 = 0, rg_T = 0, rg_s0 = 0, rg_len = 0;
+        bool rg_have = false;
+        int tl = 0;   // tiles of this CTA so far
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
-            Tile2 ti;
-            get_tile2<RAGGED>(p, tile, ti);
-            const int b = ti.clip;
-            const int t0 = ti.t0 + (int)rank * 128;
-            const float *xb = p.x + ti.s0;
-            const long long clip_len = ragged ? p.offsets[b + 1] - ti.s0 : len;
             for (int q = 0; q < 4; ++q) {
-                const long long row0 = (long long)(t0 + 32 * q);
+                Tile2 ti;
+                long long row0;
+                if constexpr (!ragged) {
+                    get_tile2<false>(p, tile, ti);
+                    row0 = (long long)(ti.t0 + (int)rank * 128 + 32 * q);
+                } else {
+                    const int g = (p.passes > 1 ? tile / p.passes : tile) * 8 + (int)rank * 4 + q;   // chunk index in the packed chunk order
+                    ti.pass = 0;
+                    if (g >= total_chunks) {          // beyond the last chunk: no frames
+                        ti.clip = 0; ti.T = 0; ti.s0 = 0; ti.f0 = 0;
+                        row0 = 0;
+                    } else {
+                        while (g >= rg_hi) {          // warp-uniform: the largest clip whose first chunk is <= g
+                            const int idx = rg_clip + 1 + lane;
+                            const int v = idx <= p.n_clips ? __ldg(p.tile_prefix + idx) : 0x7fffffff;
+                            const int cnt = __popc(__ballot_sync(0xffffffffu, v <= g));
+                            if (cnt == 32) { rg_clip += 32; rg_lo = __shfl_sync(0xffffffffu, v, 31); continue; }
+                            if (cnt > 0) { rg_lo = __shfl_sync(0xffffffffu, v, cnt - 1); rg_clip += cnt; }
+                            rg_hi = __shfl_sync(0xffffffffu, v, cnt);
+                            rg_have = false;
+                        }
+                        if (!rg_have) {
+                            rg_f0 = p.frame_offsets[rg_clip];
+                            rg_T = p.frame_offsets[rg_clip + 1] - rg_f0;
+                            rg_s0 = __ldg(p.offsets + rg_clip);
+                            rg_len = __ldg(p.offsets + rg_clip + 1) - rg_s0;
+                            rg_have = true;
+                        }
+                        ti.clip = rg_clip; ti.T = rg_T; ti.s0 = rg_s0; ti.f0 = rg_f0;
+                        row0 = (long long)(g - rg_lo) * 32;
+                    }
+                }
+                const int b = ti.clip;
+                const float *xb = p.x + ti.s0;
+                const long long clip_len = ragged ? rg_len : len;
                 const int n_rows = row0 < ti.T ? p.rows_per_chunk : 0;
                 long long avail = clip_len - row0 * p.hop;                 // samples of the clip from the chunk's first row on
                 avail = avail < 0 ? 0 : avail;
@@ -449,6 +487,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     if (++eq == 4) { eq = 0; if (++etp == P) { etp = 0; eph ^= 1u; } }
                 }
                 const uint32_t full = BAR(V_STG_FULL + cq + 4 * ctp);
+                // ragged: the chunk's misalignment travels with it (read by the converters after their wait on `full`; the
+                // thread that writes it is the one that arrives on `full`, so the arrival publishes it)
+                ChunkInfo *const info = chunk_info + q + 4 * (tl & 7);
+                ChunkInfo info_v;
+                info_v.row0 = ti.f0 + row0;
+                info_v.nvalid = (int)(ti.T - row0 <= 0 ? 0 : (ti.T - row0 < 32 ? ti.T - row0 : 32));
+                info_v.dlt = (int)(ti.s0 & 3ll);
+                const uint32_t info_bar = BAR(V_INFO + q + 4 * (tl & 7));   // for the epilogue warps, which wait on nothing else the loader signals
                 TRACE(11);
                 if (p.vpad > 0 && !by_tma && n_rows > 0) {
                     // Edge chunk of a reflect-padded clip (its first chunk and its last one or two): hop-rows that lie inside the
@@ -473,6 +519,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     }
                     __syncwarp();   // every lane's stores precede lane 0's arrival below
                     if (elect_one()) {
+                        if (ragged) { *info = info_v; mbar_arrive(info_bar); }
                         if (bulk_bytes) mbar_arrive_expect_tx(full, bulk_bytes);
                         else mbar_arrive(full);
                         for (int r = 0; r < n_rows; ++r) {
@@ -499,7 +546,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                         dstp[idx] = g < total ? __ldg(p.x + g) : 0.f;
                     }
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(full);
+                    if (lane == 0) { *info = info_v; mbar_arrive(info_bar); mbar_arrive(full); }
                     __syncwarp();
                     TRACE(12);
                     if (++slot == S) slot = 0;
@@ -515,6 +562,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                     __syncwarp();
                 }
                 if (elect_one()) {
+                    if (ragged) { *info = info_v; mbar_arrive(info_bar); }
                     if (by_tma) {
                         // one tensor-map box = the whole chunk: rows_per_chunk hop-rows of pitch width (implicit im2col)
                         mbar_arrive_expect_tx(full, (uint32_t)p.rows_per_chunk * (uint32_t)p.pitch_bytes);
@@ -540,6 +588,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 ++chunk_count;
                 if (++cq == 4) { cq = 0; if (++ctp == P) { ctp = 0; cph ^= 1u; } }
             }
+            ++tl;
         }
         (void)cph;
         if (EARLY_LOADER) cluster_wait();   // the phase it arrived on at set-up, before the exit barrier below
@@ -723,22 +772,41 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         uint32_t sph = 0;
         const bool fast_log = p.n_mfcc == 0 && !p.output_power && p.tap == nullptr;
         bool dep_done = false;
+        int tl = 0;   // tiles of this CTA so far
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+            // where this warp's 32 rows go: dense batches by division; ragged ones from the loader's chunk record (acquired through
+            // the INFO barrier of this ring entry: this warp is its only waiter and waits for each of its phases once, in order)
+            long long out_row0;       // ragged: first output row of the chunk
+            int nvalid32;             // ragged: frames of the chunk that exist
             Tile2 ti;
-            get_tile2<RAGGED>(p, tile, ti);
+            if constexpr (RAGGED) {
+                mbar_wait(BAR(V_INFO + q + 4 * (tl & 7)), (uint32_t)((tl >> 3) & 1));
+                const ChunkInfo ci = chunk_info[q + 4 * (tl & 7)];
+                out_row0 = ci.row0; nvalid32 = ci.nvalid;
+                ti.clip = 0; ti.t0 = 0; ti.T = 0; ti.s0 = 0; ti.f0 = 0;
+                ti.pass = p.passes > 1 ? tile % p.passes : 0;
+            } else {
+                get_tile2<false>(p, tile, ti);
+                out_row0 = 0; nvalid32 = 0;
+            }
+            ++tl;
             const int b = ti.clip;
             const int t0 = ti.t0 + (int)rank * 128;
             const long long T = ti.T;
-            const bool valid = (long long)(t0 + row) < T;
+            const bool valid = RAGGED ? lane < nvalid32 : (long long)(t0 + row) < T;
             float *optr, *tptr;
             long long cstride;
             const int c_off = ti.pass * p.nb;                                   // first bin of this pass
             const int nm = p.n_mels - c_off < p.nb ? p.n_mels - c_off : p.nb;   // bins of this pass
-            if (p.feature_major) {
+            if (RAGGED) {        // packed, frame-major
+                optr = p.out + (out_row0 + lane) * p.n_ch + c_off;
+                tptr = p.tap ? p.tap + (out_row0 + lane) * p.n_mels + c_off : nullptr;
+                cstride = 1;
+            } else if (p.feature_major) {
                 optr = p.out + ((long long)b * p.n_ch + c_off) * T + t0 + row;
                 tptr = p.tap ? p.tap + ((long long)b * p.n_mels + c_off) * T + t0 + row : nullptr;
                 cstride = T;
-            } else {   // frame-major; ragged batches: packed, the clip starts at frame ti.f0
+            } else {   // frame-major
                 optr = p.out + (ti.f0 + t0 + row) * p.n_ch + c_off;
                 tptr = p.tap ? p.tap + (ti.f0 + t0 + row) * p.n_mels + c_off : nullptr;
                 cstride = 1;
@@ -800,9 +868,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 const uint32_t eb = acc_empty_remote + (uint32_t)stage * 8u;
                 // frame-major MFCCT with a staging block: this warp's 32 frames start at row (t0 + 32 q) of the clip
                 float *estage = (p.off_epi && !p.feature_major) ? reinterpret_cast<float *>(smem + p.off_epi) + q * 32 * p.n_mfcc : nullptr;
-                float *ewout = p.out + (ti.f0 + t0 + q * 32) * p.n_ch;
+                float *ewout = RAGGED ? p.out + out_row0 * p.n_ch : p.out + (ti.f0 + t0 + q * 32) * p.n_ch;
                 const long long erem = T - (long long)(t0 + q * 32);
-                const int envalid = erem <= 0 ? 0 : (erem < 32 ? (int)erem : 32);
+                const int envalid = RAGGED ? nvalid32 : (erem <= 0 ? 0 : (erem < 32 ? (int)erem : 32));
                 if (p.n_mfcc == 0) epi_generic<0>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
                 else if (p.dct_pitch <= 16) epi_generic<4>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
                 else if (p.dct_pitch <= 40) epi_generic<10>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
@@ -825,20 +893,32 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         uint32_t aph = (uint32_t)((g / p.a_slots) & 1);
         // SHARE (single accumulator stage, log-Mel): this warp also drains its share of the previous tile's accumulator --
         // after its second K-step of the next tile, so that the MMAs find operands waiting when the drain releases them.
-        int pend_tile = -1, dstage = 0;
+        int pend_tile = -1, pend_tl = 0, dstage = 0;
+        int tl = 0;   // tiles of this CTA so far
         uint32_t dph = 0;
         bool dep_done = false;
         const uint32_t acc_empty_remote = mapa_cluster(BAR(V_ACC_EMPTY), 0);
 #define DRAIN_PENDING()                                                                                          \
         do {                                                                                                     \
             Tile2 dt;                                                                                            \
-            get_tile2<RAGGED>(p, pend_tile, dt);                                                                 \
-            const int drow = q * 32 + lane, dt0 = dt.t0 + (int)rank * 128;                                       \
-            const bool dvalid = (long long)(dt0 + drow) < dt.T;                                                  \
-            const int dc_off = dt.pass * p.nb;                                                                   \
+            bool dvalid;                                                                                         \
+            float *doptr;                                                                                        \
+            int dc_off;                                                                                          \
+            if constexpr (RAGGED) {   /* this warp converted the chunk of tile pend_tl itself: its record is in the ring */ \
+                const ChunkInfo ci = chunk_info[q + 4 * (pend_tl & 7)];                                          \
+                dt.T = 0;                                                                                        \
+                dc_off = (p.passes > 1 ? pend_tile % p.passes : 0) * p.nb;                                       \
+                dvalid = lane < ci.nvalid;                                                                       \
+                doptr = p.out + (ci.row0 + lane) * p.n_ch + dc_off;                                              \
+            } else {                                                                                             \
+                get_tile2<false>(p, pend_tile, dt);                                                              \
+                const int drow = q * 32 + lane, dt0 = dt.t0 + (int)rank * 128;                                   \
+                dvalid = (long long)(dt0 + drow) < dt.T;                                                         \
+                dc_off = dt.pass * p.nb;                                                                         \
+                doptr = p.feature_major ? p.out + ((long long)dt.clip * p.n_ch + dc_off) * dt.T + dt0 + drow     \
+                                        : p.out + (dt.f0 + dt0 + drow) * p.n_ch + dc_off;                        \
+            }                                                                                                    \
             const int dnm = p.n_mels - dc_off < p.nb ? p.n_mels - dc_off : p.nb;                                 \
-            float *doptr = p.feature_major ? p.out + ((long long)dt.clip * p.n_ch + dc_off) * dt.T + dt0 + drow   \
-                                           : p.out + (dt.f0 + dt0 + drow) * p.n_ch + dc_off;                     \
             mbar_wait(BAR(V_ACC_FULL + dstage), dph);                                                            \
             if (!dep_done) { asm volatile("griddepcontrol.wait;" ::: "memory"); dep_done = true; }               \
             tc_fence_after();                                                                                    \
@@ -855,25 +935,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             TRACE(40);
             const char *gxb = nullptr;   // DIRECT: this thread's frame in global memory
-            if (DIRECT) {
+            if constexpr (DIRECT && !RAGGED) {   // (the direct-load form is dense only)
                 Tile2 ti;
-                get_tile2<RAGGED>(p, tile, ti);
+                get_tile2<false>(p, tile, ti);
                 const long long trow = ti.t0 + (int)rank * 128 + q * 32 + lane;
                 gxb = reinterpret_cast<const char *>(p.x + ti.s0 + (trow < ti.T ? trow : 0) * p.hop);   // rows of no frame re-read frame 0
             } else {
                 mbar_wait(BAR(V_STG_FULL + sbar), sph);
             }
-            if (RAGGED) {   // a template parameter: the dense instantiation must not carry this call in its converter loop
-                // ragged: group 0's warp realigns its chunk (see the loader), the other groups wait for it
-                if (g == 0) {
-                    ragged_realign(p.offsets, p.tile_prefix, p.n_clips, p.passes > 1 ? tile / p.passes : tile,
-                                   reinterpret_cast<float *>(smem + p.off_stg + (size_t)sslot * p.slot_bytes),
-                                   p.rows_per_chunk * (p.pitch_bytes >> 2), lane);
-                    if (lane == 0) mbar_arrive(BAR(V_STG_READY + sbar));
-                } else {
-                    mbar_wait(BAR(V_STG_READY + sbar), sph);
-                }
-            }
+            // ragged: words by which this chunk sits further into its rows than the load table says (see load_shifted)
+            const int dlt = RAGGED ? chunk_info[q + 4 * (tl & 7)].dlt : 0;
             TRACE(41);
             const uint32_t fb = row_off + (uint32_t)sslot * (uint32_t)p.slot_bytes;
             bool released = false;
@@ -896,27 +967,33 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 TRACE(42);
                 const short *tb = p.tab[u];
                 float fw[KS], bw[KS];
-#pragma unroll
-                for (int i = 0; i < NQ; ++i) {
-                    const float4 f = DIRECT ? ldg128(gxb + (int)tb[i]) : lds128(fb + (uint32_t)(int)tb[i]);
-                    fw[4 * i + 0] = f.x; fw[4 * i + 1] = f.y; fw[4 * i + 2] = f.z; fw[4 * i + 3] = f.w;
-                }
-                // mirrored partner of pair e is the sample at position KS-1-e of the descending run
-                if (SIGMA == 0) {
-#pragma unroll
-                    for (int i = 0; i < NQ; ++i) {
-                        const float4 f = DIRECT ? ldg128(gxb + (int)tb[4 + i]) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs+4i .. rs+4i+3
-                        bw[KS - 1 - (4 * i + 0)] = f.x; bw[KS - 1 - (4 * i + 1)] = f.y;
-                        bw[KS - 1 - (4 * i + 2)] = f.z; bw[KS - 1 - (4 * i + 3)] = f.w;
-                    }
+                if (RAGGED && dlt != 0) {   // warp-uniform: one misalignment per chunk
+                    if (dlt == 1) load_shifted<KS, SIGMA, 1>(fb, tb, fw, bw);
+                    else if (dlt == 2) load_shifted<KS, SIGMA, 2>(fb, tb, fw, bw);
+                    else load_shifted<KS, SIGMA, 3>(fb, tb, fw, bw);
                 } else {
 #pragma unroll
                     for (int i = 0; i < NQ; ++i) {
-                        const float4 f = DIRECT ? ldg128(gxb + (int)tb[4 + i]) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs-1+4i .. rs+2+4i
-                        if (i > 0) bw[KS - 1 - (4 * i - 1)] = f.x;                  // position 4i-1 of the run
-                        bw[KS - 1 - (4 * i + 0)] = f.y; bw[KS - 1 - (4 * i + 1)] = f.z; bw[KS - 1 - (4 * i + 2)] = f.w;
+                        const float4 f = DIRECT ? ldg128(gxb + (int)tb[i]) : lds128(fb + (uint32_t)(int)tb[i]);
+                        fw[4 * i + 0] = f.x; fw[4 * i + 1] = f.y; fw[4 * i + 2] = f.z; fw[4 * i + 3] = f.w;
                     }
-                    bw[0] = DIRECT ? ldg32(gxb + (int)tb[8]) : lds32(fb + (uint32_t)(int)tb[8]);   // position KS-1 of the run
+                    // mirrored partner of pair e is the sample at position KS-1-e of the descending run
+                    if (SIGMA == 0) {
+#pragma unroll
+                        for (int i = 0; i < NQ; ++i) {
+                            const float4 f = DIRECT ? ldg128(gxb + (int)tb[4 + i]) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs+4i .. rs+4i+3
+                            bw[KS - 1 - (4 * i + 0)] = f.x; bw[KS - 1 - (4 * i + 1)] = f.y;
+                            bw[KS - 1 - (4 * i + 2)] = f.z; bw[KS - 1 - (4 * i + 3)] = f.w;
+                        }
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < NQ; ++i) {
+                            const float4 f = DIRECT ? ldg128(gxb + (int)tb[4 + i]) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs-1+4i .. rs+2+4i
+                            if (i > 0) bw[KS - 1 - (4 * i - 1)] = f.x;                  // position 4i-1 of the run
+                            bw[KS - 1 - (4 * i + 0)] = f.y; bw[KS - 1 - (4 * i + 1)] = f.z; bw[KS - 1 - (4 * i + 2)] = f.w;
+                        }
+                        bw[0] = DIRECT ? ldg32(gxb + (int)tb[8]) : lds32(fb + (uint32_t)(int)tb[8]);   // position KS-1 of the run
+                    }
                 }
                 const uint32_t dst = lane_taddr + (uint32_t)aslot * (uint32_t)p.unit_cols;
                 if (PREC == P2_COMP) {
@@ -999,7 +1076,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             if (SHARE) {
                 if (pend_tile >= 0) DRAIN_PENDING();   // short windows: fewer than three K-steps per group
                 pend_tile = tile;
+                pend_tl = tl;
             }
+            ++tl;
         }
         if (SHARE && pend_tile >= 0) DRAIN_PENDING();   // the last tile
 #undef STG_RELEASE_IF_LAST

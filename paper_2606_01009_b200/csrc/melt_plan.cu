@@ -260,8 +260,8 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
         if (rc) return rc;
         const bool v2 = p->v2_ok && !p->k2.direct && (((uintptr_t)x & 15) == 0);
         if (v2) {
-            // the CTA-pair kernel: 256-frame tiles, looked up on the device; chunks start at any sample of the packed buffer
-            rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, tile_prefix, 256, st);
+            // the CTA-pair kernel: tiles of 8 chunks of 32 frames, looked up on the device; chunks start at any sample of the packed buffer
+            rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, tile_prefix, 32, st);   // exclusive prefix of 32-frame chunks per clip
             K2Params k2 = p->k2;
             k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = 0; k2.frames_per_clip = 0;
             k2.tiles_per_clip = 0; k2.n_tiles = -1;
