@@ -246,8 +246,9 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) melt_fwd_kernel(const __grid_c
                             else v = fmaxf(fmaf(__log2f(praw), kLog10_2, p.out_log10_offset), -10.f);  // Eq. (8), contract form
                             if (p.n_mfcc > 0) {
                                 const float *drow = dct_s + m * p.dct_pitch;
-                                if (p.dct_pitch <= 16) dct_accumulate<4>(cacc, drow, v);
-                                else if (p.dct_pitch <= 40) dct_accumulate<10>(cacc, drow, v);
+                                if (p.dct_pitch <= 16) dct_accumulate<4>(cacc, drow, v);       // the table's rows are padded to 16 cepstra
+                                else if (p.dct_pitch <= 32) dct_accumulate<8>(cacc, drow, v);
+                                else if (p.dct_pitch <= 48) dct_accumulate<12>(cacc, drow, v);
                                 else dct_accumulate<16>(cacc, drow, v);
                                 if (p.tap && valid) p.tap[tbase + m * cstride_tap] = v;
                             } else if (valid) {

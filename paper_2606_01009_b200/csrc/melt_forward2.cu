@@ -28,7 +28,8 @@ int plan_build_v2(melt_plan *p) {
     k.nb = round_up2((M + k.passes - 1) / k.passes, 16);
     if (k.nb < 32) k.nb = 32;
     // ---- what the kernel covers (everything else stays on the general v1 kernel)
-    if (k.units > V2_MAX_UNITS || (H & 3) || (k1.a0 & 3)) return MELT_OK;
+    k.a0 = k1.a0; k.b0 = k1.b0;
+    if ((H & 3) || (k1.a0 & 3)) return MELT_OK;
     if (p->pad != MELT_PAD_NONE && (N & 7)) return MELT_OK;   // reflect padding: the padded copy keeps every clip start 16-byte aligned
     if (k.passes > 1 && p->n_mfcc > 0) return MELT_OK;             // the DCT needs all bins of a frame in one pass
     const int rs = k1.b0 - (k.kstep - 1);           // lowest sample of the mirrored run of unit 0
@@ -93,7 +94,12 @@ int plan_build_v2(melt_plan *p) {
         int row = n >= 0 ? n / H : -((-n + H - 1) / H);
         return (row * pitch_words + (n - row * H)) * 4;
     };
-    for (int u = 0; u < k.units; ++u) {
+    if (!k.direct && k.units > V2_MAX_UNITS) return MELT_OK;   // the staged forms look their offsets up per K-step
+    if (k.direct) {   // the direct-load form computes them: every read must stay inside the frame, [0, N) samples
+        const int lo = k1.b0 - k.kstep * (k.units - 1) - (k.kstep - 1) - sigma, hi = k1.a0 + k.kstep * k.units;
+        if (lo < 0 || hi > N || k1.b0 + 1 > N) return MELT_OK;
+    }
+    for (int u = 0; u < (k.direct ? 0 : k.units); ++u) {
         const int nq = k.kstep / 4;
         for (int i = 0; i < nq; ++i) k.tab[u][i] = (short)off_of(k1.a0 + k.kstep * u + 4 * i);
         const int run = k1.b0 - k.kstep * u - (k.kstep - 1);   // lowest sample of the mirrored run

@@ -79,6 +79,12 @@ __device__ __forceinline__ uint64_t f2_sub(uint64_t a, uint64_t b) {
     asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
     return r;
 }
+__device__ __forceinline__ uint64_t f2_fma(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ void f2_unpack(uint64_t a, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a)); }
 __device__ __forceinline__ uint64_t f2_mul(uint64_t a, uint64_t b) {
     uint64_t r;
     asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
@@ -145,65 +151,74 @@ __device__ __forceinline__ void epi_fast_share(uint32_t t_r, uint32_t t_i, int n
 }
 
 // Epilogue of one tile for one thread (= frame) in the general case: power or log output, optional tap of the log-Mel
-// matrix, optional DCT-II with 4 * KQ accumulators (KQ = 0: no DCT).  Returns after handing the accumulator stage back.
-template <int KQ>
+// matrix, optional DCT-II.  The DCT keeps 16 accumulators: more than 16 cepstra are produced in blocks of 16, the log-Mel
+// values being re-formed from tensor memory for every block (the paper's K = 40 costs three passes over the bins; keeping 40
+// .. 64 accumulators per thread instead pushed the whole kernel to 128 registers with spills).  Returns after handing the
+// accumulator stage back.
+template <bool HAS_DCT>
 __device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uint32_t t_i, const float *dct_s, float *optr, float *tptr,
                                             long long cstride, bool valid, int lane, uint32_t acc_empty_bar, int nm,
                                             float *stage, float *warp_out, int nvalid) {
     const float kLog10_2 = 0.30102999566398120f;
-    float cacc[KQ > 0 ? 4 * KQ : 1];
+    const int K = p.n_mfcc;
+    for (int q0 = 0; q0 < (HAS_DCT ? K : 1); q0 += 16) {
+        float cacc[HAS_DCT ? 16 : 1];
 #pragma unroll
-    for (int k = 0; k < (KQ > 0 ? 4 * KQ : 1); ++k) cacc[k] = 0.f;
-    for (int c0 = 0; c0 < p.nb; c0 += 16) {
-        uint32_t vr[16], vi[16];
-        tmem_ld16(t_r + (uint32_t)c0, vr);
-        tmem_ld16(t_i + (uint32_t)c0, vi);
-        tmem_wait_ld();
+        for (int k = 0; k < (HAS_DCT ? 16 : 1); ++k) cacc[k] = 0.f;
+        for (int c0 = 0; c0 < p.nb; c0 += 16) {
+            uint32_t vr[16], vi[16];
+            tmem_ld16(t_r + (uint32_t)c0, vr);
+            tmem_ld16(t_i + (uint32_t)c0, vi);
+            tmem_wait_ld();
 #pragma unroll
-        for (int c = 0; c < 16; ++c) {
-            const int m = c0 + c;
-            if (m < nm) {
-                const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
-                const float praw = fmaf(r, r, im * im);                                          // Eq. (4)
-                float v;
-                if (p.output_power) v = praw * p.out_scale;
-                else v = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, p.out_log10_offset), -10.f);       // Eq. (8), contract form
-                if (KQ > 0) {
-                    const float *drow = dct_s + m * p.dct_pitch;
+            for (int c = 0; c < 16; ++c) {
+                const int m = c0 + c;
+                if (m < nm) {
+                    const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                    const float praw = fmaf(r, r, im * im);                                          // Eq. (4)
+                    float v;
+                    if (p.output_power) v = praw * p.out_scale;
+                    else v = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, p.out_log10_offset), -10.f);       // Eq. (8), contract form
+                    if (HAS_DCT) {
+                        const float *drow = dct_s + m * p.dct_pitch + q0;
 #pragma unroll
-                    for (int q4 = 0; q4 < KQ; ++q4) {
-                        const float4 d = *reinterpret_cast<const float4 *>(drow + 4 * q4);
-                        cacc[4 * q4 + 0] = fmaf(d.x, v, cacc[4 * q4 + 0]);
-                        cacc[4 * q4 + 1] = fmaf(d.y, v, cacc[4 * q4 + 1]);
-                        cacc[4 * q4 + 2] = fmaf(d.z, v, cacc[4 * q4 + 2]);
-                        cacc[4 * q4 + 3] = fmaf(d.w, v, cacc[4 * q4 + 3]);
+                        for (int q4 = 0; q4 < 4; ++q4) {   // the table's rows are zero padded to whole blocks of 16 cepstra
+                            const float4 d = *reinterpret_cast<const float4 *>(drow + 4 * q4);   // D[q0 + 4 q4 .. + 3][m]
+                            cacc[4 * q4 + 0] = fmaf(d.x, v, cacc[4 * q4 + 0]);
+                            cacc[4 * q4 + 1] = fmaf(d.y, v, cacc[4 * q4 + 1]);
+                            cacc[4 * q4 + 2] = fmaf(d.z, v, cacc[4 * q4 + 2]);
+                            cacc[4 * q4 + 3] = fmaf(d.w, v, cacc[4 * q4 + 3]);
+                        }
+                        if (q0 == 0 && tptr && valid) tptr[m * cstride] = v;
+                    } else if (valid) {
+                        optr[m * cstride] = v;
                     }
-                    if (tptr && valid) tptr[m * cstride] = v;
-                } else if (valid) {
-                    optr[m * cstride] = v;
                 }
             }
         }
-    }
-    tc_fence_before();
-    __syncwarp();
-    if (lane == 0) mbar_arrive_remote(acc_empty_bar);
-    if (KQ > 0 && stage != nullptr) {                                                           // Eq. (9)
-        // frame-major cepstra: the 32 frames of this warp are 32 * n_mfcc consecutive floats of the output.  Every thread
-        // parks its row in shared memory, then the warp writes the block with consecutive lanes on consecutive addresses
-        // (a thread storing its own row touches n_mfcc scattered 4-byte pieces: 13x the sector traffic for 13 cepstra).
-        const int K = p.n_mfcc;
+        if (!HAS_DCT || q0 + 16 >= K) {   // last pass over the accumulators: the MMAs of the tile after next may overwrite them
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_remote(acc_empty_bar);
+        }
+        if (HAS_DCT && stage != nullptr) {                                                           // Eq. (9)
+            // frame-major cepstra: the 32 frames of this warp are 32 * n_mfcc consecutive floats of the output.  Every thread
+            // parks its row in shared memory, then the warp writes the block with consecutive lanes on consecutive addresses
+            // (a thread storing its own row touches n_mfcc scattered 4-byte pieces: 13x the sector traffic for 13 cepstra).
 #pragma unroll
-        for (int k = 0; k < 4 * KQ; ++k)
-            if (k < K) stage[lane * K + k] = cacc[k];
+            for (int k = 0; k < 16; ++k)
+                if (q0 + k < K) stage[lane * K + q0 + k] = cacc[k];
+        } else if (HAS_DCT && valid) {
+#pragma unroll
+            for (int k = 0; k < 16; ++k)
+                if (q0 + k < K) optr[(q0 + k) * cstride] = cacc[k];
+        }
+    }
+    if (HAS_DCT && stage != nullptr) {
         __syncwarp();
         const int n_out = nvalid * K;
         for (int w = lane; w < n_out; w += 32) warp_out[w] = stage[w];
         __syncwarp();
-    } else if (KQ > 0 && valid) {
-#pragma unroll
-        for (int k = 0; k < 4 * KQ; ++k)
-            if (k < p.n_mfcc) optr[k * cstride] = cacc[k];
     }
 }
 
@@ -376,7 +391,26 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     TRACE_DECL
     TRACE(1);
     if (warp == W_LOAD && DIRECT) {
-        // windows too long for staged 32-frame chunks: the converter threads read their frames straight from global memory
+        // Windows too long for staged 32-frame chunks: the converter threads read their frames straight from global memory.
+        // This warp pulls the sample span of every tile of this CTA into L2 ahead of them (bulk prefetches of 16 KB, one per
+        // lane and round), so that their loads cost L2 hits: a tile is 256 hops + one window of contiguous samples.
+        if constexpr (!RAGGED) {
+            for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+                Tile2 ti;
+                get_tile2<false>(p, tile, ti);
+                const long long r0 = ti.t0 + (long long)rank * 128;
+                if (r0 >= ti.T) continue;
+                const long long nfr = ti.T - r0 < 128 ? ti.T - r0 : 128;
+                const char *src = reinterpret_cast<const char *>(p.x + ti.s0 + r0 * p.hop);
+                long long bytes = ((nfr - 1) * p.hop + p.n_fft) * 4;
+                const long long room = (p.len - r0 * p.hop) * 4;
+                bytes = (bytes < room ? bytes : room) & ~15ll;
+                for (long long o = (long long)lane * 16384; o < bytes; o += 32ll * 16384) {
+                    const long long n = bytes - o < 16384 ? bytes - o : 16384;
+                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src + o), "r"((uint32_t)n) : "memory");
+                }
+            }
+        }
     } else if (warp == W_LOAD) {
         // ============================================================== signal loader (bulk-copy engine)
         // The whole warp runs the (uniform) loop; one elected lane issues the copies.
@@ -871,10 +905,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 float *ewout = RAGGED ? p.out + out_row0 * p.n_ch : p.out + (ti.f0 + t0 + q * 32) * p.n_ch;
                 const long long erem = T - (long long)(t0 + q * 32);
                 const int envalid = RAGGED ? nvalid32 : (erem <= 0 ? 0 : (erem < 32 ? (int)erem : 32));
-                if (p.n_mfcc == 0) epi_generic<0>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
-                else if (p.dct_pitch <= 16) epi_generic<4>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
-                else if (p.dct_pitch <= 40) epi_generic<10>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
-                else epi_generic<16>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
+                if (p.n_mfcc == 0) epi_generic<false>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
+                else epi_generic<true>(p, t_r, t_i, dct_s, optr, tptr, cstride, valid, lane, eb, nm, estage, ewout, envalid);
             }
             TRACE(32);
             if (++stage == p.acc_stages) { stage = 0; sph ^= 1u; }
@@ -965,7 +997,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 if (SHARE && pend_tile >= 0 && u >= u0 + 2 * NG) DRAIN_PENDING();
                 // ---- loads: NQ forward quads, NQ mirrored quads (+ one single when the mirrored run starts at 1 mod 4)
                 TRACE(42);
-                const short *tb = p.tab[u];
+                const short *tb = p.tab[DIRECT ? 0 : u];
+                // direct-load form: frames are read in place, sample n of a frame is byte 4 n of it -- no table (and no limit on
+                // the number of K-steps): forward quads from a0 + KS u, mirrored quads from b0 - KS u - (KS - 1) - SIGMA
+                const int dfw = DIRECT ? 4 * (p.a0 + KS * u) : 0, dbw = DIRECT ? 4 * (p.b0 - KS * u - (KS - 1) - SIGMA) : 0;
                 float fw[KS], bw[KS];
                 if (RAGGED && dlt != 0) {   // warp-uniform: one misalignment per chunk
                     if (dlt == 1) load_shifted<KS, SIGMA, 1>(fb, tb, fw, bw);
@@ -974,25 +1009,25 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 } else {
 #pragma unroll
                     for (int i = 0; i < NQ; ++i) {
-                        const float4 f = DIRECT ? ldg128(gxb + (int)tb[i]) : lds128(fb + (uint32_t)(int)tb[i]);
+                        const float4 f = DIRECT ? ldg128(gxb + dfw + 16 * i) : lds128(fb + (uint32_t)(int)tb[i]);
                         fw[4 * i + 0] = f.x; fw[4 * i + 1] = f.y; fw[4 * i + 2] = f.z; fw[4 * i + 3] = f.w;
                     }
                     // mirrored partner of pair e is the sample at position KS-1-e of the descending run
                     if (SIGMA == 0) {
 #pragma unroll
                         for (int i = 0; i < NQ; ++i) {
-                            const float4 f = DIRECT ? ldg128(gxb + (int)tb[4 + i]) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs+4i .. rs+4i+3
+                            const float4 f = DIRECT ? ldg128(gxb + dbw + 16 * i) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs+4i .. rs+4i+3
                             bw[KS - 1 - (4 * i + 0)] = f.x; bw[KS - 1 - (4 * i + 1)] = f.y;
                             bw[KS - 1 - (4 * i + 2)] = f.z; bw[KS - 1 - (4 * i + 3)] = f.w;
                         }
                     } else {
 #pragma unroll
                         for (int i = 0; i < NQ; ++i) {
-                            const float4 f = DIRECT ? ldg128(gxb + (int)tb[4 + i]) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs-1+4i .. rs+2+4i
+                            const float4 f = DIRECT ? ldg128(gxb + dbw + 16 * i) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs-1+4i .. rs+2+4i
                             if (i > 0) bw[KS - 1 - (4 * i - 1)] = f.x;                  // position 4i-1 of the run
                             bw[KS - 1 - (4 * i + 0)] = f.y; bw[KS - 1 - (4 * i + 1)] = f.z; bw[KS - 1 - (4 * i + 2)] = f.w;
                         }
-                        bw[0] = DIRECT ? ldg32(gxb + (int)tb[8]) : lds32(fb + (uint32_t)(int)tb[8]);   // position KS-1 of the run
+                        bw[0] = DIRECT ? ldg32(gxb + 4 * (p.b0 - KS * u)) : lds32(fb + (uint32_t)(int)tb[8]);   // position KS-1 of the run
                     }
                 }
                 const uint32_t dst = lane_taddr + (uint32_t)aslot * (uint32_t)p.unit_cols;

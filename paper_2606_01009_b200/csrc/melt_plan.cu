@@ -83,7 +83,7 @@ int plan_build_device(melt_plan *p) {
     k.a_slots = std::min(MAX_A_SLOTS, (512 - k.a_col0) / k.unit_cols);
     if (k.a_slots < 2) return fail(MELT_ERR_UNSUPPORTED, "tensor-memory budget exceeded (nb=%d)", k.nb);
     k.unit_b_bytes = (uint32_t)(k.nk * k.nb * 32);
-    k.dct_pitch = round_up(std::max(p->n_mfcc, 1), 4);
+    k.dct_pitch = round_up(std::max(p->n_mfcc, 1), 16);   // floats per Mel bin: whole blocks of 16 cepstra (zero padded)
 
     // ---- shared-memory plan
     const uint32_t tab_bytes = (uint32_t)(k.units * k.kstep * 4);

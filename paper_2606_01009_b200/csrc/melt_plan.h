@@ -34,7 +34,7 @@ struct KParams {
     int stg_comb, stg_slots, chunk_units, stg_pitch, stg_slot_words;
     unsigned long long hop_inv40;          // ceil(2^40 / hop): exact division of sample indices < 2^24
     uint32_t off_b, off_stg, off_tab, off_dct, off_bar, smem_bytes;
-    int dct_pitch;                         // floats per Mel bin in the DCT table (n_mfcc rounded up to 4)
+    int dct_pitch;                         // floats per Mel bin in the DCT table (n_mfcc rounded up to 16)
     // ---- numerics
     float in_scale, out_scale, out_log10_offset;
     int output_power;
@@ -70,6 +70,7 @@ struct K2Params {
     // ---- analysis geometry (as KParams)
     int n_fft, hop, n_mels, n_mfcc, n_ch;
     int kstep, units, nb, nk, unit_cols;
+    int a0, b0;                // fold geometry: pairs (a0 + j, b0 - j)
     int acc_cols, acc_stages, a_slots, a_col0;
     // ---- staging ring of 32-frame chunks: rows of `hop` samples at a padded pitch
     int rows_per_chunk, pitch_bytes, slot_bytes, stg_slots;

@@ -173,3 +173,32 @@ def make_inputs(cfg, n_clips=None, seed=None):
     if cfg.startswith("cfg4"):
         return dict(x=hires_batch(n, c["seed"], c["fs"], c["clip_len"]), offsets=None)
     raise KeyError(cfg)
+
+
+# ------------------------------------------------------------------------------------------------ the paper's own shapes
+# Table 4 of the paper -- spectral front end 16 kHz / N = 400 / H = 160 /
+# M = 80 / 80-7600 Hz, cepstral front end N = 1200 / H = 160 / M = 128 / K = 40 / 0-8000 Hz, "symmetric Hann" --
+# on what the paper sweeps: one clip of 1 .. 160 s (Table 5), the number of Mel bins 40 .. 512 at 160 s
+# (Fig. 6) and batches of 1 .. 256 utterances of 4 s (Fig. 7).  The paper measures on LibriSpeech /
+# Libri6000 speech; these clips are the seeded harmonic-tone mixes of speaker_ragged (a voiced-speech-like spectrum), which
+# stand in for that material.  No padding, frame-major output (the paper states neither; readings R3 / R5).
+_SPEC = dict(fs=16000.0, n_fft=400, hop=160, window=WINDOW_HANN_SYMMETRIC, n_mels=80, fmin=80.0, fmax=7600.0, n_mfcc=0,
+             pad_reflect=False, drop_last=False, layout="frame_major")
+_CEP = dict(fs=16000.0, n_fft=1200, hop=160, window=WINDOW_HANN_SYMMETRIC, n_mels=128, fmin=0.0, fmax=8000.0, n_mfcc=40,
+            pad_reflect=False, drop_last=False, layout="frame_major")
+PAPER_CONFIGS = {}
+for _d in (1, 10, 40, 160):
+    PAPER_CONFIGS["paper_spec_%ds" % _d] = dict(_SPEC, n_clips=1, clip_len=16000 * _d, seed=BASE_SEED + 100 + _d)
+    PAPER_CONFIGS["paper_cep_%ds" % _d] = dict(_CEP, n_clips=1, clip_len=16000 * _d, seed=BASE_SEED + 300 + _d)
+for _m in (40, 128, 256, 512):
+    PAPER_CONFIGS["paper_mel%d_160s" % _m] = dict(_SPEC, n_mels=_m, n_clips=1, clip_len=16000 * 160, seed=BASE_SEED + 500 + _m)
+for _b in (1, 16, 256):
+    PAPER_CONFIGS["paper_batch%d_4s" % _b] = dict(_SPEC, n_clips=_b, clip_len=64000, seed=BASE_SEED + 700 + _b)
+
+
+def make_paper_inputs(name, n_clips=None):
+    """Dense batch [n_clips, clip_len] float32 of a PAPER_CONFIGS entry: per clip 2-6 harmonic tones + noise (speaker_ragged's law)."""
+    c = PAPER_CONFIGS[name]
+    n = c["n_clips"] if n_clips is None else int(n_clips)
+    x, off = speaker_ragged(n, c["seed"], c["fs"], c["clip_len"], c["clip_len"])
+    return dict(x=x.reshape(n, c["clip_len"]), offsets=None)
