@@ -72,15 +72,24 @@ int plan_build_v2(melt_plan *p) {
         if (k.b_resident) { k.b_resident = 0; k.b_slots = std::min(8, k.units); }
         else --k.b_slots;
         if (k.b_slots < std::min(3, k.units)) {   // the issuers take two K-steps per iteration: two different slabs at least
-            // not even a streamed basis leaves room for staged chunks (windows of thousands of samples): no staging at all,
-            // the converter threads read their frames from global memory (L2 serves the 4x frame overlap)
-            k.direct = 1; k.b_slots = std::min(8, k.units); k.stg_slots = 0;
-            k.off_stg = (uint32_t)round_up2((int)((uint32_t)k.b_slots * k.unit_b_bytes), 128) + 128;
+            // Not even a streamed basis leaves room for staged 32-frame chunks (windows of thousands of samples: a chunk is
+            // 32 hops of the signal).  K-STEP STAGING instead: the loader brings, per converter warp and K-step, just the two
+            // runs of kstep (+4) samples of its 32 frames -- one tensor-map box of (kstep + 4) x 32 each, 32 rows one hop apart
+            // -- into a two-slot ring per converter warp (4 lane quarters x 3 groups).  (An earlier version let the converter
+            // threads read their frames from global memory: every lane of a load touches another 128-byte line, and the L1
+            // tag stage, not L2 or DRAM, bounded the kernel at ~3000 cycles per K-step.)
+            k.direct = 1; k.stg_slots = 0;
+            k.kslot_bytes = 2 * 32 * (k.kstep + 4) * 4;
+            for (k.b_slots = std::min(8, k.units);; --k.b_slots) {
+                k.off_stg = (uint32_t)round_up2((int)((uint32_t)k.b_slots * k.unit_b_bytes), 128) + 128;
+                if ((long long)k.off_stg + 24LL * k.kslot_bytes + 128 + dct_bytes + bar_bytes + 256 <= SMEM_BUDGET) break;
+                if (k.b_slots <= std::min(3, k.units)) return MELT_OK;
+            }
             break;
         }
     }
     k.stg_phases = std::max(1, (k.stg_slots + 3) / 4);
-    k.off_dct = (uint32_t)round_up2((int)(k.off_stg + (uint32_t)k.stg_slots * k.slot_bytes + 128), 128);
+    k.off_dct = (uint32_t)round_up2((int)(k.off_stg + (uint32_t)k.stg_slots * k.slot_bytes + (k.direct ? 24u * k.kslot_bytes : 0u) + 128), 128);
     k.off_epi = epi_bytes ? k.off_dct + dct_only : 0;
     k.off_bar = (uint32_t)round_up2((int)(k.off_dct + dct_bytes), 128);
     k.smem_bytes = k.off_bar + bar_bytes;
@@ -95,10 +104,7 @@ int plan_build_v2(melt_plan *p) {
         return (row * pitch_words + (n - row * H)) * 4;
     };
     if (!k.direct && k.units > V2_MAX_UNITS) return MELT_OK;   // the staged forms look their offsets up per K-step
-    if (k.direct) {   // the direct-load form computes them: every read must stay inside the frame, [0, N) samples
-        const int lo = k1.b0 - k.kstep * (k.units - 1) - (k.kstep - 1) - sigma, hi = k1.a0 + k.kstep * k.units;
-        if (lo < 0 || hi > N || k1.b0 + 1 > N) return MELT_OK;
-    }
+    // (K-step staging computes its box coordinates; what a box covers outside [0, N) of a frame row is zero-filled by the engine)
     for (int u = 0; u < (k.direct ? 0 : k.units); ++u) {
         const int nq = k.kstep / 4;
         for (int i = 0; i < nq; ++i) k.tab[u][i] = (short)off_of(k1.a0 + k.kstep * u + 4 * i);
@@ -185,7 +191,26 @@ static EncodeTiledFn encode_tiled_fn() {
 
 int v2_encode_tmap(K2Params &k) {
     k.tma_rows = 0;
-    if (k.direct) return MELT_OK;   // no staging, no tensor map
+    if (k.direct) {
+        // K-step staging: rows = frames (stride hop, extent n_fft: what a box covers beyond a frame's window is out of bounds and
+        // zero-filled), one box = (kstep + 4) samples of 32 consecutive frames
+        EncodeTiledFn encd = encode_tiled_fn();
+        if (!encd || k.len < k.n_fft) return MELT_OK;
+        const long long frows = (k.len - k.n_fft) / k.hop + 1;
+        if (frows > 0x7fffffffLL) return MELT_OK;
+        CUtensorMap tmd;
+        const cuuint64_t gd[3] = {(cuuint64_t)k.n_fft, (cuuint64_t)frows, (cuuint64_t)k.n_clips};
+        const cuuint64_t gs[2] = {(cuuint64_t)k.hop * 4u, (cuuint64_t)k.len * 4u};
+        const cuuint32_t bx[3] = {(cuuint32_t)(k.kstep + 4), 32u, 1u};
+        const cuuint32_t es[3] = {1u, 1u, 1u};
+        if ((gs[0] & 15) || (gs[1] & 15) || gs[1] >= (1ull << 40)) return MELT_OK;
+        if (encd(&tmd, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float *>(k.x), gd, gs, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                 CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return MELT_OK;
+        memcpy(k.tmap, &tmd, 128);
+        k.tma_rows = (int)frows;
+        return MELT_OK;
+    }
     EncodeTiledFn enc = encode_tiled_fn();
     const long long W = k.pitch_bytes / 4;
     // virtual reflect padding: a chunk starts at any multiple of 4 samples of the clip, i.e. at column (start % hop) of hop-row

@@ -38,7 +38,7 @@ enum { P2_COMP = 0, P2_TF32 = 1, P2_BF16 = 2 };
 // barrier indices (8 bytes each)
 enum {
     V_STG_FULL = 0, V_STG_EMPTY = V2_MAX_STG, V_A_FULL = 2 * V2_MAX_STG, V_A_EMPTY = V_A_FULL + 16, V_ACC_FULL = V_A_EMPTY + 16,
-    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_DONE = V_B_PEER + V2_MAX_UNITS, V_STG_READY = V_DONE + 1, V_B_EMPTY = V_STG_READY + V2_MAX_STG, V_INFO = V_B_EMPTY + 8, V_NBARS = V_INFO + 32
+    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_DONE = V_B_PEER + V2_MAX_UNITS, V_STG_READY = V_DONE + 1, V_B_EMPTY = V_STG_READY + V2_MAX_STG, V_INFO = V_B_EMPTY + 8, V_KFULL = V_INFO + 32, V_KEMPTY = V_KFULL + 24, V_NBARS = V_KEMPTY + 24
 };
 constexpr int V2_MAX_A_SLOTS = 16;
 constexpr int W_LOAD = 0, W_MMA = 1, W_BASIS = 2, W_MMA2 = 3, W_EPI0 = 4, W_CONV0 = 8;
@@ -281,6 +281,26 @@ __device__ __forceinline__ void load_shifted(uint32_t fb, const short *tb, float
     }
 }
 
+// K-step staging (very long windows): the thread's row of the slot holds samples n0 .. n0 + KS + 3 of its frame (forward block,
+// n0 = a0 + KS u) and run - SIGMA .. run - SIGMA + KS + 3 (mirrored block, `half` bytes further), both 16-byte aligned.
+template <int KS, int SIGMA>
+__device__ __forceinline__ void load_kstaged(uint32_t kb, uint32_t half, float (&fw)[KS], float (&bw)[KS]) {
+    constexpr int NQ = KS / 4, NB = NQ + (SIGMA > 0 ? 1 : 0);
+    float wb[KS + 4];
+#pragma unroll
+    for (int i = 0; i < NQ; ++i) {
+        const float4 f = lds128(kb + 16u * (uint32_t)i);
+        fw[4 * i + 0] = f.x; fw[4 * i + 1] = f.y; fw[4 * i + 2] = f.z; fw[4 * i + 3] = f.w;
+    }
+#pragma unroll
+    for (int i = 0; i < NB; ++i) {
+        const float4 g = lds128(kb + half + 16u * (uint32_t)i);
+        wb[4 * i + 0] = g.x; wb[4 * i + 1] = g.y; wb[4 * i + 2] = g.z; wb[4 * i + 3] = g.w;
+    }
+#pragma unroll
+    for (int e = 0; e < KS; ++e) bw[KS - 1 - e] = wb[SIGMA + e];   // sample `run + e` of the descending run is the partner of pair KS - 1 - e
+}
+
 static_assert(V_NBARS <= V2_THREADS, "one thread per barrier at set-up");
 template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM, bool DIRECT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
@@ -344,6 +364,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             mbar_init(BAR(V_STG_READY + lane), 1u);
         }
         mbar_init(BAR(V_INFO + lane), 1u);   // 32 = 8 tile phases x 4 lane quarters: chunk info published (ragged batches)
+        if (lane < 24) {                      // K-step staging: two slots per converter warp (4 quarters x up to 3 groups)
+            mbar_init(BAR(V_KFULL + lane), 1u);
+            mbar_init(BAR(V_KEMPTY + lane), 1u);
+        }
         fence_barrier_init();
     } else if (warp == W_MMA || warp == W_MMA2) {
         const int n_b = STREAM ? 8 : (p.units < V2_MAX_UNITS ? p.units : V2_MAX_UNITS);   // basis barriers in use
@@ -391,23 +415,31 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     TRACE_DECL
     TRACE(1);
     if (warp == W_LOAD && DIRECT) {
-        // Windows too long for staged 32-frame chunks: the converter threads read their frames straight from global memory.
-        // This warp pulls the sample span of every tile of this CTA into L2 ahead of them (bulk prefetches of 16 KB, one per
-        // lane and round), so that their loads cost L2 hits: a tile is 256 hops + one window of contiguous samples.
+        // K-step staging (windows too long for staged 32-frame chunks): lane (3 q + g) of this warp feeds converter warp (q, g):
+        // for each of its K-steps u = g, g + NG, ... one box with the forward run and one with the mirrored run -- (KS + 4)
+        // samples of the warp's 32 frames, rows one hop apart in the signal -- into the warp's own two-slot ring.  Twelve lanes
+        // run their (identical-length) sequences side by side, so a wait for a free slot is shared by twelve copies.
         if constexpr (!RAGGED) {
+            const int lq = lane / 3, lg = lane - 3 * lq;           // lane quarter and converter group this lane feeds
+            const bool active = lane < 12 && lg < NG;
+            if (lane == 0) tma_prefetch_desc(p.tmap);
+            int kslot = 0;
+            uint32_t kph = 0;
+            const uint32_t ring0 = sbase + p.off_stg + (uint32_t)(lane * 2) * (uint32_t)p.kslot_bytes;
+            const uint32_t half = (uint32_t)p.kslot_bytes >> 1;
             for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
                 Tile2 ti;
                 get_tile2<false>(p, tile, ti);
-                const long long r0 = ti.t0 + (long long)rank * 128;
-                if (r0 >= ti.T) continue;
-                const long long nfr = ti.T - r0 < 128 ? ti.T - r0 : 128;
-                const char *src = reinterpret_cast<const char *>(p.x + ti.s0 + r0 * p.hop);
-                long long bytes = ((nfr - 1) * p.hop + p.n_fft) * 4;
-                const long long room = (p.len - r0 * p.hop) * 4;
-                bytes = (bytes < room ? bytes : room) & ~15ll;
-                for (long long o = (long long)lane * 16384; o < bytes; o += 32ll * 16384) {
-                    const long long n = bytes - o < 16384 ? bytes - o : 16384;
-                    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src + o), "r"((uint32_t)n) : "memory");
+                const int r0 = ti.t0 + (int)rank * 128 + 32 * lq;   // first frame of the quarter (rows beyond the clip are zero-filled)
+                for (int u = lg; u < p.units; u += NG) {
+                    if (active) {
+                        mbar_wait(BAR(V_KEMPTY + 2 * lane + kslot), kph ^ 1u);
+                        const uint32_t full = BAR(V_KFULL + 2 * lane + kslot), dst = ring0 + (uint32_t)kslot * (uint32_t)p.kslot_bytes;
+                        mbar_arrive_expect_tx(full, (uint32_t)p.kslot_bytes);
+                        tma_load_3d(dst, p.tmap, p.a0 + KS * u, r0, ti.clip, full);                                  // samples a0 + KS u ..
+                        tma_load_3d(dst + half, p.tmap, p.b0 - KS * u - (KS - 1) - SIGMA, r0, ti.clip, full);      // the mirrored run, from its aligned start
+                        if (++kslot == 2) { kslot = 0; kph ^= 1u; }
+                    }
                 }
             }
         }
@@ -927,6 +959,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         // after its second K-step of the next tile, so that the MMAs find operands waiting when the drain releases them.
         int pend_tile = -1, pend_tl = 0, dstage = 0;
         int tl = 0;   // tiles of this CTA so far
+        // K-step staging (DIRECT): this warp's two-slot ring, fed by lane 3 q + g of the loader warp
+        const int kidx = 2 * (3 * q + g);
+        const uint32_t kring = sbase + p.off_stg + (uint32_t)kidx * (uint32_t)p.kslot_bytes + (uint32_t)lane * (uint32_t)((KS + 4) * 4);
+        int kslot = 0;
+        uint32_t kph = 0;
         uint32_t dph = 0;
         bool dep_done = false;
         const uint32_t acc_empty_remote = mapa_cluster(BAR(V_ACC_EMPTY), 0);
@@ -966,12 +1003,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         int u = g;
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             TRACE(40);
-            const char *gxb = nullptr;   // DIRECT: this thread's frame in global memory
-            if constexpr (DIRECT && !RAGGED) {   // (the direct-load form is dense only)
-                Tile2 ti;
-                get_tile2<false>(p, tile, ti);
-                const long long trow = ti.t0 + (int)rank * 128 + q * 32 + lane;
-                gxb = reinterpret_cast<const char *>(p.x + ti.s0 + (trow < ti.T ? trow : 0) * p.hop);   // rows of no frame re-read frame 0
+            if constexpr (DIRECT) {
+                // K-step staging: this group takes K-steps g, g + NG, ... of every tile (the loader feeds them in that order);
+                // ring position of the tile's first one from the running K-step count
+                u = g;
+                const int ug0 = tl * p.units + g;
+                aslot = ug0 % p.a_slots;
+                aph = (uint32_t)((ug0 / p.a_slots) & 1);
             } else {
                 mbar_wait(BAR(V_STG_FULL + sbar), sph);
             }
@@ -984,7 +1022,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             // folded (its samples are in registers), not after the operand store and its hand-off.
 #define STG_RELEASE_IF_LAST()                                                                       \
             do {                                                                                    \
-                if (!DIRECT && u + NG >= p.units) {                                                 \
+                if (DIRECT) {   /* K-step staging: the slot of this K-step goes back to the loader */   \
+                    __syncwarp();                                                                   \
+                    if (lane == 0) mbar_arrive(BAR(V_KEMPTY + kidx + kslot));                       \
+                    if (++kslot == 2) { kslot = 0; kph ^= 1u; }                                     \
+                } else if (u + NG >= p.units) {                                                     \
                     __syncwarp();                                                                   \
                     if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sbar));                            \
                     released = true;                                                                \
@@ -998,36 +1040,36 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 // ---- loads: NQ forward quads, NQ mirrored quads (+ one single when the mirrored run starts at 1 mod 4)
                 TRACE(42);
                 const short *tb = p.tab[DIRECT ? 0 : u];
-                // direct-load form: frames are read in place, sample n of a frame is byte 4 n of it -- no table (and no limit on
-                // the number of K-steps): forward quads from a0 + KS u, mirrored quads from b0 - KS u - (KS - 1) - SIGMA
-                const int dfw = DIRECT ? 4 * (p.a0 + KS * u) : 0, dbw = DIRECT ? 4 * (p.b0 - KS * u - (KS - 1) - SIGMA) : 0;
                 float fw[KS], bw[KS];
-                if (RAGGED && dlt != 0) {   // warp-uniform: one misalignment per chunk
+                if constexpr (DIRECT) {     // K-step staging: this K-step's two runs wait in the warp's own ring
+                    mbar_wait(BAR(V_KFULL + kidx + kslot), kph);
+                    load_kstaged<KS, SIGMA>(kring + (uint32_t)kslot * (uint32_t)p.kslot_bytes, (uint32_t)p.kslot_bytes >> 1, fw, bw);
+                } else if (RAGGED && dlt != 0) {   // warp-uniform: one misalignment per chunk
                     if (dlt == 1) load_shifted<KS, SIGMA, 1>(fb, tb, fw, bw);
                     else if (dlt == 2) load_shifted<KS, SIGMA, 2>(fb, tb, fw, bw);
                     else load_shifted<KS, SIGMA, 3>(fb, tb, fw, bw);
                 } else {
 #pragma unroll
                     for (int i = 0; i < NQ; ++i) {
-                        const float4 f = DIRECT ? ldg128(gxb + dfw + 16 * i) : lds128(fb + (uint32_t)(int)tb[i]);
+                        const float4 f = lds128(fb + (uint32_t)(int)tb[i]);
                         fw[4 * i + 0] = f.x; fw[4 * i + 1] = f.y; fw[4 * i + 2] = f.z; fw[4 * i + 3] = f.w;
                     }
                     // mirrored partner of pair e is the sample at position KS-1-e of the descending run
                     if (SIGMA == 0) {
 #pragma unroll
                         for (int i = 0; i < NQ; ++i) {
-                            const float4 f = DIRECT ? ldg128(gxb + dbw + 16 * i) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs+4i .. rs+4i+3
+                            const float4 f = lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs+4i .. rs+4i+3
                             bw[KS - 1 - (4 * i + 0)] = f.x; bw[KS - 1 - (4 * i + 1)] = f.y;
                             bw[KS - 1 - (4 * i + 2)] = f.z; bw[KS - 1 - (4 * i + 3)] = f.w;
                         }
                     } else {
 #pragma unroll
                         for (int i = 0; i < NQ; ++i) {
-                            const float4 f = DIRECT ? ldg128(gxb + dbw + 16 * i) : lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs-1+4i .. rs+2+4i
+                            const float4 f = lds128(fb + (uint32_t)(int)tb[4 + i]);     // samples rs-1+4i .. rs+2+4i
                             if (i > 0) bw[KS - 1 - (4 * i - 1)] = f.x;                  // position 4i-1 of the run
                             bw[KS - 1 - (4 * i + 0)] = f.y; bw[KS - 1 - (4 * i + 1)] = f.z; bw[KS - 1 - (4 * i + 2)] = f.w;
                         }
-                        bw[0] = DIRECT ? ldg32(gxb + 4 * (p.b0 - KS * u)) : lds32(fb + (uint32_t)(int)tb[8]);   // position KS-1 of the run
+                        bw[0] = lds32(fb + (uint32_t)(int)tb[8]);   // position KS-1 of the run
                     }
                 }
                 const uint32_t dst = lane_taddr + (uint32_t)aslot * (uint32_t)p.unit_cols;

@@ -286,6 +286,8 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
     if (T == 0) return MELT_OK;
     const long long tpc = (T + TILE_M - 1) / TILE_M;
     if (tpc * n_clips > 0x7fffffffLL) return fail(MELT_ERR_UNSUPPORTED, "too many tiles");
+    const float *const x_caller = x;
+    const long long len_caller = len;
     if (p->v2_ok && !(tap && ((uintptr_t)tap & 3))) {
         K2Params k2 = p->k2;
         const bool aligned = v2_accepts(p, x, len);
@@ -317,9 +319,14 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
         k2.tiles_per_clip = (int)tpc2; k2.n_tiles = (int)(tpc2 * n_clips);
         k2.offsets = nullptr; k2.frame_offsets = nullptr; k2.tile_prefix = nullptr;
         v2_encode_tmap(k2);
-        rc = launch_forward2(p, k2, st);
-        if (scratch) cudaFreeAsync(scratch, st);
-        return rc;
+        if (!k2.direct || k2.tma_rows > 0) {   // (K-step staging needs its tensor map; without one the general kernel takes the batch)
+            rc = launch_forward2(p, k2, st);
+            if (scratch) cudaFreeAsync(scratch, st);
+            return rc;
+        }
+        if (scratch) cudaFreeAsync(scratch, st);   // the general kernel pads / realigns on the fly: give it the caller's batch
+        x = x_caller;
+        len = len_caller;
     }
     kp.offsets = nullptr; kp.frame_offsets = nullptr; kp.tile_prefix = nullptr;
     kp.len = len; kp.frames_per_clip = T; kp.tiles_per_clip = (int)tpc; kp.n_tiles = (int)(tpc * n_clips);

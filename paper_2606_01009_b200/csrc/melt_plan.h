@@ -74,6 +74,7 @@ struct K2Params {
     int acc_cols, acc_stages, a_slots, a_col0;
     // ---- staging ring of 32-frame chunks: rows of `hop` samples at a padded pitch
     int rows_per_chunk, pitch_bytes, slot_bytes, stg_slots;
+    int kslot_bytes;           // K-step staging (direct form): bytes of one slot = forward + mirrored block of 32 x (kstep + 4) samples
     int stg_phases;            // ceil(stg_slots / 4): staging barriers are indexed [lane quarter + 4 (tile mod stg_phases)]
     int vpad;                  // MELT_PAD_REFLECT on this kernel: frames start vpad = n_fft/2 samples before sample t * hop, the
                                // samples beyond the clip are mirrored by the loader's edge path (0: no padding)
@@ -98,7 +99,7 @@ struct K2Params {
     // ---- plan-owned device data
     const uint8_t *b_img;  // [2 ranks][passes][units] slabs of unit_b_bytes
     int passes;                // passes over the Mel bins (nb bins each); > 1 needs the streamed basis
-    int direct;                // no staging: converter threads read their frames from global memory (very long windows)
+    int direct;                // very long windows: K-step staging (the loader stages two runs of kstep + 4 samples per frame and K-step)
     int b_resident, b_slots;   // basis half resident in shared memory (b_slots = units), or streamed through a ring of b_slots K-step slabs
     const float *dct;      // [n_mels][dct_pitch]
     // ---- per-unit shared-memory byte offsets (relative to the first sample of the thread's frame)
