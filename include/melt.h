@@ -69,6 +69,9 @@ typedef enum {
     MELT_OPT_INPUT_SCALE_LOG2 = 4, /* s in [-24, 24]: samples are multiplied by 2^s before the fp16 split of the
                                       COMPENSATED mode (exact; undone in the epilogue); default 12 */
     MELT_OPT_OUTPUT = 5,           /* melt_output; default LOG */
+    MELT_OPT_OUTPUT_DTYPE = 7,     /* melt_dtype of `out`; default F32.  F16 / BF16 halve the bytes the kernel stores (the Whisper-shaped
+                                      batch is bound by HBM traffic); log-Mel output (n_mfcc == 0, MELT_OUTPUT_LOG, no tap) only */
+    MELT_OPT_LOG_EPS_EXP10 = 8,    /* e in [-30, 0]: the epsilon of MELT_OUTPUT_LN_EPS is 10^e; default -10 */
     MELT_OPT_INPUT_READY = 6       /* 0/1, default 0.  Consecutive forwards on one stream overlap on the device (programmatic
                                       dependent launch: the next forward's blocks start on the SMs the previous kernel has
                                       already vacated).  With 0 a forward waits for the completion of whatever precedes it in
@@ -101,9 +104,17 @@ typedef enum {
 } melt_pad;
 
 typedef enum {
-    MELT_OUTPUT_LOG = 0,  /* log10(max(S, 1e-10)), then the DCT when n_mfcc > 0 */
-    MELT_OUTPUT_POWER = 1 /* S itself (Eq. 4); only with n_mfcc == 0 */
+    MELT_OUTPUT_LOG = 0,    /* log10(max(S, 1e-10)), then the DCT when n_mfcc > 0: the contract form (BASELINE.json north_star) */
+    MELT_OUTPUT_POWER = 1,  /* S itself (Eq. 4); only with n_mfcc == 0 */
+    MELT_OUTPUT_LN_EPS = 2  /* the paper's own form, Eq. (8): ln(S + eps), natural logarithm (PAPER.md:343 measures
+                               in nats), eps = 10^MELT_OPT_LOG_EPS_EXP10 (the paper does not state it); then the DCT when n_mfcc > 0 */
 } melt_output;
+
+typedef enum {
+    MELT_DTYPE_F32 = 0,
+    MELT_DTYPE_F16 = 1,  /* IEEE half, round to nearest even: |error| <= 2^-11 |value| (3.9e-3 at |log10| in [8, 16)) */
+    MELT_DTYPE_BF16 = 2  /* bfloat16, round to nearest even: |error| <= 2^-8 |value| */
+} melt_dtype;
 
 /*
  * melt_plan_create -- builds the analysis frequencies (Eq. 1-2), the window, the window-folded cos/sin basis
@@ -150,10 +161,11 @@ int melt_plan_get_centres(const melt_plan *plan, double *f_hz);
  *   x    device, fp32, [batch, len] contiguous, 4-byte aligned.  When every clip start is 16-byte aligned (x and len*4)
  *        the kernel frames x in place; otherwise one pass first copies the batch into pool scratch at an aligned clip
  *        stride (see "Conventions");
- *   out  device, fp32, batch * C * T floats, T = melt_num_frames(plan, len), layout per MELT_OPT_LAYOUT.
+ *   out  device, batch * C * T elements of MELT_OPT_OUTPUT_DTYPE (fp32 unless set otherwise), T = melt_num_frames(plan, len),
+ *        layout per MELT_OPT_LAYOUT; aligned to its element size.
  * batch == 0 or T == 0 is a successful no-op.  Returns a melt_status.
  */
-int melt_forward(const melt_plan *plan, const float *x, int batch, long long len, float *out, void *stream);
+int melt_forward(const melt_plan *plan, const float *x, int batch, long long len, void *out, void *stream);
 
 /*
  * melt_forward_host -- melt_forward on HOST buffers: x_host [batch, len] in, out_host (batch * C * T floats, layout per
@@ -164,20 +176,20 @@ int melt_forward(const melt_plan *plan, const float *x, int batch, long long len
  * or reusing x_host.  The call itself returns without waiting.  Pinned (page-locked) host buffers are needed for the copies
  * to be asynchronous.  Device copies of x and out come from the plan's scratch pool (see "Conventions").
  */
-int melt_forward_host(const melt_plan *plan, const float *x_host, int batch, long long len, float *out_host, void *stream);
+int melt_forward_host(const melt_plan *plan, const float *x_host, int batch, long long len, void *out_host, void *stream);
 
 /*
  * melt_forward_ragged -- the whole hot path on clips packed back to back (configs[3]).
  *   x                  device, fp32, packed samples;
  *   offsets            device, int64, n_clips + 1 ascending sample offsets into x (clip i = [offsets[i], offsets[i+1]));
- *   out                device, fp32, packed frame-major [sum_i T_i, C]; the caller sizes it from the clip lengths
+ *   out                device, MELT_OPT_OUTPUT_DTYPE (fp32 by default), packed frame-major [sum_i T_i, C]; the caller sizes it from the clip lengths
  *                      (an upper bound is sum_i melt_num_frames(len_i));
  *   out_frame_offsets  device, int64, n_clips + 1: written by the library, frame offset of every clip in `out`
  *                      (out_frame_offsets[n_clips] = total frames).  Must not be NULL.
  * n_clips <= 2^20.  Frame-major layout only.  No host synchronisation: tiles are assigned on the device.
  */
 int melt_forward_ragged(const melt_plan *plan, const float *x, const long long *offsets, int n_clips,
-                        float *out, long long *out_frame_offsets, void *stream);
+                        void *out, long long *out_frame_offsets, void *stream);
 
 /*
  * melt_forward_tap -- as melt_forward / melt_forward_ragged (offsets == NULL selects the dense form, in which

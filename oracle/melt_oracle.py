@@ -143,3 +143,9 @@ def dct_apply(Lmat, n_mfcc):
     if rc:
         raise ValueError("melt_oracle_dct_apply rc=%d" % rc)
     return Cout
+
+
+def ln_eps(P, eps=1e-10):
+    """Eq. (8) as printed: ln(S + eps), natural logarithm (PAPER.md:343 measures in nats), from the oracle's fp64
+    S.  The paper does not state eps (reading R2); the CUDA path's default is 1e-10."""
+    return np.log(np.asarray(P, np.float64) + float(eps))

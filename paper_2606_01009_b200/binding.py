@@ -14,11 +14,12 @@ MELT_OK, MELT_ERR_INVALID_ARG, MELT_ERR_UNSUPPORTED, MELT_ERR_ALIGNMENT, MELT_ER
 MELT_WINDOW_HANN_PERIODIC, MELT_WINDOW_HANN_SYMMETRIC, MELT_WINDOW_RECT = 0, 1, 2
 MELT_MEL_HTK, MELT_MEL_SLANEY = 0, 1
 MELT_OPT_LAYOUT, MELT_OPT_PRECISION, MELT_OPT_DROP_LAST, MELT_OPT_PAD, MELT_OPT_INPUT_SCALE_LOG2, MELT_OPT_OUTPUT, \
-    MELT_OPT_INPUT_READY = range(7)
+    MELT_OPT_INPUT_READY, MELT_OPT_OUTPUT_DTYPE, MELT_OPT_LOG_EPS_EXP10 = range(9)
 MELT_LAYOUT_FRAME_MAJOR, MELT_LAYOUT_FEATURE_MAJOR = 0, 1
 MELT_PREC_COMPENSATED, MELT_PREC_TF32, MELT_PREC_BF16 = 0, 1, 2
 MELT_PAD_NONE, MELT_PAD_REFLECT = 0, 1
-MELT_OUTPUT_LOG, MELT_OUTPUT_POWER = 0, 1
+MELT_OUTPUT_LOG, MELT_OUTPUT_POWER, MELT_OUTPUT_LN_EPS = 0, 1, 2
+MELT_DTYPE_F32, MELT_DTYPE_F16, MELT_DTYPE_BF16 = 0, 1, 2
 
 # every symbol include/melt.h declares (tests/test_abi.py checks the header against this list and the .so) ...
 SYMBOLS = [

@@ -242,7 +242,8 @@ __global__ void __launch_bounds__(NUM_THREADS, 1) melt_fwd_kernel(const __grid_c
                             const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
                             const float praw = fmaf(r, r, im * im);                         // Eq. (4)
                             float v;
-                            if (p.output_power) v = praw * p.out_scale;
+                            if (p.output_power == 1) v = praw * p.out_scale;
+                            else if (p.output_power == 2) v = lg2_ftz(fmaf(praw, p.out_scale, p.ln_eps)) * 0.69314718055994531f;   // ln(S + eps)
                             else v = fmaxf(fmaf(__log2f(praw), kLog10_2, p.out_log10_offset), -10.f);  // Eq. (8), contract form
                             if (p.n_mfcc > 0) {
                                 const float *drow = dct_s + m * p.dct_pitch;

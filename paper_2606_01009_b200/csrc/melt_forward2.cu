@@ -79,23 +79,23 @@ int plan_build_v2(melt_plan *p) {
             // threads read their frames from global memory: every lane of a load touches another 128-byte line, and the L1
             // tag stage, not L2 or DRAM, bounded the kernel at ~3000 cycles per K-step.)
             k.direct = 1; k.stg_slots = 0;
-            k.kslot_bytes = 2 * 32 * (k.kstep + 4) * 4;
+            k.kslot_bytes = 2 * 32 * (4 * k.kstep + 4) * 4;   // forward + mirrored block: 32 frames x (four K-steps + 4 samples)
             for (k.b_slots = std::min(8, k.units);; --k.b_slots) {
                 k.off_stg = (uint32_t)round_up2((int)((uint32_t)k.b_slots * k.unit_b_bytes), 128) + 128;
-                if ((long long)k.off_stg + 24LL * k.kslot_bytes + 128 + dct_bytes + bar_bytes + 256 <= SMEM_BUDGET) break;
+                if ((long long)k.off_stg + 8LL * k.kslot_bytes + 128 + dct_bytes + bar_bytes + 256 <= SMEM_BUDGET) break;
                 if (k.b_slots <= std::min(3, k.units)) return MELT_OK;
             }
             break;
         }
     }
     k.stg_phases = std::max(1, (k.stg_slots + 3) / 4);
-    k.off_dct = (uint32_t)round_up2((int)(k.off_stg + (uint32_t)k.stg_slots * k.slot_bytes + (k.direct ? 24u * k.kslot_bytes : 0u) + 128), 128);
+    k.off_dct = (uint32_t)round_up2((int)(k.off_stg + (uint32_t)k.stg_slots * k.slot_bytes + (k.direct ? 8u * k.kslot_bytes : 0u) + 128), 128);
     k.off_epi = epi_bytes ? k.off_dct + dct_only : 0;
     k.off_bar = (uint32_t)round_up2((int)(k.off_dct + dct_bytes), 128);
     k.smem_bytes = k.off_bar + bar_bytes;
     if (k.smem_bytes > (uint32_t)SMEM_BUDGET) return MELT_OK;
     k.in_scale = k1.in_scale; k.out_scale = k1.out_scale; k.out_log10_offset = k1.out_log10_offset;
-    k.output_power = k1.output_power; k.feature_major = k1.feature_major;
+    k.output_power = k1.output_power; k.feature_major = k1.feature_major; k.ln_eps = k1.ln_eps; k.out_dtype = 0;
 
     // ---- per-unit load table: byte offset of sample n of a frame = ((n div H) * pitch + n mod H) * 4 (floor division)
     auto off_of = [&](int n) -> int {
@@ -201,7 +201,7 @@ int v2_encode_tmap(K2Params &k) {
         CUtensorMap tmd;
         const cuuint64_t gd[3] = {(cuuint64_t)k.n_fft, (cuuint64_t)frows, (cuuint64_t)k.n_clips};
         const cuuint64_t gs[2] = {(cuuint64_t)k.hop * 4u, (cuuint64_t)k.len * 4u};
-        const cuuint32_t bx[3] = {(cuuint32_t)(k.kstep + 4), 32u, 1u};
+        const cuuint32_t bx[3] = {(cuuint32_t)(4 * k.kstep + 4), 32u, 1u};
         const cuuint32_t es[3] = {1u, 1u, 1u};
         if ((gs[0] & 15) || (gs[1] & 15) || gs[1] >= (1ull << 40)) return MELT_OK;
         if (encd(&tmd, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, const_cast<float *>(k.x), gd, gs, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE,

@@ -121,8 +121,29 @@ static __device__ long long *g_melt_trace = nullptr;   // [2 ranks][16 warps][10
 // accumulator is drained by several warps per lane quarter (single accumulator stage: the MMAs of the next tile cannot
 // start before the drain, so the converter warps take their share of it instead of waiting).
 __device__ __forceinline__ void epi_fast_share(uint32_t t_r, uint32_t t_i, int nb, int n_mels, float *optr, long long cstride,
-                                               bool valid, float off, int blk0, int step) {
+                                               bool valid, float off, int blk0, int step, int ot = 0) {
     const float kLog10_2 = 0.30102999566398120f;
+    if (ot != 0) {
+        // 16-bit output (MELT_OPT_OUTPUT_DTYPE): optr / cstride count 2-byte elements; fp16 or bf16, round to nearest even
+        unsigned short *o16 = reinterpret_cast<unsigned short *>(optr);
+        for (int c0 = 16 * blk0; c0 < nb; c0 += 16 * step) {
+            uint32_t vr[16], vi[16];
+            tmem_ld16(t_r + (uint32_t)c0, vr);
+            tmem_ld16(t_i + (uint32_t)c0, vi);
+            tmem_wait_ld();
+            const int nrem = n_mels - c0;
+            unsigned short *o = o16 + (long long)c0 * cstride;
+#pragma unroll
+            for (int c = 0; c < 16; ++c) {
+                const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                const float v = fmaxf(fmaf(lg2_ftz(fmaf(r, r, im * im)), kLog10_2, off), -10.f);
+                const unsigned short bits = ot == 1 ? __half_as_ushort(__float2half_rn(v)) : __bfloat16_as_ushort(__float2bfloat16_rn(v));
+                if (valid && c < nrem) *o = bits;
+                o += cstride;
+            }
+        }
+        return;
+    }
     for (int c0 = 16 * blk0; c0 < nb; c0 += 16 * step) {
         uint32_t vr[16], vi[16];
         tmem_ld16(t_r + (uint32_t)c0, vr);
@@ -177,7 +198,8 @@ __device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uin
                     const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
                     const float praw = fmaf(r, r, im * im);                                          // Eq. (4)
                     float v;
-                    if (p.output_power) v = praw * p.out_scale;
+                    if (p.output_power == 1) v = praw * p.out_scale;
+                    else if (p.output_power == 2) v = lg2_ftz(fmaf(praw, p.out_scale, p.ln_eps)) * 0.69314718055994531f;   // Eq. (8) as printed: ln(S + eps)
                     else v = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, p.out_log10_offset), -10.f);       // Eq. (8), contract form
                     if (HAS_DCT) {
                         const float *drow = dct_s + m * p.dct_pitch + q0;
@@ -220,6 +242,11 @@ __device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uin
         for (int w = lane; w < n_out; w += 32) warp_out[w] = stage[w];
         __syncwarp();
     }
+}
+
+// Address of output element `idx` (elements of 4 bytes, or of 2 bytes with a 16-bit MELT_OPT_OUTPUT_DTYPE).
+__device__ __forceinline__ float *out_at(const K2Params &p, long long idx) {
+    return p.out_dtype == 0 ? p.out + idx : reinterpret_cast<float *>(reinterpret_cast<unsigned short *>(p.out) + idx);
 }
 
 // Where a 256-frame tile lives: dense batches by division, ragged ones by binary search in the device-side tile prefix.
@@ -281,8 +308,8 @@ __device__ __forceinline__ void load_shifted(uint32_t fb, const short *tb, float
     }
 }
 
-// K-step staging (very long windows): the thread's row of the slot holds samples n0 .. n0 + KS + 3 of its frame (forward block,
-// n0 = a0 + KS u) and run - SIGMA .. run - SIGMA + KS + 3 (mirrored block, `half` bytes further), both 16-byte aligned.
+// K-block staging (very long windows): kb points at samples n0 .. of the thread's frame (forward run of the K-step, n0 = a0 + KS u)
+// and kb + half at run - SIGMA .. (its mirrored run from the aligned sample below it), both 16-byte aligned, KS + 4 samples each.
 template <int KS, int SIGMA>
 __device__ __forceinline__ void load_kstaged(uint32_t kb, uint32_t half, float (&fw)[KS], float (&bw)[KS]) {
     constexpr int NQ = KS / 4, NB = NQ + (SIGMA > 0 ? 1 : 0);
@@ -366,7 +393,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         mbar_init(BAR(V_INFO + lane), 1u);   // 32 = 8 tile phases x 4 lane quarters: chunk info published (ragged batches)
         if (lane < 24) {                      // K-step staging: two slots per converter warp (4 quarters x up to 3 groups)
             mbar_init(BAR(V_KFULL + lane), 1u);
-            mbar_init(BAR(V_KEMPTY + lane), 1u);
+            mbar_init(BAR(V_KEMPTY + lane), (uint32_t)NG);   // every converter group of the quarter releases every block
         }
         fence_barrier_init();
     } else if (warp == W_MMA || warp == W_MMA2) {
@@ -415,29 +442,31 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     TRACE_DECL
     TRACE(1);
     if (warp == W_LOAD && DIRECT) {
-        // K-step staging (windows too long for staged 32-frame chunks): lane (3 q + g) of this warp feeds converter warp (q, g):
-        // for each of its K-steps u = g, g + NG, ... one box with the forward run and one with the mirrored run -- (KS + 4)
-        // samples of the warp's 32 frames, rows one hop apart in the signal -- into the warp's own two-slot ring.  Twelve lanes
-        // run their (identical-length) sequences side by side, so a wait for a free slot is shared by twelve copies.
+        // K-block staging (windows too long for staged 32-frame chunks): lane q of this warp feeds the converter warps of lane
+        // quarter q: per block of four K-steps one box with the forward runs and one with the mirrored runs -- (4 KS + 4)
+        // consecutive samples of the quarter's 32 frames each, rows one hop apart in the signal -- into the quarter's two-slot
+        // ring.  Four K-steps per box because the tensor-map engine pays per ROW: boxes of a single K-step (80-byte rows) held
+        // the kernel at ~1000 cycles per K-step.  Every converter group has a K-step in every block (four consecutive K-steps
+        // cover all residues mod 2 and mod 3), so every warp of the quarter waits for -- and releases -- every block.
         if constexpr (!RAGGED) {
-            const int lq = lane / 3, lg = lane - 3 * lq;           // lane quarter and converter group this lane feeds
-            const bool active = lane < 12 && lg < NG;
+            const bool active = lane < 4;
             if (lane == 0) tma_prefetch_desc(p.tmap);
             int kslot = 0;
             uint32_t kph = 0;
             const uint32_t ring0 = sbase + p.off_stg + (uint32_t)(lane * 2) * (uint32_t)p.kslot_bytes;
             const uint32_t half = (uint32_t)p.kslot_bytes >> 1;
+            const int nblk = (p.units + 3) >> 2;
             for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
                 Tile2 ti;
                 get_tile2<false>(p, tile, ti);
-                const int r0 = ti.t0 + (int)rank * 128 + 32 * lq;   // first frame of the quarter (rows beyond the clip are zero-filled)
-                for (int u = lg; u < p.units; u += NG) {
+                const int r0 = ti.t0 + (int)rank * 128 + 32 * lane;   // first frame of the quarter (rows beyond the clip are zero-filled)
+                for (int kb = 0; kb < nblk; ++kb) {
                     if (active) {
                         mbar_wait(BAR(V_KEMPTY + 2 * lane + kslot), kph ^ 1u);
                         const uint32_t full = BAR(V_KFULL + 2 * lane + kslot), dst = ring0 + (uint32_t)kslot * (uint32_t)p.kslot_bytes;
                         mbar_arrive_expect_tx(full, (uint32_t)p.kslot_bytes);
-                        tma_load_3d(dst, p.tmap, p.a0 + KS * u, r0, ti.clip, full);                                  // samples a0 + KS u ..
-                        tma_load_3d(dst + half, p.tmap, p.b0 - KS * u - (KS - 1) - SIGMA, r0, ti.clip, full);      // the mirrored run, from its aligned start
+                        tma_load_3d(dst, p.tmap, p.a0 + KS * 4 * kb, r0, ti.clip, full);                                       // samples a0 + KS (4 kb) ..
+                        tma_load_3d(dst + half, p.tmap, p.b0 - KS * (4 * kb + 3) - (KS - 1) - SIGMA, r0, ti.clip, full);    // the mirrored runs of K-steps 4 kb + 3 .. 4 kb
                         if (++kslot == 2) { kslot = 0; kph ^= 1u; }
                     }
                 }
@@ -959,9 +988,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         // after its second K-step of the next tile, so that the MMAs find operands waiting when the drain releases them.
         int pend_tile = -1, pend_tl = 0, dstage = 0;
         int tl = 0;   // tiles of this CTA so far
-        // K-step staging (DIRECT): this warp's two-slot ring, fed by lane 3 q + g of the loader warp
-        const int kidx = 2 * (3 * q + g);
-        const uint32_t kring = sbase + p.off_stg + (uint32_t)kidx * (uint32_t)p.kslot_bytes + (uint32_t)lane * (uint32_t)((KS + 4) * 4);
+        // K-block staging (DIRECT): the two-slot ring of this lane quarter, fed by lane q of the loader warp; a row = 4 KS + 4 samples
+        const int kidx = 2 * q;
+        const uint32_t kring = sbase + p.off_stg + (uint32_t)kidx * (uint32_t)p.kslot_bytes + (uint32_t)lane * (uint32_t)((4 * KS + 4) * 4);
+        int cur_blk = -1;
         int kslot = 0;
         uint32_t kph = 0;
         uint32_t dph = 0;
@@ -978,14 +1008,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 dt.T = 0;                                                                                        \
                 dc_off = (p.passes > 1 ? pend_tile % p.passes : 0) * p.nb;                                       \
                 dvalid = lane < ci.nvalid;                                                                       \
-                doptr = p.out + (ci.row0 + lane) * p.n_ch + dc_off;                                              \
+                doptr = out_at(p, (ci.row0 + lane) * p.n_ch + dc_off);                                           \
             } else {                                                                                             \
                 get_tile2<false>(p, pend_tile, dt);                                                              \
                 const int drow = q * 32 + lane, dt0 = dt.t0 + (int)rank * 128;                                   \
                 dvalid = (long long)(dt0 + drow) < dt.T;                                                         \
                 dc_off = dt.pass * p.nb;                                                                         \
-                doptr = p.feature_major ? p.out + ((long long)dt.clip * p.n_ch + dc_off) * dt.T + dt0 + drow     \
-                                        : p.out + (dt.f0 + dt0 + drow) * p.n_ch + dc_off;                        \
+                doptr = p.feature_major ? out_at(p, ((long long)dt.clip * p.n_ch + dc_off) * dt.T + dt0 + drow)  \
+                                        : out_at(p, (dt.f0 + dt0 + drow) * p.n_ch + dc_off);                     \
             }                                                                                                    \
             const int dnm = p.n_mels - dc_off < p.nb ? p.n_mels - dc_off : p.nb;                                 \
             mbar_wait(BAR(V_ACC_FULL + dstage), dph);                                                            \
@@ -993,7 +1023,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             tc_fence_after();                                                                                    \
             const uint32_t dtr = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)dstage * (uint32_t)p.acc_cols; \
             epi_fast_share(dtr, dtr + (uint32_t)p.nb, p.nb, dnm, doptr, p.feature_major ? dt.T : 1, dvalid,      \
-                           p.out_log10_offset, DRAIN0 + g, DRAINERS);                                            \
+                           p.out_log10_offset, DRAIN0 + g, DRAINERS, p.out_dtype);                               \
             tc_fence_before();                                                                                   \
             __syncwarp();                                                                                        \
             if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)dstage * 8u);                         \
@@ -1010,6 +1040,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 const int ug0 = tl * p.units + g;
                 aslot = ug0 % p.a_slots;
                 aph = (uint32_t)((ug0 / p.a_slots) & 1);
+                cur_blk = -1;
             } else {
                 mbar_wait(BAR(V_STG_FULL + sbar), sph);
             }
@@ -1022,11 +1053,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             // folded (its samples are in registers), not after the operand store and its hand-off.
 #define STG_RELEASE_IF_LAST()                                                                       \
             do {                                                                                    \
-                if (DIRECT) {   /* K-step staging: the slot of this K-step goes back to the loader */   \
-                    __syncwarp();                                                                   \
-                    if (lane == 0) mbar_arrive(BAR(V_KEMPTY + kidx + kslot));                       \
-                    if (++kslot == 2) { kslot = 0; kph ^= 1u; }                                     \
-                } else if (u + NG >= p.units) {                                                     \
+                if (!DIRECT && u + NG >= p.units) {                                                 \
                     __syncwarp();                                                                   \
                     if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sbar));                            \
                     released = true;                                                                \
@@ -1041,9 +1068,20 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 TRACE(42);
                 const short *tb = p.tab[DIRECT ? 0 : u];
                 float fw[KS], bw[KS];
-                if constexpr (DIRECT) {     // K-step staging: this K-step's two runs wait in the warp's own ring
-                    mbar_wait(BAR(V_KFULL + kidx + kslot), kph);
-                    load_kstaged<KS, SIGMA>(kring + (uint32_t)kslot * (uint32_t)p.kslot_bytes, (uint32_t)p.kslot_bytes >> 1, fw, bw);
+                if constexpr (DIRECT) {     // K-block staging: the runs of this K-step lie in the block's slot of the quarter's ring
+                    const int kb = u >> 2;
+                    while (cur_blk < kb) {   // warp-uniform: move on to the block of this K-step (every block is waited for and released)
+                        if (cur_blk >= 0) {
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(BAR(V_KEMPTY + kidx + kslot));
+                            if (++kslot == 2) { kslot = 0; kph ^= 1u; }
+                        }
+                        ++cur_blk;
+                        mbar_wait(BAR(V_KFULL + kidx + kslot), kph);
+                    }
+                    const uint32_t kbase = kring + (uint32_t)kslot * (uint32_t)p.kslot_bytes;
+                    const uint32_t off_f = (uint32_t)((u - 4 * kb) * KS * 4), off_b = ((uint32_t)p.kslot_bytes >> 1) + (uint32_t)((4 * kb + 3 - u) * KS * 4);
+                    load_kstaged<KS, SIGMA>(kbase + off_f, off_b - off_f, fw, bw);
                 } else if (RAGGED && dlt != 0) {   // warp-uniform: one misalignment per chunk
                     if (dlt == 1) load_shifted<KS, SIGMA, 1>(fb, tb, fw, bw);
                     else if (dlt == 2) load_shifted<KS, SIGMA, 2>(fb, tb, fw, bw);
@@ -1142,6 +1180,17 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 while (aslot >= p.a_slots) { aslot -= p.a_slots; aph ^= 1u; }
             }
             u -= p.units;   // position in the next tile
+            if constexpr (DIRECT) {   // the blocks of this tile this warp had no K-step in (a partial last block), and the last one held
+                const int nblk = (p.units + 3) >> 2;
+                while (cur_blk < nblk) {
+                    if (cur_blk >= 0) {
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(BAR(V_KEMPTY + kidx + kslot));
+                        if (++kslot == 2) { kslot = 0; kph ^= 1u; }
+                    }
+                    if (++cur_blk < nblk) mbar_wait(BAR(V_KFULL + kidx + kslot), kph);
+                }
+            }
             if (!DIRECT && !released) {   // a group without K-steps in this geometry
                 __syncwarp();
                 if (lane == 0) mbar_arrive(BAR(V_STG_EMPTY + sbar));

@@ -129,7 +129,8 @@ int plan_build_device(melt_plan *p) {
     k.in_scale = (float)std::ldexp(1.0, s_in);
     k.out_scale = (float)std::ldexp(1.0, -2 * (s_in + s_b));
     k.out_log10_offset = (float)(-2.0 * (s_in + s_b) * std::log10(2.0));
-    k.output_power = p->output == MELT_OUTPUT_POWER;
+    k.output_power = p->output;   // melt_output
+    k.ln_eps = (float)std::pow(10.0, (double)p->eps_exp10);
     k.pad = p->pad; k.drop_last = p->drop_last; k.feature_major = p->layout == MELT_LAYOUT_FEATURE_MAJOR;
 
     // ---- staging offset table: for folded index j, where samples a0 + j and b0 - j of a frame live in a staging slot
@@ -216,10 +217,11 @@ int plan_build_device(melt_plan *p) {
     return plan_build_v2(p);   // the CTA-pair kernel takes the geometries it covers; this kernel stays the general path
 }
 
-static int validate_common(const melt_plan *p, const float *x, float *out) {
+static int validate_common(const melt_plan *p, const float *x, void *out) {
     if (!p) return fail(MELT_ERR_INVALID_ARG, "plan is NULL");
     if (!x || !out) return fail(MELT_ERR_INVALID_ARG, "x / out is NULL");
-    if (((uintptr_t)x & 3) || ((uintptr_t)out & 3)) return fail(MELT_ERR_ALIGNMENT, "x / out must be 4-byte aligned");
+    const uintptr_t omask = p->out_dtype == MELT_DTYPE_F32 ? 3 : 1;
+    if (((uintptr_t)x & 3) || ((uintptr_t)out & omask)) return fail(MELT_ERR_ALIGNMENT, "x must be 4-byte aligned, out aligned to its element size");
     int dev = -1;
     MELT_CUDA(cudaGetDevice(&dev));
     if (dev != p->device) return fail(MELT_ERR_INVALID_ARG, "plan was created on device %d, current device is %d", p->device, dev);
@@ -238,9 +240,13 @@ static int scratch_alloc(const melt_plan *p, void **ptr, size_t bytes, cudaStrea
 }
 
 static int forward_impl(const melt_plan *p, const float *x, const long long *offsets, int n_clips, long long len,
-                        float *out, float *tap, long long *out_frame_offsets, void *stream, bool input_ready) {
-    int rc = validate_common(p, x, out);
+                        void *out_any, float *tap, long long *out_frame_offsets, void *stream, bool input_ready) {
+    int rc = validate_common(p, x, out_any);
     if (rc) return rc;
+    float *out = static_cast<float *>(out_any);   // 16-bit outputs: the CTA-pair kernel addresses it in bytes
+    const bool out16 = p->out_dtype != MELT_DTYPE_F32;
+    if (out16 && (p->n_mfcc > 0 || p->output != MELT_OUTPUT_LOG || tap))
+        return fail(MELT_ERR_UNSUPPORTED, "16-bit output: log-Mel output (n_mfcc == 0, MELT_OUTPUT_LOG, no tap) only");
     if (n_clips < 0) return fail(MELT_ERR_INVALID_ARG, "negative clip count");
     if (tap && ((uintptr_t)tap & 3)) return fail(MELT_ERR_ALIGNMENT, "logmel must be 4-byte aligned");
     p->used.store(true, std::memory_order_relaxed);
@@ -267,6 +273,7 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
             k2.tiles_per_clip = 0; k2.n_tiles = -1;
             k2.offsets = offsets; k2.frame_offsets = out_frame_offsets; k2.tile_prefix = tile_prefix;
             k2.vpad = reflect ? p->n_fft / 2 : 0;
+            k2.out_dtype = p->out_dtype;
             k2.input_ready = 0;   // the scan kernel just ahead in the stream produces what the kernel reads at its entry
             if (rc == MELT_OK && v2_encode_tmap_ragged(k2) == MELT_OK && k2.tma_rows > 0) {
                 rc = launch_forward2(p, k2, st);
@@ -274,6 +281,7 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
                 return rc;
             }
         }
+        if (rc == MELT_OK && out16) rc = fail(MELT_ERR_UNSUPPORTED, "16-bit output needs the CTA-pair kernel (hop %% 4 == 0, 16-byte aligned x, staged window)");
         if (rc == MELT_OK) rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, tile_prefix, TILE_M, st);
         kp.offsets = offsets; kp.frame_offsets = out_frame_offsets; kp.tile_prefix = tile_prefix;
         kp.len = 0; kp.frames_per_clip = 0; kp.tiles_per_clip = 0; kp.n_tiles = -1;
@@ -316,6 +324,7 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
         const long long tpc2 = (T + 255) / 256;
         if (tpc2 * n_clips * std::max(1, p->k2.passes) > 0x7fffffffLL) { if (scratch) cudaFreeAsync(scratch, st); return fail(MELT_ERR_UNSUPPORTED, "too many tiles"); }
         k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = len; k2.frames_per_clip = T;
+        k2.out_dtype = p->out_dtype;
         k2.tiles_per_clip = (int)tpc2; k2.n_tiles = (int)(tpc2 * n_clips);
         k2.offsets = nullptr; k2.frame_offsets = nullptr; k2.tile_prefix = nullptr;
         v2_encode_tmap(k2);
@@ -328,6 +337,7 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
         x = x_caller;
         len = len_caller;
     }
+    if (out16) return fail(MELT_ERR_UNSUPPORTED, "16-bit output needs the CTA-pair kernel (hop %% 4 == 0, n_fft with an aligned fold)");
     kp.offsets = nullptr; kp.frame_offsets = nullptr; kp.tile_prefix = nullptr;
     kp.len = len; kp.frames_per_clip = T; kp.tiles_per_clip = (int)tpc; kp.n_tiles = (int)(tpc * n_clips);
     return launch_forward(p, kp, st);
@@ -362,7 +372,7 @@ extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window
     p->fs = fs; p->fmin = fmin; p->fmax = fmax; p->n_fft = n_fft; p->hop = hop; p->window = window; p->n_mels = n_mels;
     p->mel_scale = mel_scale; p->n_mfcc = n_mfcc;
     p->layout = MELT_LAYOUT_FRAME_MAJOR; p->precision = MELT_PREC_COMPENSATED; p->drop_last = 0; p->pad = MELT_PAD_NONE;
-    p->in_scale_log2 = 12; p->output = MELT_OUTPUT_LOG; p->input_ready = 0; p->used.store(false); p->device = dev; p->sm_count = prop.multiProcessorCount;
+    p->in_scale_log2 = 12; p->output = MELT_OUTPUT_LOG; p->input_ready = 0; p->out_dtype = MELT_DTYPE_F32; p->eps_exp10 = -10; p->used.store(false); p->device = dev; p->sm_count = prop.multiProcessorCount;
     p->d_bimg = nullptr; p->d_bimg2 = nullptr; p->v2_ok = false; p->v2_sigma = 0; p->d_tab = nullptr; p->d_dct = nullptr;
     p->pool = nullptr; p->copy_in = nullptr; p->copy_out = nullptr;
     memset(&p->kp, 0, sizeof(p->kp));
@@ -425,9 +435,16 @@ extern "C" int melt_plan_set_option(melt_plan *p, int key, int value) {
             if (value < -24 || value > 24) return fail(MELT_ERR_INVALID_ARG, "bad input scale %d", value);
             p->in_scale_log2 = value; break;
         case MELT_OPT_OUTPUT:
-            if (value < 0 || value > 1) return fail(MELT_ERR_INVALID_ARG, "bad output %d", value);
+            if (value < 0 || value > 2) return fail(MELT_ERR_INVALID_ARG, "bad output %d", value);
             if (value == MELT_OUTPUT_POWER && p->n_mfcc > 0) return fail(MELT_ERR_INVALID_ARG, "power output needs n_mfcc == 0");
             p->output = value; break;
+        case MELT_OPT_OUTPUT_DTYPE:
+            if (value < 0 || value > 2) return fail(MELT_ERR_INVALID_ARG, "bad output dtype %d", value);
+            p->out_dtype = value;
+            return MELT_OK;   // checked against the other options at the forward call
+        case MELT_OPT_LOG_EPS_EXP10:
+            if (value < -30 || value > 0) return fail(MELT_ERR_INVALID_ARG, "bad eps exponent %d", value);
+            p->eps_exp10 = value; break;
         case MELT_OPT_INPUT_READY:
             if (value < 0 || value > 1) return fail(MELT_ERR_INVALID_ARG, "bad input_ready %d", value);
             p->input_ready = value;
@@ -469,23 +486,27 @@ extern "C" int melt_plan_get_centres(const melt_plan *p, double *f_hz) {
 
 extern "C" const char *melt_plan_describe(const melt_plan *p) { return p ? p->desc.c_str() : ""; }
 
-extern "C" int melt_forward(const melt_plan *p, const float *x, int batch, long long len, float *out, void *stream) {
+extern "C" int melt_forward(const melt_plan *p, const float *x, int batch, long long len, void *out, void *stream) {
     return forward_impl(p, x, nullptr, batch, len, out, nullptr, nullptr, stream, p && p->input_ready);
 }
 
 // Host buffers: the batch is cut into groups of clips; upload of group k + 1 (copy_in stream), kernel of group k (the caller's
 // stream) and download of group k - 1 (copy_out stream) overlap.  PCIe is full duplex, so the call costs about
 // max(upload, download) + one group's worth of the other two stages instead of their sum.
-extern "C" int melt_forward_host(const melt_plan *p, const float *x_host, int batch, long long len, float *out_host, void *stream) {
+extern "C" int melt_forward_host(const melt_plan *p, const float *x_host, int batch, long long len, void *out_host_any, void *stream) {
     if (!p) return fail(MELT_ERR_INVALID_ARG, "plan is NULL");
     if (batch < 0 || len < 0) return fail(MELT_ERR_INVALID_ARG, "negative batch / len");
     const long long T = frames_for(p, len);
     if (batch == 0 || T == 0) return MELT_OK;
-    if (!x_host || !out_host) return fail(MELT_ERR_INVALID_ARG, "x_host / out_host is NULL");
+    if (!x_host || !out_host_any) return fail(MELT_ERR_INVALID_ARG, "x_host / out_host is NULL");
     int dev = -1;
     MELT_CUDA(cudaGetDevice(&dev));
     if (dev != p->device) return fail(MELT_ERR_INVALID_ARG, "plan was created on device %d, current device is %d", p->device, dev);
-    const size_t clip_in = (size_t)len, clip_out = (size_t)T * (size_t)p->kp.n_ch;
+    // device / host output copies are handled in units of 4 bytes: a clip of 16-bit outputs must be a whole number of them
+    const size_t esize = p->out_dtype == MELT_DTYPE_F32 ? 4 : 2;
+    if (((size_t)T * (size_t)p->kp.n_ch * esize) & 3) return fail(MELT_ERR_UNSUPPORTED, "melt_forward_host: 16-bit output needs an even number of elements per clip");
+    float *out_host = static_cast<float *>(out_host_any);
+    const size_t clip_in = (size_t)len, clip_out = (size_t)T * (size_t)p->kp.n_ch * esize / 4;
     cudaStream_t st = (cudaStream_t)stream;
     float *ws_in = nullptr, *ws_out = nullptr;
     int rc = scratch_alloc(p, (void **)&ws_in, (size_t)batch * clip_in * sizeof(float), st);
@@ -539,7 +560,7 @@ extern "C" int melt_forward_host(const melt_plan *p, const float *x_host, int ba
     if (e != cudaSuccess) return cuda_fail(e, "melt_forward_host pipeline");
     return MELT_OK;
 }
-extern "C" int melt_forward_ragged(const melt_plan *p, const float *x, const long long *offsets, int n_clips, float *out,
+extern "C" int melt_forward_ragged(const melt_plan *p, const float *x, const long long *offsets, int n_clips, void *out,
                                    long long *out_frame_offsets, void *stream) {
     if (!offsets) return fail(MELT_ERR_INVALID_ARG, "offsets is NULL");
     return forward_impl(p, x, offsets, n_clips, 0, out, nullptr, out_frame_offsets, stream, false);

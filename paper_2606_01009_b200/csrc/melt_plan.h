@@ -37,7 +37,8 @@ struct KParams {
     int dct_pitch;                         // floats per Mel bin in the DCT table (n_mfcc rounded up to 16)
     // ---- numerics
     float in_scale, out_scale, out_log10_offset;
-    int output_power;
+    int output_power;                      // melt_output: 0 log10 clamp, 1 power, 2 ln(S + eps)
+    float ln_eps;                          // MELT_OUTPUT_LN_EPS: eps
     // ---- batch
     const float *x;
     float *out, *tap;
@@ -85,7 +86,9 @@ struct K2Params {
     uint32_t off_epi;          // MFCCT, frame-major: per epilogue warp 32 x n_mfcc floats to transpose the cepstra for coalesced stores (0 = none)
     int dct_pitch;
     float in_scale, out_scale, out_log10_offset;
-    int output_power, feature_major;
+    int output_power, feature_major;   // output_power: melt_output (0 log10 clamp, 1 power, 2 ln(S + eps))
+    float ln_eps;              // MELT_OUTPUT_LN_EPS: eps
+    int out_dtype;             // melt_dtype of `out` (16-bit forms: plain log-Mel only; `out` is then addressed in bytes)
     // ---- batch (dense)
     const float *x;
     float *out, *tap;
@@ -119,7 +122,7 @@ struct K2Params {
 struct melt_plan {
     double fs, fmin, fmax;
     int n_fft, hop, window, n_mels, mel_scale, n_mfcc;
-    int layout, precision, drop_last, pad, in_scale_log2, output, input_ready;
+    int layout, precision, drop_last, pad, in_scale_log2, output, input_ready, out_dtype, eps_exp10;
     mutable std::atomic<bool> used;    // set by the first forward call: options are frozen from then on
     int device, sm_count;
     std::vector<double> centres, win;

@@ -333,3 +333,14 @@ def test_batch_and_ragged_wrappers():
     np.testing.assert_array_equal(rag["C"][5:12], single["C"])
     dense = orc.forward_batch(np.stack([xs[0], xs[0][::-1].copy()]), **kw)
     assert dense["P"].shape == (2, 4, 40)
+
+
+def test_ln_eps_form_closed_values():
+    """Eq. (8) as printed, ln(S + eps): an on-bin tone of amplitude 0.5 gives S = (A N / 4)^2 = 2500 (pin P3) -> ln(2500 + eps);
+    silence gives ln(eps); and the two log forms are tied by ln(S) = ln(10) log10(S) wherever eps is negligible."""
+    from oracle import melt_oracle as orc
+    np.testing.assert_allclose(orc.ln_eps(np.array([2500.0, 0.0]), 1e-10), [np.log(2500.0 + 1e-10), np.log(1e-10)], rtol=0, atol=1e-15)
+    x = (0.5 * np.cos(2 * np.pi * 35 * np.arange(400) / 400.0 + 0.3)).astype(np.float32)
+    ref = orc.forward(x, fs=16000.0, n_fft=400, hop=160, window_kind=0, n_mels=1, fmin=0.0, fmax=5600.0, want=("P", "L"))
+    np.testing.assert_allclose(orc.ln_eps(ref["P"])[0, 0], np.log(2500.0), atol=1e-6)
+    np.testing.assert_allclose(orc.ln_eps(ref["P"]), np.log(10.0) * ref["L"], atol=1e-9)
