@@ -51,6 +51,13 @@ def lib():
     path = _build.LIB
     if not os.path.exists(path) or _build._stale():
         path = _build.build()
+    _lib = load(path)
+    return _lib
+
+
+def load(path):
+    """ctypes handle of a library build at `path` with every prototype declared (lib() uses it for the product library; tests
+    load variant builds next to it)."""
     L = C.CDLL(path)
     vp, ip, ll, dbl = C.c_void_p, C.c_int, C.c_longlong, C.c_double
     L.melt_plan_create.restype = vp
@@ -75,7 +82,6 @@ def lib():
     L.melt_selftest_umma.argtypes = [ip, ip, ip, vp, vp, vp]
     L.melt_selftest_umma2.argtypes = [ip, ip, ip, vp, vp, vp]
     L.melt_selftest_poison_smem.argtypes = [vp]
-    _lib = L
     return L
 
 

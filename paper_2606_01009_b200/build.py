@@ -34,12 +34,13 @@ def _stale():
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False, extra=()) -> str:
-    """Compile every .cu under csrc/ for sm_100a and link libmelt_b200.so.  Returns the library path."""
-    if not force and not _stale():
+def build(force: bool = False, verbose: bool = False, extra=(), out_path: str = None, objdir: str = None) -> str:
+    """Compile every .cu under csrc/ for sm_100a and link libmelt_b200.so.  Returns the library path.
+    out_path / objdir: build a VARIANT (extra compile flags, e.g. -DMELT_STRICT_CLUSTER_SYNC) somewhere else, leaving the library alone."""
+    if out_path is None and not force and not _stale():
         return LIB
     nvcc = _nvcc()
-    objdir = os.path.join(HERE, "build")
+    objdir = objdir or os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)
     objs = []
     procs = []
@@ -54,10 +55,11 @@ def build(force: bool = False, verbose: bool = False, extra=()) -> str:
             print(out)
         if pr.returncode != 0:
             raise RuntimeError("nvcc failed: %s\n%s" % (" ".join(cmd), out))
-    tmp = LIB + ".tmp.%d" % os.getpid()
+    lib = out_path or LIB
+    tmp = lib + ".tmp.%d" % os.getpid()
     subprocess.run([nvcc, "-shared", "-o", tmp] + objs + ["-lcudart"], check=True)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":

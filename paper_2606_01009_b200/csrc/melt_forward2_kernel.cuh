@@ -180,7 +180,10 @@ template <bool HAS_DCT>
 __device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uint32_t t_i, const float *dct_s, float *optr, float *tptr,
                                             long long cstride, bool valid, int lane, uint32_t acc_empty_bar, int nm,
                                             float *stage, float *warp_out, int nvalid) {
-    const float kLog10_2 = 0.30102999566398120f;
+    const bool ln_form = p.output_power == 2;
+    const float la = ln_form ? p.out_scale : 1.f, lb = ln_form ? p.ln_eps : 0.f;
+    const float lc = ln_form ? 0.69314718055994531f : 0.30102999566398120f, ld = ln_form ? 0.f : p.out_log10_offset;
+    const float lmin = ln_form ? -3.0e38f : -10.f;
     const int K = p.n_mfcc;
     for (int q0 = 0; q0 < (HAS_DCT ? K : 1); q0 += 16) {
         float cacc[HAS_DCT ? 16 : 1];
@@ -198,9 +201,11 @@ __device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uin
                     const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
                     const float praw = fmaf(r, r, im * im);                                          // Eq. (4)
                     float v;
+                    // one formula for both log forms (two branches inside the unrolled bin loop cost the ragged MFCCT batch 35 %):
+                    //   contract form (Eq. 8, DESIGN R2): log10(max(S, 1e-10)) = max(lg2(1 * praw + 0) * log10(2) + offset, -10)
+                    //   printed form:                     ln(S + eps)          = max(lg2(scale * praw + eps) * ln(2) + 0, -inf)
                     if (p.output_power == 1) v = praw * p.out_scale;
-                    else if (p.output_power == 2) v = lg2_ftz(fmaf(praw, p.out_scale, p.ln_eps)) * 0.69314718055994531f;   // Eq. (8) as printed: ln(S + eps)
-                    else v = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, p.out_log10_offset), -10.f);       // Eq. (8), contract form
+                    else v = fmaxf(fmaf(lg2_ftz(fmaf(praw, la, lb)), lc, ld), lmin);
                     if (HAS_DCT) {
                         const float *drow = dct_s + m * p.dct_pitch + q0;
 #pragma unroll
@@ -328,15 +333,15 @@ __device__ __forceinline__ void load_kstaged(uint32_t kb, uint32_t half, float (
     for (int e = 0; e < KS; ++e) bw[KS - 1 - e] = wb[SIGMA + e];   // sample `run + e` of the descending run is the partner of pair KS - 1 - e
 }
 
-static_assert(V_NBARS <= V2_THREADS, "one thread per barrier at set-up");
 template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM, bool DIRECT>
-__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
     extern __shared__ __align__(128) uint8_t smem[];
     // Who drains the accumulators: MODE 0 the four epilogue warps alone; MODE 1 (single accumulator stage, log-Mel) the epilogue
     // warps and the converter warps together; MODE 2 (log-Mel) there are no epilogue warps -- they form a third converter
     // group and every converter warp drains a third of the bins of the previous tile.
     constexpr bool SHARE = MODE != 0;
-    constexpr int NG = MODE == 2 ? V2_CONV_GROUPS + 1 : V2_CONV_GROUPS;   // converter groups
+    constexpr int NG = MODE == 2 ? V2_CONV_GROUPS : V2_CONV_GROUPS - 1;   // converter groups: 3 without epilogue warps, 2 next to them
+    constexpr int NT = v2_threads(MODE);                                  // threads of the block
     constexpr int CONV0 = MODE == 2 ? W_EPI0 : W_CONV0;                   // first converter warp
     constexpr int DRAINERS = MODE == 2 ? NG : 1 + NG;                     // warps per lane quarter that drain (SHARE)
     constexpr int DRAIN0 = MODE == 2 ? 0 : 1;                             // block index of converter group 0's share
@@ -366,7 +371,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
     // up; the two issuer warps set up all other barriers.  The loader joins the cluster barrier by arriving early and waiting
     // at its very end (it needs nothing the barrier publishes).
     constexpr bool EARLY_LOADER = !DIRECT;                       // direct-load form: the loader warp has no work
-    constexpr int SETUP_THREADS = EARLY_LOADER ? V2_THREADS - 32 : V2_THREADS;
+    constexpr int SETUP_THREADS = EARLY_LOADER ? NT - 32 : NT;
     if (warp == W_BASIS) {
         tmem_alloc2(smem_u32(tmem_ptr_s), 512);
         tmem_relinquish2();
@@ -382,7 +387,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
             *reinterpret_cast<float4 *>(smem + p.off_stg + (size_t)s * p.slot_bytes - 256 + 16 * j) = make_float4(0.f, 0.f, 0.f, 0.f);
         fence_proxy_async_smem();  // the zero fill (generic proxy) is ordered before the bulk copies (async proxy) that follow
     }
-    static_assert(13 * 24 <= V2_THREADS - 128, "one thread per 16 bytes of margin");
+    static_assert(13 * 24 <= NT - 128, "one thread per 16 bytes of margin");
     if (warp == W_LOAD) {
         // staging barriers: FULL (one arrival + transaction bytes), EMPTY (one arrival per converter group), READY (ragged)
         if (lane < V2_MAX_STG) {
@@ -407,15 +412,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         fence_barrier_init();
     }
     if (p.n_mfcc > 0)
-        for (int i = tid; i < p.n_mels * p.dct_pitch; i += V2_THREADS) dct_s[i] = __ldg(p.dct + i);
+        for (int i = tid; i < p.n_mels * p.dct_pitch; i += NT) dct_s[i] = __ldg(p.dct + i);
     TRACE_PT(1);
     uint32_t tmem_base = 0;
     if (EARLY_LOADER && warp == W_LOAD) {
         // the loader: margins cleared (named barrier with the clearing warps), its own barriers set up -> start copying
-        asm volatile("bar.sync 1, %0;" ::"n"(V2_THREADS - 96) : "memory");
+        asm volatile("bar.sync 1, %0;" ::"n"(NT - 96) : "memory");
         cluster_arrive_relaxed();
     } else {
-        if (EARLY_LOADER && tid >= 128) asm volatile("bar.arrive 1, %0;" ::"n"(V2_THREADS - 96) : "memory");
+        if (EARLY_LOADER && tid >= 128) asm volatile("bar.arrive 1, %0;" ::"n"(NT - 96) : "memory");
         TRACE_PT(2);
         tc_fence_before();
         asm volatile("bar.sync 2, %0;" ::"n"(SETUP_THREADS) : "memory");   // tensor memory allocated, barriers set up (this CTA)
@@ -865,7 +870,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
         const float kLog10_2 = 0.30102999566398120f;
         int stage = 0;
         uint32_t sph = 0;
-        const bool fast_log = p.n_mfcc == 0 && !p.output_power && p.tap == nullptr;
+        // (plain log-Mel output never comes here: it runs without epilogue warps, MODE 2)
         bool dep_done = false;
         int tl = 0;   // tiles of this CTA so far
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
@@ -916,46 +921,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(V2_THREADS, 1) melt_
                 // single accumulator stage, log-Mel: this warp drains every third 16-bin block, the two converter warps of the
                 // lane quarter the others
                 epi_fast_share(t_r, t_i, p.nb, nm, optr, cstride, valid, p.out_log10_offset, 0, DRAINERS);
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
-            } else if (fast_log) {
-                // log-Mel, no DCT, no tap: the common case.  Whole 16-bin blocks take predicated stores without per-element
-                // bounds tests; the tensor-memory loads of the next block are in flight while this one is computed and stored.
-                float *o = optr;
-                const float off = p.out_log10_offset;
-                const int n_whole = nm & ~15;
-                uint32_t vr[16], vi[16];
-                if (n_whole > 0) { tmem_ld16(t_r, vr); tmem_ld16(t_i, vi); }
-                for (int c0 = 0; c0 < n_whole; c0 += 16) {
-                    float v[16];
-                    tmem_wait_ld();
-#pragma unroll
-                    for (int c = 0; c < 16; ++c) {
-                        const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
-                        v[c] = fmaf(r, r, im * im);                                                          // Eq. (4)
-                    }
-                    if (c0 + 16 < p.nb) { tmem_ld16(t_r + (uint32_t)(c0 + 16), vr); tmem_ld16(t_i + (uint32_t)(c0 + 16), vi); }
-                    if (valid) {
-#pragma unroll
-                        for (int c = 0; c < 16; ++c) {
-                            *o = fmaxf(fmaf(lg2_ftz(v[c]), kLog10_2, off), -10.f);                           // Eq. (8), contract form
-                            o += cstride;
-                        }
-                    }
-                }
-                if (n_whole < p.nb) {   // last, partial block (its loads were issued above, or here when it is the only one)
-                    if (n_whole == 0) { tmem_ld16(t_r, vr); tmem_ld16(t_i, vi); }
-                    tmem_wait_ld();
-                    const int nrem = nm - n_whole;
-#pragma unroll
-                    for (int c = 0; c < 16; ++c) {
-                        const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
-                        const float praw = fmaf(r, r, im * im);
-                        if (valid && c < nrem) *o = fmaxf(fmaf(lg2_ftz(praw), kLog10_2, off), -10.f);
-                        o += cstride;
-                    }
-                }
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
@@ -1249,7 +1214,7 @@ static int launch_one_s(const K2Params &kp, int grid, cudaStream_t stream) {
     // (K2Params::input_ready, MELT_OPT_INPUT_READY).
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid, 1, 1);
-    cfg.blockDim = dim3(V2_THREADS, 1, 1);
+    cfg.blockDim = dim3(v2_threads(MODE), 1, 1);
     cfg.dynamicSmemBytes = kp.smem_bytes;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
