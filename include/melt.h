@@ -106,6 +106,10 @@ typedef enum {
 typedef enum {
     MELT_OUTPUT_LOG = 0,    /* log10(max(S, 1e-10)), then the DCT when n_mfcc > 0: the contract form (BASELINE.json north_star) */
     MELT_OUTPUT_POWER = 1,  /* S itself (Eq. 4); only with n_mfcc == 0 */
+    MELT_OUTPUT_LOG_WHISPER = 3, /* the contract log10 form followed by Whisper's dynamic-range normalisation (PAPER.md:424 configures MelT
+                               "to Whisper's 80-bin log-Mel specification"; the normalisation itself is Whisper's): per clip,
+                               L <- max(L, max_clip(L) - 8), then (L + 4) / 4.  Dense batches, n_mfcc == 0, fp32 output.  Two small
+                               kernels behind the forward kernel (per-clip maximum, rescale in place): two more passes over `out` */
     MELT_OUTPUT_LN_EPS = 2  /* the paper's own form, Eq. (8): ln(S + eps), natural logarithm (PAPER.md:343 measures
                                in nats), eps = 10^MELT_OPT_LOG_EPS_EXP10 (the paper does not state it); then the DCT when n_mfcc > 0 */
 } melt_output;

@@ -149,3 +149,10 @@ def ln_eps(P, eps=1e-10):
     """Eq. (8) as printed: ln(S + eps), natural logarithm (PAPER.md:343 measures in nats), from the oracle's fp64
     S.  The paper does not state eps (reading R2); the CUDA path's default is 1e-10."""
     return np.log(np.asarray(P, np.float64) + float(eps))
+
+
+def whisper_norm(L):
+    """Whisper's dynamic-range normalisation of one clip's log10-Mel matrix L [T, M] (any layout: only the clip maximum enters):
+    L <- max(L, max(L) - 8), then (L + 4) / 4 (PAPER.md:424 configures MelT to Whisper's log-Mel specification)."""
+    L = np.asarray(L, np.float64)
+    return (np.maximum(L, L.max() - 8.0) + 4.0) / 4.0

@@ -18,7 +18,7 @@ MELT_OPT_LAYOUT, MELT_OPT_PRECISION, MELT_OPT_DROP_LAST, MELT_OPT_PAD, MELT_OPT_
 MELT_LAYOUT_FRAME_MAJOR, MELT_LAYOUT_FEATURE_MAJOR = 0, 1
 MELT_PREC_COMPENSATED, MELT_PREC_TF32, MELT_PREC_BF16 = 0, 1, 2
 MELT_PAD_NONE, MELT_PAD_REFLECT = 0, 1
-MELT_OUTPUT_LOG, MELT_OUTPUT_POWER, MELT_OUTPUT_LN_EPS = 0, 1, 2
+MELT_OUTPUT_LOG, MELT_OUTPUT_POWER, MELT_OUTPUT_LN_EPS, MELT_OUTPUT_LOG_WHISPER = 0, 1, 2, 3
 MELT_DTYPE_F32, MELT_DTYPE_F16, MELT_DTYPE_BF16 = 0, 1, 2
 
 # every symbol include/melt.h declares (tests/test_abi.py checks the header against this list and the .so) ...

@@ -59,8 +59,8 @@ int plan_build_v2(melt_plan *p) {
     const uint32_t dct_bytes = dct_only + epi_bytes;
     const uint32_t bar_bytes = (uint32_t)round_up2(V_NBARS * 8 + 16 + 32 * 16, 128);   // barriers, tensor-memory address, chunk records of ragged batches (32 x 16 B)
     k.off_b = 0;
-    // The basis half stays resident when that leaves room for at least five staging slots; otherwise (long windows) its
-    // K-step slabs are streamed from L2 through the deepest ring (<= 8 slabs) that still leaves five slots.
+    // The basis half stays resident when that leaves room for at least five staging slots; otherwise (long windows, > 128 bins) its
+    // K-step slabs are streamed from L2 through a ring of 8 slabs; when five chunk slots do not fit next to that: K-block staging.
     k.b_resident = 1; k.b_slots = k.units;
     if (k.passes > 1) { k.b_resident = 0; k.b_slots = std::min(8, k.units); }   // every pass needs other rows: streamed
     for (;;) {
@@ -69,15 +69,15 @@ int plan_build_v2(melt_plan *p) {
         const long long room = (long long)SMEM_BUDGET - k.off_stg - 128 - dct_bytes - bar_bytes - 256;
         k.stg_slots = (int)std::min<long long>(room > 0 ? room / k.slot_bytes : 0, V2_MAX_STG);
         if (k.stg_slots >= 5) break;
-        if (k.b_resident) { k.b_resident = 0; k.b_slots = std::min(8, k.units); }
-        else --k.b_slots;
-        if (k.b_slots < std::min(3, k.units)) {   // the issuers take two K-steps per iteration: two different slabs at least
-            // Not even a streamed basis leaves room for staged 32-frame chunks (windows of thousands of samples: a chunk is
-            // 32 hops of the signal).  K-STEP STAGING instead: the loader brings, per converter warp and K-step, just the two
-            // runs of kstep (+4) samples of its 32 frames -- one tensor-map box of (kstep + 4) x 32 each, 32 rows one hop apart
-            // -- into a two-slot ring per converter warp (4 lane quarters x 3 groups).  (An earlier version let the converter
-            // threads read their frames from global memory: every lane of a load touches another 128-byte line, and the L1
-            // tag stage, not L2 or DRAM, bounded the kernel at ~3000 cycles per K-step.)
+        if (k.b_resident) { k.b_resident = 0; k.b_slots = std::min(8, k.units); continue; }
+        {
+            // Not even a streamed basis with its full ring leaves room for five staged 32-frame chunks (long windows: a chunk is
+            // 32 hops of the signal).  K-BLOCK STAGING instead: the loader brings, per lane quarter and block of four K-steps, just
+            // the forward and the mirrored runs of its 32 frames -- one tensor-map box of (4 kstep + 4) x 32 samples each, rows one
+            // hop apart -- into a two-slot ring per quarter.  (r01 let the converter threads read their frames from global memory:
+            // every lane of a load touches another 128-byte line, and the L1 tag stage, not L2 or DRAM, bounded the kernel at
+            // ~3000 cycles per K-step.  A shallower basis ring would buy the five chunk slots for 1024-sample windows -- cfg4a ran
+            // that way until r02: 56 us against 46 us with K-block staging.)
             k.direct = 1; k.stg_slots = 0;
             k.kslot_bytes = 2 * 32 * (4 * k.kstep + 4) * 4;   // forward + mirrored block: 32 frames x (four K-steps + 4 samples)
             for (k.b_slots = std::min(8, k.units);; --k.b_slots) {

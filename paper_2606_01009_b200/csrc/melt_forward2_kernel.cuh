@@ -123,6 +123,7 @@ static __device__ long long *g_melt_trace = nullptr;   // [2 ranks][16 warps][10
 __device__ __forceinline__ void epi_fast_share(uint32_t t_r, uint32_t t_i, int nb, int n_mels, float *optr, long long cstride,
                                                bool valid, float off, int blk0, int step, int ot = 0) {
     const float kLog10_2 = 0.30102999566398120f;
+    const bool vec4 = cstride == 1 && ((reinterpret_cast<uintptr_t>(optr) & 15) == 0) && ot == 0;   // (warp-uniform: rows are n_ch * 4 bytes apart)
     if (ot != 0) {
         // 16-bit output (MELT_OPT_OUTPUT_DTYPE): optr / cstride count 2-byte elements; fp16 or bf16, round to nearest even
         unsigned short *o16 = reinterpret_cast<unsigned short *>(optr);
@@ -133,13 +134,27 @@ __device__ __forceinline__ void epi_fast_share(uint32_t t_r, uint32_t t_i, int n
             tmem_wait_ld();
             const int nrem = n_mels - c0;
             unsigned short *o = o16 + (long long)c0 * cstride;
+            unsigned short bits[16];
 #pragma unroll
             for (int c = 0; c < 16; ++c) {
                 const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
                 const float v = fmaxf(fmaf(lg2_ftz(fmaf(r, r, im * im)), kLog10_2, off), -10.f);
-                const unsigned short bits = ot == 1 ? __half_as_ushort(__float2half_rn(v)) : __bfloat16_as_ushort(__float2bfloat16_rn(v));
-                if (valid && c < nrem) *o = bits;
-                o += cstride;
+                bits[c] = ot == 1 ? __half_as_ushort(__float2half_rn(v)) : __bfloat16_as_ushort(__float2bfloat16_rn(v));
+            }
+            if (nrem >= 16 && cstride == 1 && (reinterpret_cast<uintptr_t>(o) & 15) == 0) {   // frame-major rows: two 128-bit stores
+                if (valid) {
+                    uint32_t w[8];
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) w[c] = (uint32_t)bits[2 * c] | ((uint32_t)bits[2 * c + 1] << 16);
+                    reinterpret_cast<uint4 *>(o)[0] = make_uint4(w[0], w[1], w[2], w[3]);
+                    reinterpret_cast<uint4 *>(o)[1] = make_uint4(w[4], w[5], w[6], w[7]);
+                }
+            } else {
+#pragma unroll
+                for (int c = 0; c < 16; ++c) {
+                    if (valid && c < nrem) *o = bits[c];
+                    o += cstride;
+                }
             }
         }
         return;
@@ -151,7 +166,20 @@ __device__ __forceinline__ void epi_fast_share(uint32_t t_r, uint32_t t_i, int n
         tmem_wait_ld();
         const int nrem = n_mels - c0;   // bins of this block that exist
         float *o = optr + (long long)c0 * cstride;
-        if (nrem >= 16) {
+        if (nrem >= 16 && vec4) {
+            // frame-major rows (cstride == 1, 16-byte aligned): the block is 64 contiguous bytes of this thread's row -- four 128-bit
+            // stores fill whole 32-byte sectors (one 4-byte store per bin touches 32 sectors per instruction for 128 useful bytes)
+            if (valid) {
+                float v[16];
+#pragma unroll
+                for (int c = 0; c < 16; ++c) {
+                    const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                    v[c] = fmaxf(fmaf(lg2_ftz(fmaf(r, r, im * im)), kLog10_2, off), -10.f);
+                }
+#pragma unroll
+                for (int c = 0; c < 16; c += 4) *reinterpret_cast<float4 *>(o + c) = make_float4(v[c], v[c + 1], v[c + 2], v[c + 3]);
+            }
+        } else if (nrem >= 16) {
             if (valid) {
 #pragma unroll
                 for (int c = 0; c < 16; ++c) {

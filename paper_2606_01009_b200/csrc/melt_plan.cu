@@ -129,7 +129,7 @@ int plan_build_device(melt_plan *p) {
     k.in_scale = (float)std::ldexp(1.0, s_in);
     k.out_scale = (float)std::ldexp(1.0, -2 * (s_in + s_b));
     k.out_log10_offset = (float)(-2.0 * (s_in + s_b) * std::log10(2.0));
-    k.output_power = p->output;   // melt_output
+    k.output_power = p->output == MELT_OUTPUT_LOG_WHISPER ? MELT_OUTPUT_LOG : p->output;   // melt_output of the forward kernel (the Whisper normalisation is a post-pass)
     k.ln_eps = (float)std::pow(10.0, (double)p->eps_exp10);
     k.pad = p->pad; k.drop_last = p->drop_last; k.feature_major = p->layout == MELT_LAYOUT_FEATURE_MAJOR;
 
@@ -239,6 +239,35 @@ static int scratch_alloc(const melt_plan *p, void **ptr, size_t bytes, cudaStrea
     return MELT_OK;
 }
 
+// ---- MELT_OUTPUT_LOG_WHISPER post-pass: per clip, L <- (max(L, max_clip(L) - 8) + 4) / 4 (any layout: a clip is `per_clip` contiguous floats)
+__device__ __forceinline__ int float_order(float f) { const int i = __float_as_int(f); return i >= 0 ? i : i ^ 0x7fffffff; }   // monotone float -> int
+__global__ void whisper_max_kernel(const float *__restrict__ out, long long per_clip, int *__restrict__ cmax) {
+    const float *o = out + (long long)blockIdx.y * per_clip;
+    float m = -3.0e38f;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < per_clip; i += (long long)gridDim.x * blockDim.x) m = fmaxf(m, __ldg(o + i));
+    for (int d = 16; d > 0; d >>= 1) m = fmaxf(m, __shfl_xor_sync(0xffffffffu, m, d));
+    if ((threadIdx.x & 31) == 0) atomicMax(cmax + blockIdx.y, float_order(m));
+}
+__global__ void whisper_apply_kernel(float *__restrict__ out, long long per_clip, const int *__restrict__ cmax) {
+    float *o = out + (long long)blockIdx.y * per_clip;
+    const int c = cmax[blockIdx.y];
+    const float floor_v = __int_as_float(c >= 0 ? c : c ^ 0x7fffffff) - 8.0f;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < per_clip; i += (long long)gridDim.x * blockDim.x)
+        o[i] = (fmaxf(o[i], floor_v) + 4.0f) * 0.25f;
+}
+static int scratch_alloc(const melt_plan *p, void **ptr, size_t bytes, cudaStream_t st);
+static int whisper_normalise(const melt_plan *p, float *out, int n_clips, long long per_clip, cudaStream_t st) {
+    int *cmax = nullptr;
+    int rc = scratch_alloc(p, (void **)&cmax, sizeof(int) * (size_t)n_clips, st);
+    if (rc) return rc;
+    cudaError_t e = cudaMemsetAsync(cmax, 0x80, sizeof(int) * (size_t)n_clips, st);   // 0x80808080: below the order key of any log10 value
+    const unsigned bx = (unsigned)std::max<long long>(1, std::min<long long>((per_clip + 2047) / 2048, 256));
+    if (e == cudaSuccess) { whisper_max_kernel<<<dim3(bx, (unsigned)n_clips), 256, 0, st>>>(out, per_clip, cmax); e = cudaGetLastError(); }
+    if (e == cudaSuccess) { whisper_apply_kernel<<<dim3(bx, (unsigned)n_clips), 256, 0, st>>>(out, per_clip, cmax); e = cudaGetLastError(); }
+    cudaFreeAsync(cmax, st);
+    return e == cudaSuccess ? MELT_OK : cuda_fail(e, "whisper normalisation");
+}
+
 static int forward_impl(const melt_plan *p, const float *x, const long long *offsets, int n_clips, long long len,
                         void *out_any, float *tap, long long *out_frame_offsets, void *stream, bool input_ready) {
     int rc = validate_common(p, x, out_any);
@@ -247,6 +276,8 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
     const bool out16 = p->out_dtype != MELT_DTYPE_F32;
     if (out16 && (p->n_mfcc > 0 || p->output != MELT_OUTPUT_LOG || tap))
         return fail(MELT_ERR_UNSUPPORTED, "16-bit output: log-Mel output (n_mfcc == 0, MELT_OUTPUT_LOG, no tap) only");
+    const bool whisper = p->output == MELT_OUTPUT_LOG_WHISPER;
+    if (whisper && (offsets || tap)) return fail(MELT_ERR_UNSUPPORTED, "Whisper-normalised output: dense batches without tap only");
     if (n_clips < 0) return fail(MELT_ERR_INVALID_ARG, "negative clip count");
     if (tap && ((uintptr_t)tap & 3)) return fail(MELT_ERR_ALIGNMENT, "logmel must be 4-byte aligned");
     p->used.store(true, std::memory_order_relaxed);
@@ -331,6 +362,7 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
         if (!k2.direct || k2.tma_rows > 0) {   // (K-step staging needs its tensor map; without one the general kernel takes the batch)
             rc = launch_forward2(p, k2, st);
             if (scratch) cudaFreeAsync(scratch, st);
+            if (rc == MELT_OK && whisper) rc = whisper_normalise(p, out, n_clips, (long long)T * p->kp.n_ch, st);
             return rc;
         }
         if (scratch) cudaFreeAsync(scratch, st);   // the general kernel pads / realigns on the fly: give it the caller's batch
@@ -340,7 +372,9 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
     if (out16) return fail(MELT_ERR_UNSUPPORTED, "16-bit output needs the CTA-pair kernel (hop %% 4 == 0, n_fft with an aligned fold)");
     kp.offsets = nullptr; kp.frame_offsets = nullptr; kp.tile_prefix = nullptr;
     kp.len = len; kp.frames_per_clip = T; kp.tiles_per_clip = (int)tpc; kp.n_tiles = (int)(tpc * n_clips);
-    return launch_forward(p, kp, st);
+    rc = launch_forward(p, kp, st);
+    if (rc == MELT_OK && whisper) rc = whisper_normalise(p, out, n_clips, (long long)T * p->kp.n_ch, st);
+    return rc;
 }
 
 }  // namespace melt
@@ -435,8 +469,8 @@ extern "C" int melt_plan_set_option(melt_plan *p, int key, int value) {
             if (value < -24 || value > 24) return fail(MELT_ERR_INVALID_ARG, "bad input scale %d", value);
             p->in_scale_log2 = value; break;
         case MELT_OPT_OUTPUT:
-            if (value < 0 || value > 2) return fail(MELT_ERR_INVALID_ARG, "bad output %d", value);
-            if (value == MELT_OUTPUT_POWER && p->n_mfcc > 0) return fail(MELT_ERR_INVALID_ARG, "power output needs n_mfcc == 0");
+            if (value < 0 || value > 3) return fail(MELT_ERR_INVALID_ARG, "bad output %d", value);
+            if ((value == MELT_OUTPUT_POWER || value == MELT_OUTPUT_LOG_WHISPER) && p->n_mfcc > 0) return fail(MELT_ERR_INVALID_ARG, "power / Whisper-normalised output needs n_mfcc == 0");
             p->output = value; break;
         case MELT_OPT_OUTPUT_DTYPE:
             if (value < 0 || value > 2) return fail(MELT_ERR_INVALID_ARG, "bad output dtype %d", value);
@@ -513,11 +547,14 @@ extern "C" int melt_forward_host(const melt_plan *p, const float *x_host, int ba
     if (rc) return rc;
     rc = scratch_alloc(p, (void **)&ws_out, (size_t)batch * clip_out * sizeof(float), st);
     if (rc) { cudaFreeAsync(ws_in, st); return rc; }
-    // groups of clips: about 4 MB of input each, at most 16 groups
-    int per = (int)std::max<size_t>(1, ((size_t)4 << 20) / (clip_in * sizeof(float)));
-    if ((batch + per - 1) / per > 16) per = (batch + 15) / 16;
+    // groups of clips: about 8 MB of input each, at most 16 groups.  The first upload and the last download are not overlapped, which
+    // argues for small groups; every group costs ~8 runtime calls on the host, which argues against: 32 groups of 2 MB made the
+    // Whisper-shaped batch host-bound (1.61 ms against 1.31 ms with 8 groups).
+    constexpr int kMaxGroups = 16;
+    int per = (int)std::max<size_t>(1, ((size_t)8 << 20) / (clip_in * sizeof(float)));
+    if ((batch + per - 1) / per > kMaxGroups) per = (batch + kMaxGroups - 1) / kMaxGroups;
     const int groups = (batch + per - 1) / per;
-    cudaEvent_t ev_start = nullptr, ev_in[16] = {}, ev_k[16] = {}, ev_done = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_in[kMaxGroups] = {}, ev_k[kMaxGroups] = {}, ev_done = nullptr;
     cudaError_t e = cudaEventCreateWithFlags(&ev_start, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ev_done, cudaEventDisableTiming);
     for (int g = 0; g < groups && e == cudaSuccess; ++g) {
@@ -527,7 +564,7 @@ extern "C" int melt_forward_host(const melt_plan *p, const float *x_host, int ba
     auto cleanup = [&]() {   // destroying a recorded event is legal: its resources are released when it has completed
         if (ev_start) cudaEventDestroy(ev_start);
         if (ev_done) cudaEventDestroy(ev_done);
-        for (int g = 0; g < 16; ++g) { if (ev_in[g]) cudaEventDestroy(ev_in[g]); if (ev_k[g]) cudaEventDestroy(ev_k[g]); }
+        for (int g = 0; g < kMaxGroups; ++g) { if (ev_in[g]) cudaEventDestroy(ev_in[g]); if (ev_k[g]) cudaEventDestroy(ev_k[g]); }
     };
     if (e != cudaSuccess) { cleanup(); cudaFreeAsync(ws_in, st); cudaFreeAsync(ws_out, st); return cuda_fail(e, "cudaEventCreate"); }
     // the copy streams start behind everything already in the caller's stream (which includes the scratch allocations)

@@ -46,6 +46,8 @@ def plan_for(c, precision="compensated", layout=None, pad=None, drop_last=None, 
     mb.melt_plan_set_option(plan, mb.MELT_OPT_PAD, int(bool(pad)))
     if output == "power":
         mb.melt_plan_set_option(plan, mb.MELT_OPT_OUTPUT, mb.MELT_OUTPUT_POWER)
+    if output == "whisper":
+        mb.melt_plan_set_option(plan, mb.MELT_OPT_OUTPUT, mb.MELT_OUTPUT_LOG_WHISPER)
     if output == "ln":
         mb.melt_plan_set_option(plan, mb.MELT_OPT_OUTPUT, mb.MELT_OUTPUT_LN_EPS)
     if input_ready:

@@ -344,3 +344,10 @@ def test_ln_eps_form_closed_values():
     ref = orc.forward(x, fs=16000.0, n_fft=400, hop=160, window_kind=0, n_mels=1, fmin=0.0, fmax=5600.0, want=("P", "L"))
     np.testing.assert_allclose(orc.ln_eps(ref["P"])[0, 0], np.log(2500.0), atol=1e-6)
     np.testing.assert_allclose(orc.ln_eps(ref["P"]), np.log(10.0) * ref["L"], atol=1e-9)
+
+
+def test_whisper_norm_closed_values():
+    from oracle import melt_oracle as orc
+    L = np.array([[2.0, -10.0, -5.9], [-6.0, -6.1, 1.0]])
+    # max = 2 -> floor -6: values below -6 are raised to it; then (L + 4) / 4
+    np.testing.assert_allclose(orc.whisper_norm(L), [[1.5, -0.5, -0.475], [-0.5, -0.5, 1.25]], rtol=0, atol=1e-15)

@@ -130,3 +130,23 @@ def test_paper_form_mfcct_is_the_dct_of_ln():
     assert np.abs(L_gpu - Lref)[mask].max() <= pu.LOG_BAR * np.log(10.0)
     for b in range(2):
         assert np.abs(C_gpu[b] - orc.dct_apply(L_gpu[b], 13)).max() <= 2e-4
+
+
+@pytest.mark.parametrize("layout", ["feature_major", "frame_major"])
+def test_whisper_dynamic_range_normalisation(layout):
+    """MELT_OUTPUT_LOG_WHISPER: per clip L <- (max(L, max_clip(L) - 8) + 4) / 4 on top of the contract log10 form.  The clip maximum is a
+    loud bin (error ~1e-4), so inside the log mask the error is the log error / 4; below the clamp both sides sit on the floor."""
+    orc = _orc()
+    c = dict(_wl().CONFIGS["cfg1"]); c["name"] = "cfg1"
+    x = _wl().make_inputs("cfg1", 3)["x"]
+    x[1] *= 1e-3                                            # a quiet clip: its own maximum sets its own floor
+    got = pu.gpu_dense(c, x, "compensated", layout=layout, output="whisper")
+    ref = orc.forward_batch(x, want=("P", "L"), **pu.oracle_kwargs(c))
+    want = np.stack([orc.whisper_norm(ref["L"][b]) for b in range(3)])
+    assert got.shape == want.shape and np.isfinite(got).all()
+    fmax = ref["P"].max(axis=-1, keepdims=True)
+    mask = ref["P"] >= pu.MASK_FLOOR * fmax
+    assert np.abs(got - want)[mask].max() <= pu.LOG_BAR / 4 + 1e-6
+    for b in range(3):                                      # the floor itself: (max(max_clip - 8, -10) + 4) / 4 (-10: the log10 clamp)
+        floor = (max(ref["L"][b].max() - 8.0, -10.0) + 4.0) / 4.0
+        assert abs(got[b].min() - floor) <= 1e-3 and got[b].max() <= (ref["L"][b].max() + 4.0) / 4.0 + 1e-3
