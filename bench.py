@@ -610,7 +610,10 @@ def main():
     kernel_ms = ms_per_step                      # one launch per step: average launch duration over the timed region
     kernel_ms_median = statistics.median(per_ms)  # isolated launches (second pass, an event between every two launches)
     dtype = PREC_DTYPE[args.precision]
-    tf32_tflops = measure_tf32_peak(torch)       # cuBLAS TF32 on this GPU, this run (MEASURED_PEAKS.json has bf16 only)
+    tf32_cublas = measure_tf32_peak(torch)       # cuBLAS TF32 on this GPU, this run (MEASURED_PEAKS.json has bf16 only)
+    # the denominator is the LARGER of that measurement and the measured bf16 peak x the nominal TF32:bf16 ratio of 1/2: the
+    # cuBLAS TF32 GEMM of this image runs at 680-770 TFLOP/s, which this library's own TF32 path reaches on cfg2
+    tf32_tflops = max(tf32_cublas, 0.5 * peaks["bf16_tflops"])
     roof = roofline_of(nums, kernel_ms, peaks, dtype, tf32_tflops)
     t_ref = max(roof["t_hbm_us"], roof["t_tensor_us"]) * 1e-3          # roofline time of one step, ms
     roof["traffic"] = None
@@ -623,7 +626,7 @@ def main():
                  "ordered": {"ms_per_step": ordered_ms, "note": "MELT_OPT_INPUT_READY=0, the library default: no read of x before the "
                              "previous kernel in the stream has completed (only set-up overlaps)"},
                  "overlap_curve_us_per_step": overlap_curve,
-                 "tensor_peak_dtype": dtype, "tf32_tflops_measured": tf32_tflops,
+                 "tensor_peak_dtype": dtype, "tf32_tflops_measured": tf32_cublas, "tf32_tflops_peak_used": tf32_tflops,
                  "algorithmic_bytes": nums["bytes_in"] + nums["bytes_out"], "algorithmic_flops": nums["flops"],
                  "frac_vs_tf32_roofline": max(roof["t_hbm_us"] * 1e-6, nums["flops"] / (tf32_tflops * 1e12)) / (kernel_ms * 1e-3)})
     prof = os.path.join(ROOT, "profiles", "traffic_%s_%s.json" % (cfg, args.precision))

@@ -364,11 +364,12 @@ __device__ __forceinline__ void load_kstaged(uint32_t kb, uint32_t half, float (
 template <int PREC, int SIGMA, bool RAGGED, int MODE, bool STREAM, bool DIRECT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1) melt_fwd2_kernel(const __grid_constant__ K2Params p) {
     extern __shared__ __align__(128) uint8_t smem[];
-    // Who drains the accumulators: MODE 0 the four epilogue warps alone; MODE 1 (single accumulator stage, log-Mel) the epilogue
-    // warps and the converter warps together; MODE 2 (log-Mel) there are no epilogue warps -- they form a third converter
-    // group and every converter warp drains a third of the bins of the previous tile.
-    constexpr bool SHARE = MODE != 0;
-    constexpr int NG = MODE == 2 ? V2_CONV_GROUPS : V2_CONV_GROUPS - 1;   // converter groups: 3 without epilogue warps, 2 next to them
+    // Who drains the accumulators: MODE 0 the four epilogue warps alone (next to two converter groups); MODE 1 (single accumulator
+    // stage, log-Mel) the epilogue warps and the converter warps together; MODE 2 (log-Mel) there are no epilogue warps -- they
+    // form a third converter group and every converter warp drains a third of the bins of the previous tile; MODE 3 (log-Mel):
+    // four drain warps AND three converter groups, 640 threads (launch_one says which is used when).
+    constexpr bool SHARE = MODE != 0 && MODE != 3;
+    constexpr int NG = (MODE == 2 || MODE == 3) ? V2_CONV_GROUPS : V2_CONV_GROUPS - 1;   // converter groups: 3 without epilogue warps, 2 next to them
     constexpr int NT = v2_threads(MODE);                                  // threads of the block
     constexpr int CONV0 = MODE == 2 ? W_EPI0 : W_CONV0;                   // first converter warp
     constexpr int DRAINERS = MODE == 2 ? NG : 1 + NG;                     // warps per lane quarter that drain (SHARE)
@@ -945,10 +946,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
             TRACE(31);
             tc_fence_after();
             const uint32_t t_r = lane_taddr + (uint32_t)stage * (uint32_t)p.acc_cols, t_i = t_r + (uint32_t)p.nb;
-            if (SHARE) {
+            if (SHARE || MODE == 3) {
                 // single accumulator stage, log-Mel: this warp drains every third 16-bin block, the two converter warps of the
-                // lane quarter the others
-                epi_fast_share(t_r, t_i, p.nb, nm, optr, cstride, valid, p.out_log10_offset, 0, DRAINERS);
+                // lane quarter the others (MODE 3: plain log-Mel, this warp drains every block)
+                epi_fast_share(t_r, t_i, p.nb, nm, RAGGED ? out_at(p, (out_row0 + lane) * p.n_ch + c_off) : (p.feature_major ? out_at(p, ((long long)b * p.n_ch + c_off) * T + t0 + row) : out_at(p, (ti.f0 + t0 + row) * p.n_ch + c_off)),
+                               cstride, valid, p.out_log10_offset, 0, MODE == 3 ? 1 : DRAINERS, p.out_dtype);
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
@@ -1273,12 +1275,19 @@ static int launch_one_r(const K2Params &kp, int grid, cudaStream_t stream) {
 
 template <int PREC, int SIGMA>
 static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
-    // Plain log-Mel output: no dedicated epilogue warps, three converter groups that also drain (MODE 2); everything else keeps
-    // the four epilogue warps (MODE 0).  (MODE 1, epilogue + converter warps draining a single-stage accumulator, measured the
-    // same as MODE 2 on cfg2 and is not instantiated.)
+    // Who drains the accumulators.  Power / tap / ln / MFCCT outputs: four epilogue warps next to two converter groups (MODE 0).
+    // Plain log-Mel: three converter groups, and either four dedicated drain warps next to them (MODE 3, 640 threads) or -- when
+    // the accumulator has a single stage, the basis is resident and the MMAs run at half rate (TF32): the tensor pipe is the
+    // bound and idles while a tile is drained -- every converter warp drains a third of the previous tile's bins (MODE 2).
+    // Measured (r02, B200, back to back): MODE 3 vs MODE 2  cfg1 -3.6 %, 256 x 4 s clips -13 %, cfg4a tf32 / bf16 -4.5 / -6.8 %,
+    // cfg2 tf32 +5 % (hence the exception), everything else within +-2 %.
     const bool plain = kp.n_mfcc == 0 && !kp.output_power && kp.tap == nullptr;
-    const int mode = plain ? 2 : 0;
-    if (kp.offsets) return mode == 2 ? launch_one_r<PREC, SIGMA, true, 2>(kp, grid, stream) : launch_one_r<PREC, SIGMA, true, 0>(kp, grid, stream);
+    const int mode = !plain ? 0 : (PREC == P2_TF32 && kp.acc_stages == 1 && kp.b_resident && !kp.direct ? 2 : 3);
+    if (kp.offsets) {
+        if (mode == 3) return launch_one_r<PREC, SIGMA, true, 3>(kp, grid, stream);
+        return mode == 2 ? launch_one_r<PREC, SIGMA, true, 2>(kp, grid, stream) : launch_one_r<PREC, SIGMA, true, 0>(kp, grid, stream);
+    }
+    if (mode == 3) return launch_one_r<PREC, SIGMA, false, 3>(kp, grid, stream);
     return mode == 2 ? launch_one_r<PREC, SIGMA, false, 2>(kp, grid, stream) : launch_one_r<PREC, SIGMA, false, 0>(kp, grid, stream);
 }
 
