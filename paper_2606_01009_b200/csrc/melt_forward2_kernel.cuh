@@ -107,7 +107,7 @@ static __device__ long long *g_melt_trace = nullptr;   // [2 ranks][16 warps][10
 #define TRACE_WORDS (2 * 16 * 1024 + 592 + 148 * 8 + 64)   // one region per traced launch (K2Params::trace_slot)
 #define TRACE_BASE (g_melt_trace + (size_t)p.trace_slot * TRACE_WORDS)
 #define TRACE_PT(i) do { if (g_melt_trace && threadIdx.x == 0) TRACE_BASE[2 * 16 * 1024 + 592 + blockIdx.x * 8 + (i)] = clock64(); } while (0)
-#define TRACE_DECL int tr_n = 0; long long *tr_buf = (g_melt_trace && cluster_id_x() == 0 && (threadIdx.x & 31) == 0) ? TRACE_BASE + ((size_t)cluster_ctarank() * 16 + (threadIdx.x >> 5)) * 1024 : nullptr;
+#define TRACE_DECL int tr_n = 0; long long *tr_buf = (g_melt_trace && cluster_id_x() == 0 && (threadIdx.x & 31) == 0 && threadIdx.x < 512) ? TRACE_BASE + ((size_t)cluster_ctarank() * 16 + (threadIdx.x >> 5)) * 1024 : nullptr;
 #define TRACE(tag) do { if (tr_buf && tr_n < 1023) tr_buf[++tr_n] = ((long long)(tag) << 48) | (clock64() & 0xFFFFFFFFFFFFll); if (tr_buf) tr_buf[0] = tr_n; } while (0)
 #define TRACE_CTA(which) do { if (g_melt_trace && threadIdx.x == 0) { TRACE_BASE[2 * 16 * 1024 + blockIdx.x * 2 + (which)] = (long long)globaltimer_ns(); TRACE_BASE[2 * 16 * 1024 + 296 + blockIdx.x * 2 + (which)] = clock64(); } } while (0)
 #else
@@ -534,12 +534,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
         long long rg_f0 = 0, rg_T = 0, rg_s0 = 0, rg_len = 0;
         bool rg_have = false;
         int tl = 0;   // tiles of this CTA so far
+        // This warp's loop is the pacemaker of the whole kernel (one chunk per ~quarter tile), and a 64-bit division costs it
+        // hundreds of cycles: per chunk there is none.  Reflect padding moves a chunk's start vpad samples down = r_pad hop-rows
+        // up and c0_pad columns in; a ragged clip's start in the 2-D map (row, column) is divided out once per clip.
+        const int vq = p.vpad > 0 ? p.vpad / p.hop : 0, vr = p.vpad - vq * p.hop;
+        const int c0_pad = vr ? p.hop - vr : 0, r_pad = vq + (vr ? 1 : 0);
+        long long rg_rclip = 0;
+        int rg_cclip = 0;
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
+            Tile2 ti_tile;
+            if constexpr (!ragged) get_tile2<false>(p, tile, ti_tile);
             for (int q = 0; q < 4; ++q) {
                 Tile2 ti;
                 long long row0;
                 if constexpr (!ragged) {
-                    get_tile2<false>(p, tile, ti);
+                    ti = ti_tile;
                     row0 = (long long)(ti.t0 + (int)rank * 128 + 32 * q);
                 } else {
                     const int g = (p.passes > 1 ? tile / p.passes : tile) * 8 + (int)rank * 4 + q;   // chunk index in the packed chunk order
@@ -563,6 +572,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                             rg_s0 = __ldg(p.offsets + rg_clip);
                             rg_len = __ldg(p.offsets + rg_clip + 1) - rg_s0;
                             rg_have = true;
+                            const long long sc = (rg_s0 & ~3ll) - p.vpad;    // where the clip's frame 0 starts (aligned down; may be < 0)
+                            rg_rclip = sc / p.hop;
+                            rg_cclip = (int)(sc - rg_rclip * p.hop);
+                            if (rg_cclip < 0) { rg_cclip += p.hop; --rg_rclip; }
                         }
                         ti.clip = rg_clip; ti.T = rg_T; ti.s0 = rg_s0; ti.f0 = rg_f0;
                         row0 = (long long)(g - rg_lo) * 32;
@@ -572,10 +585,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                 const float *xb = p.x + ti.s0;
                 const long long clip_len = ragged ? rg_len : len;
                 const int n_rows = row0 < ti.T ? p.rows_per_chunk : 0;
-                long long avail = clip_len - row0 * p.hop;                 // samples of the clip from the chunk's first row on
-                avail = avail < 0 ? 0 : avail;
-                const long long want = (long long)n_rows * p.hop;
-                const uint32_t total_b = (uint32_t)(avail < want ? avail : want) * 4u;
                 const uint32_t dst0 = sbase + p.off_stg + (uint32_t)slot * (uint32_t)p.slot_bytes;
                 // ragged: the chunk starts at sample s of the packed buffer = column s % hop of hop-row s / hop of the 2-D map
                 // The tensor-map engine wants the box to start on a 16-byte boundary: it is fetched from the aligned sample below
@@ -592,14 +601,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                     if (p.vpad == 0) {
                         by_tma = n_rows > 0 && row0 + n_rows <= (long long)p.tma_rows;
                     } else {
-                        const long long r = st >= 0 ? st / p.hop : 0;
-                        c0 = (int)(st - r * p.hop); c1 = (int)r;
-                        by_tma = n_rows > 0 && st >= 0 && r + n_rows <= (long long)p.tma_rows;   // every row of the box inside the clip
+                        c0 = c0_pad; c1 = (int)row0 - r_pad;    // st = c1 * hop + c0 (st >= 0)
+                        by_tma = n_rows > 0 && st >= 0 && (long long)c1 + n_rows <= (long long)p.tma_rows;   // every row of the box inside the clip
                     }
                 } else {
-                    s = (ti.s0 & ~3ll) + st;
-                    const long long r = s >= 0 ? s / p.hop : 0;
-                    c0 = (int)(s - r * p.hop); c1 = (int)r; c2 = 0;
+                    s = (ti.s0 & ~3ll) + st;                    // = (rg_rclip + row0) * hop + rg_cclip
+                    c0 = rg_cclip; c1 = (int)(rg_rclip + row0); c2 = 0;
                     by_tma = n_rows > 0 && s >= 0 && s + (long long)(p.rows_per_chunk - 1) * p.hop + (p.pitch_bytes >> 2) <= total;
                     if (p.vpad > 0) {   // and every valid frame of the chunk inside its clip (what lies beyond is mirrored, not the next clip)
                         const long long tlast = row0 + 31 < ti.T - 1 ? row0 + 31 : ti.T - 1;
@@ -698,6 +705,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                         tma_load_3d(dst0, p.tmap, c0, c1, c2, full);
                     } else {
                         // clip tail (or no tensor map): one bulk copy per hop-row, clipped to the clip
+                        long long avail = clip_len - row0 * p.hop;                 // samples of the clip from the chunk's first row on
+                        avail = avail < 0 ? 0 : avail;
+                        const long long want = (long long)n_rows * p.hop;
+                        const uint32_t total_b = (uint32_t)(avail < want ? avail : want) * 4u;
                         if (total_b) mbar_arrive_expect_tx(full, total_b);
                         else mbar_arrive(full);
                         uint32_t dst = dst0;
