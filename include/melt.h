@@ -196,6 +196,23 @@ int melt_forward_ragged(const melt_plan *plan, const float *x, const long long *
                         void *out, long long *out_frame_offsets, void *stream);
 
 /*
+ * melt_forward_ragged_noalloc -- melt_forward_ragged (Eq. (3)-(4), (8)-(9) on packed clips; same arguments, same
+ * results) for callers that must not allocate: code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc.  The call allocates and frees nothing, on the host or the device (no cudaMalloc / cudaFree, no memory-pool call):
+ * the only per-call scratch of the ragged path, the device-side chunk prefix of n_clips + 1 ints, lives in a file-scope device
+ * array of the library (MELT_NOALLOC_MAX_CLIPS + 1 ints = 256 KB that every GPU which loads the library holds until exit).
+ *   n_clips > MELT_NOALLOC_MAX_CLIPS is rejected with MELT_ERR_UNSUPPORTED (use melt_forward_ragged);
+ *   all calls on a device share the array: calls in ONE stream are ordered; calls that overlap on the GPU (different streams,
+ *   or this entry point on two plans at once) RACE on it -- serialise them or use melt_forward_ragged, whose scratch is per call;
+ *   the array keeps the last call's contents; every call rewrites the entries it reads, so nothing has to be cleared;
+ *   the first call on a device looks the array's address up once (cudaGetSymbolAddress; no allocation).
+ * Everything else (arguments, layouts, options, errors) as melt_forward_ragged; Whisper-normalised output is dense-only.
+ */
+#define MELT_NOALLOC_MAX_CLIPS 65536
+int melt_forward_ragged_noalloc(const melt_plan *plan, const float *x, const long long *offsets, int n_clips,
+                                void *out, long long *out_frame_offsets, void *stream);
+
+/*
  * melt_forward_tap -- as melt_forward / melt_forward_ragged (offsets == NULL selects the dense form, in which
  * n_clips is the batch and len the clip length; otherwise len is ignored), and additionally writes the log-Mel
  * matrix that feeds the DCT to `logmel` (device, fp32, same frame order and layout as `out`, n_mels channels).

@@ -24,8 +24,8 @@ MELT_DTYPE_F32, MELT_DTYPE_F16, MELT_DTYPE_BF16 = 0, 1, 2
 # every symbol include/melt.h declares (tests/test_abi.py checks the header against this list and the .so) ...
 SYMBOLS = [
     "melt_plan_create", "melt_plan_destroy", "melt_plan_set_option", "melt_num_frames", "melt_count_frames", "melt_num_channels",
-    "melt_plan_reserve", "melt_plan_get_centres", "melt_forward", "melt_forward_host", "melt_forward_ragged", "melt_forward_tap",
-    "melt_last_error", "melt_plan_describe",
+    "melt_plan_reserve", "melt_plan_get_centres", "melt_forward", "melt_forward_host", "melt_forward_ragged",
+    "melt_forward_ragged_noalloc", "melt_forward_tap", "melt_last_error", "melt_plan_describe",
 ]
 # ... and the test aids of include/melt_test.h (not part of the product API)
 TEST_SYMBOLS = ["melt_selftest_umma", "melt_selftest_umma2", "melt_selftest_poison_smem"]
@@ -74,6 +74,7 @@ def load(path):
     L.melt_plan_get_centres.argtypes = [vp, C.POINTER(dbl)]
     L.melt_forward.argtypes = [vp, vp, ip, ll, vp, vp]
     L.melt_forward_ragged.argtypes = [vp, vp, vp, ip, vp, vp, vp]
+    L.melt_forward_ragged_noalloc.argtypes = [vp, vp, vp, ip, vp, vp, vp]
     L.melt_forward_host.argtypes = [vp, vp, ip, ll, vp, vp]
     L.melt_forward_tap.argtypes = [vp, vp, vp, ip, ll, vp, vp, vp, vp]
     L.melt_last_error.restype = C.c_char_p
@@ -161,6 +162,16 @@ def melt_forward_host(plan, x_host, batch, length, out_host, stream=0):
 def melt_forward_ragged(plan, x, offsets, n_clips, out, out_frame_offsets, stream=0):
     _check(lib().melt_forward_ragged(plan, _ptr(x), _ptr(offsets), int(n_clips), _ptr(out), _ptr(out_frame_offsets),
                                      stream or None))
+
+
+MELT_NOALLOC_MAX_CLIPS = 65536
+
+
+def melt_forward_ragged_noalloc(plan, x, offsets, n_clips, out, out_frame_offsets, stream=0):
+    """melt_forward_ragged without any allocation: scratch in a fixed device array (n_clips <= MELT_NOALLOC_MAX_CLIPS;
+    calls that overlap on the GPU race on it -- see include/melt.h)."""
+    _check(lib().melt_forward_ragged_noalloc(plan, _ptr(x), _ptr(offsets), int(n_clips), _ptr(out), _ptr(out_frame_offsets),
+                                             stream or None))
 
 
 def melt_forward_tap(plan, x, offsets, n_clips, length, out, logmel, out_frame_offsets, stream=0):

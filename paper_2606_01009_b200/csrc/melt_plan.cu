@@ -602,6 +602,75 @@ extern "C" int melt_forward_ragged(const melt_plan *p, const float *x, const lon
     if (!offsets) return fail(MELT_ERR_INVALID_ARG, "offsets is NULL");
     return forward_impl(p, x, offsets, n_clips, 0, out, nullptr, out_frame_offsets, stream, false);
 }
+
+// ---------------------------------------------------------------------------------------------- allocation-free ragged forward
+// melt_forward_ragged for callers that must not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc): the
+// one piece of per-call scratch of the ragged path, the device-side chunk / tile prefix (n_clips + 1 ints), lives in this
+// file-scope device array instead of the plan's stream-ordered pool.  Every GPU that loads the library holds its 256 KB until exit.
+// In host code `g_noalloc_tile_prefix` is a host-side stand-in, not a device address: the kernels get the address that
+// cudaGetSymbolAddress returns, looked up once per device with that device current.  All calls share the array: calls that
+// overlap on the GPU (different streams) race on it; calls in one stream are ordered (the scan kernel that rewrites the array is
+// a plain launch, so it starts only after the previous forward kernel has completed).  Nothing in it has to start at zero: the
+// scan kernel writes entries 0 .. n_clips of every call before the forward kernel reads them, and no entry beyond n_clips is read.
+static __device__ __align__(256) int g_noalloc_tile_prefix[MELT_NOALLOC_MAX_CLIPS + 1];
+
+static int noalloc_tile_prefix(int device, int **ptr) {
+    static std::atomic<int *> addr[64];   // per device; zero-initialised
+    int *a = (device >= 0 && device < 64) ? addr[device].load(std::memory_order_acquire) : nullptr;
+    if (!a) {
+        MELT_CUDA(cudaGetSymbolAddress((void **)&a, g_noalloc_tile_prefix));   // the current device is `device` (validate_common)
+        if (!a) return fail(MELT_ERR_CUDA, "cudaGetSymbolAddress returned a null address");
+        if (device >= 0 && device < 64) addr[device].store(a, std::memory_order_release);
+    }
+    *ptr = a;
+    return MELT_OK;
+}
+
+extern "C" int melt_forward_ragged_noalloc(const melt_plan *p, const float *x, const long long *offsets, int n_clips, void *out_any,
+                                           long long *out_frame_offsets, void *stream) {
+    if (!offsets) return fail(MELT_ERR_INVALID_ARG, "offsets is NULL");
+    int rc = validate_common(p, x, out_any);
+    if (rc) return rc;
+    float *out = static_cast<float *>(out_any);
+    const bool out16 = p->out_dtype != MELT_DTYPE_F32;
+    if (out16 && (p->n_mfcc > 0 || p->output != MELT_OUTPUT_LOG))
+        return fail(MELT_ERR_UNSUPPORTED, "16-bit output: log-Mel output (n_mfcc == 0, MELT_OUTPUT_LOG) only");
+    if (p->output == MELT_OUTPUT_LOG_WHISPER) return fail(MELT_ERR_UNSUPPORTED, "Whisper-normalised output: dense batches only");
+    if (n_clips < 0) return fail(MELT_ERR_INVALID_ARG, "negative clip count");
+    if (n_clips > MELT_NOALLOC_MAX_CLIPS)
+        return fail(MELT_ERR_UNSUPPORTED, "melt_forward_ragged_noalloc: n_clips=%d exceeds MELT_NOALLOC_MAX_CLIPS=%d (use melt_forward_ragged)",
+                    n_clips, MELT_NOALLOC_MAX_CLIPS);
+    if (!out_frame_offsets) return fail(MELT_ERR_INVALID_ARG, "out_frame_offsets is NULL");
+    if (p->kp.feature_major) return fail(MELT_ERR_UNSUPPORTED, "ragged batches are frame-major only");
+    p->used.store(true, std::memory_order_relaxed);
+    if (n_clips == 0) return MELT_OK;
+    int *tile_prefix = nullptr;
+    rc = noalloc_tile_prefix(p->device, &tile_prefix);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    // from here on: the ragged branch of forward_impl with the static array in place of pool scratch
+    const bool v2 = p->v2_ok && !p->k2.direct && (((uintptr_t)x & 15) == 0);
+    if (v2) {
+        rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, tile_prefix, 32, st);   // exclusive prefix of 32-frame chunks per clip
+        K2Params k2 = p->k2;
+        k2.x = x; k2.out = out; k2.tap = nullptr; k2.n_clips = n_clips; k2.len = 0; k2.frames_per_clip = 0;
+        k2.tiles_per_clip = 0; k2.n_tiles = -1;
+        k2.offsets = offsets; k2.frame_offsets = out_frame_offsets; k2.tile_prefix = tile_prefix;
+        k2.vpad = p->pad == MELT_PAD_REFLECT ? p->n_fft / 2 : 0;
+        k2.out_dtype = p->out_dtype;
+        k2.input_ready = 0;   // the scan kernel just ahead in the stream produces what the kernel reads at its entry
+        if (rc == MELT_OK && v2_encode_tmap_ragged(k2) == MELT_OK && k2.tma_rows > 0) return launch_forward2(p, k2, st);
+    }
+    if (rc == MELT_OK && out16) rc = fail(MELT_ERR_UNSUPPORTED, "16-bit output needs the CTA-pair kernel (hop %% 4 == 0, 16-byte aligned x, staged window)");
+    if (rc == MELT_OK) rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, tile_prefix, TILE_M, st);
+    KParams kp = p->kp;
+    kp.x = x; kp.out = out; kp.tap = nullptr; kp.n_clips = n_clips;
+    kp.offsets = offsets; kp.frame_offsets = out_frame_offsets; kp.tile_prefix = tile_prefix;
+    kp.len = 0; kp.frames_per_clip = 0; kp.tiles_per_clip = 0; kp.n_tiles = -1;
+    if (rc == MELT_OK) rc = launch_forward(p, kp, st);
+    return rc;
+}
+
 extern "C" int melt_forward_tap(const melt_plan *p, const float *x, const long long *offsets, int n_clips, long long len,
                                 float *out, float *logmel, long long *out_frame_offsets, void *stream) {
     return forward_impl(p, x, offsets, n_clips, len, out, logmel, out_frame_offsets, stream, p && p->input_ready);
