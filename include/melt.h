@@ -161,6 +161,23 @@ int melt_num_channels(const melt_plan *plan);
 int melt_plan_get_centres(const melt_plan *plan, double *f_hz);
 
 /*
+ * melt_plan_create_stft_mel -- a plan for the CONVENTIONAL front end, the comparator of the paper (a
+ * hand-fused version is what PAPER.md:545 calls future work): frames and window as in melt_plan_create, then
+ *   X_t[k] = sum_n w[n] x_t[n] exp(-2 pi i k n / N), k = 0 .. N/2;  P_t[k] = |X_t[k]|^2;
+ *   S_t[m] = sum_k F[m][k] P_t[k],  F[m][k] = max(0, min((f_k - e_m) / (e_{m+1} - e_m), (e_{m+2} - f_k) / (e_{m+2} - e_{m+1}))),
+ *            f_k = k fs / N, e = the n_mels + 2 points uniform in HTK mel between fmin and fmax (peak 1, no normalisation; the
+ *            filter centres are the analysis frequencies of melt_plan_create with the same arguments);
+ *   out    = log10(max(S, 1e-10)).
+ * One kernel: the DFT as a tensor-core product on the same folded, compensated operands as the MelT projection, the power written
+ * back to tensor memory as the operand of a second tensor-core product with F, the log in the epilogue -- nothing between the
+ * signal and the log-Mel rows touches HBM.  Covered: even n_fft with n_fft / 2 + 1 <= 224 bins (n_fft <= 446), hop % 4 == 0,
+ * n_mels <= 128, dense batches (melt_forward, melt_forward_host), fp32 output, MELT_OPT_LAYOUT / _PAD / _DROP_LAST /
+ * _INPUT_SCALE_LOG2 / _INPUT_READY; anything else returns NULL here or MELT_ERR_UNSUPPORTED at the call.  melt_num_channels = n_mels.
+ * Ownership and errors as melt_plan_create.
+ */
+melt_plan *melt_plan_create_stft_mel(double fs, int n_fft, int hop, int window, int n_mels, double fmin, double fmax);
+
+/*
  * melt_forward -- the whole hot path on a dense batch.
  *   x    device, fp32, [batch, len] contiguous, 4-byte aligned.  When every clip start is 16-byte aligned (x and len*4)
  *        the kernel frames x in place; otherwise one pass first copies the batch into pool scratch at an aligned clip

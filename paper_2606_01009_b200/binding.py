@@ -23,7 +23,7 @@ MELT_DTYPE_F32, MELT_DTYPE_F16, MELT_DTYPE_BF16 = 0, 1, 2
 
 # every symbol include/melt.h declares (tests/test_abi.py checks the header against this list and the .so) ...
 SYMBOLS = [
-    "melt_plan_create", "melt_plan_destroy", "melt_plan_set_option", "melt_num_frames", "melt_count_frames", "melt_num_channels",
+    "melt_plan_create", "melt_plan_create_stft_mel", "melt_plan_destroy", "melt_plan_set_option", "melt_num_frames", "melt_count_frames", "melt_num_channels",
     "melt_plan_reserve", "melt_plan_get_centres", "melt_forward", "melt_forward_host", "melt_forward_ragged",
     "melt_forward_ragged_noalloc", "melt_forward_tap", "melt_last_error", "melt_plan_describe",
 ]
@@ -62,6 +62,8 @@ def load(path):
     vp, ip, ll, dbl = C.c_void_p, C.c_int, C.c_longlong, C.c_double
     L.melt_plan_create.restype = vp
     L.melt_plan_create.argtypes = [dbl, ip, ip, ip, ip, dbl, dbl, ip, ip]
+    L.melt_plan_create_stft_mel.restype = vp
+    L.melt_plan_create_stft_mel.argtypes = [dbl, ip, ip, ip, ip, dbl, dbl]
     L.melt_plan_destroy.restype = None
     L.melt_plan_destroy.argtypes = [vp]
     L.melt_plan_set_option.argtypes = [vp, ip, ip]
@@ -106,6 +108,14 @@ def melt_last_error():
 def melt_plan_create(fs, n_fft, hop, window, n_mels, fmin, fmax, mel_scale=MELT_MEL_HTK, n_mfcc=0):
     h = lib().melt_plan_create(float(fs), int(n_fft), int(hop), int(window), int(n_mels), float(fmin), float(fmax),
                                int(mel_scale), int(n_mfcc))
+    if not h:
+        raise MeltError(-1, melt_last_error())
+    return h
+
+
+def melt_plan_create_stft_mel(fs, n_fft, hop, window, n_mels, fmin, fmax):
+    """Plan of the conventional STFT -> power -> triangular Mel filterbank -> log10 front end (include/melt.h)."""
+    h = lib().melt_plan_create_stft_mel(float(fs), int(n_fft), int(hop), int(window), int(n_mels), float(fmin), float(fmax))
     if not h:
         raise MeltError(-1, melt_last_error())
     return h

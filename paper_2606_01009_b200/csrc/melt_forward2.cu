@@ -27,6 +27,17 @@ int plan_build_v2(melt_plan *p) {
     k.passes = (M + 127) / 128;                                   // more than 128 bins: several passes, each tile visited once per pass
     k.nb = round_up2((M + k.passes - 1) / k.passes, 16);
     if (k.nb < 32) k.nb = 32;
+    const bool fbank = p->fb_mels > 0;                            // conventional front end: all DFT bins of a frame in ONE pass (the
+    if (fbank) {                                                  // filterbank product needs them together), compensated operands only
+        if (!comp) return MELT_OK;
+        k.passes = 1;
+        k.nb = round_up2(M, 16);
+        k.fb_mels = p->fb_mels;
+        k.fb_nb = std::max(32, round_up2(p->fb_mels, 16));
+        k.fb_units = k.nb / 16;
+        k.fb_kind_bytes = (uint32_t)(k.fb_nb / 2) * 32u;
+        if (k.fb_nb > k.nb) return MELT_OK;                       // the filterbank's accumulator reuses the columns of I
+    }
     // ---- what the kernel covers (everything else stays on the general v1 kernel)
     k.a0 = k1.a0; k.b0 = k1.b0;
     if ((H & 3) || (k1.a0 & 3)) return MELT_OK;
@@ -56,13 +67,15 @@ int plan_build_v2(melt_plan *p) {
     const uint32_t dct_only = p->n_mfcc > 0 ? (uint32_t)(M * k.dct_pitch * 4) : 0;
     // MFCCT, frame-major: 4 epilogue warps x 32 frames x n_mfcc floats behind the DCT table (cepstra transposed for coalesced stores)
     const uint32_t epi_bytes = (p->n_mfcc > 0 && p->layout == MELT_LAYOUT_FRAME_MAJOR) ? (uint32_t)(4 * 32 * p->n_mfcc * 4) : 0;
-    const uint32_t dct_bytes = dct_only + epi_bytes;
+    const uint32_t fb_bytes = fbank ? (uint32_t)round_up2((int)(2u * (uint32_t)k.fb_units * k.fb_kind_bytes), 128) : 0;   // this CTA's half of the filterbank image
+    const uint32_t dct_bytes = dct_only + epi_bytes + fb_bytes;
     const uint32_t bar_bytes = (uint32_t)round_up2(V_NBARS * 8 + 16 + 32 * 16, 128);   // barriers, tensor-memory address, chunk records of ragged batches (32 x 16 B)
     k.off_b = 0;
     // The basis half stays resident when that leaves room for at least five staging slots; otherwise (long windows, > 128 bins) its
     // K-step slabs are streamed from L2 through a ring of 8 slabs; when five chunk slots do not fit next to that: K-block staging.
     k.b_resident = 1; k.b_slots = k.units;
     if (k.passes > 1) { k.b_resident = 0; k.b_slots = std::min(8, k.units); }   // every pass needs other rows: streamed
+    if (fbank) { k.b_resident = 0; k.b_slots = std::min(8, k.units); }          // the kernel's MODE 4 is instantiated for a streamed basis
     for (;;) {
         const uint32_t ring_bytes = (uint32_t)k.b_slots * k.unit_b_bytes;
         k.off_stg = (uint32_t)round_up2((int)ring_bytes, 128) + 128;  // 128-byte zero guard in front of the staging ring
@@ -70,6 +83,10 @@ int plan_build_v2(melt_plan *p) {
         k.stg_slots = (int)std::min<long long>(room > 0 ? room / k.slot_bytes : 0, V2_MAX_STG);
         if (k.stg_slots >= 5) break;
         if (k.b_resident) { k.b_resident = 0; k.b_slots = std::min(8, k.units); continue; }
+        if (fbank) {                     // a shallower basis ring until five chunks fit next to the filterbank image
+            if (k.b_slots > 3) { --k.b_slots; continue; }
+            return MELT_OK;
+        }
         {
             // Not even a streamed basis with its full ring leaves room for five staged 32-frame chunks (long windows: a chunk is
             // 32 hops of the signal).  K-BLOCK STAGING instead: the loader brings, per lane quarter and block of four K-steps, just
@@ -91,6 +108,7 @@ int plan_build_v2(melt_plan *p) {
     k.stg_phases = std::max(1, (k.stg_slots + 3) / 4);
     k.off_dct = (uint32_t)round_up2((int)(k.off_stg + (uint32_t)k.stg_slots * k.slot_bytes + (k.direct ? 8u * k.kslot_bytes : 0u) + 128), 128);
     k.off_epi = epi_bytes ? k.off_dct + dct_only : 0;
+    k.off_fb = k.off_dct + dct_only + epi_bytes;   // (128-byte aligned: a filterbank plan has no DCT table)
     k.off_bar = (uint32_t)round_up2((int)(k.off_dct + dct_bytes), 128);
     k.smem_bytes = k.off_bar + bar_bytes;
     if (k.smem_bytes > (uint32_t)SMEM_BUDGET) return MELT_OK;
@@ -162,6 +180,24 @@ int plan_build_v2(melt_plan *p) {
     MELT_CUDA(cudaMemcpy(p->d_bimg2, img.data(), img_bytes, cudaMemcpyHostToDevice));
     k.b_img = p->d_bimg2;
     k.dct = p->d_dct;
+    if (fbank) {
+        // B operand of the second product, D2[frame][filter] = sum_k P[frame][k] F[filter][k]: per CTA rank r its half of the filter rows,
+        // per K-step of 16 bins a bf16 "hi" slab and a bf16 "mid" slab (F = hi + mid to ~2^-17; the products hi.hi + mid.hi + hi.mid)
+        const int fh = k.fb_nb / 2;
+        const size_t fimg_bytes = (size_t)2 * k.fb_units * 2 * k.fb_kind_bytes;
+        std::vector<uint8_t> fimg(fimg_bytes, 0);
+        auto fval = [&](int row, int bin) -> double { return (row < p->fb_mels && bin < M) ? p->fb[(size_t)row * M + bin] : 0.0; };
+        for (int r = 0; r < 2; ++r)
+            for (int u = 0; u < k.fb_units; ++u)
+                for (int kk = 0; kk < 2; ++kk)
+                    pack_b_slab(OP_BF16, fh, [&](int row, int kq) {
+                        const double v = fval(r * fh + row, u * 16 + kq);
+                        return kk ? v - bf16_bits_to_f64(f64_to_bf16_bits(v)) : v;
+                    }, fimg.data() + (((size_t)r * k.fb_units + u) * 2 + kk) * k.fb_kind_bytes);
+        MELT_CUDA(cudaMalloc(&p->d_fbimg, fimg_bytes));
+        MELT_CUDA(cudaMemcpy(p->d_fbimg, fimg.data(), fimg_bytes, cudaMemcpyHostToDevice));
+        k.fb_img = p->d_fbimg;
+    }
     p->v2_ok = true;
     char buf[512];
     snprintf(buf, sizeof(buf),
@@ -309,6 +345,7 @@ int launch_forward2(const melt_plan *pl, const K2Params &kp, cudaStream_t stream
     if (pairs < 1) return MELT_OK;
     const int grid = 2 * pairs;
     const int sg = pl->v2_sigma;
+    if (kp.fb_mels > 0) return launch_forward2_fb(kp, grid, sg, stream);
     switch (pl->precision) {
         case MELT_PREC_COMPENSATED: return launch_forward2_comp(kp, grid, sg, stream);
         case MELT_PREC_TF32: return launch_forward2_tf32(kp, grid, sg, stream);

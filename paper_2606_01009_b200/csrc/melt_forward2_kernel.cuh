@@ -38,7 +38,9 @@ enum { P2_COMP = 0, P2_TF32 = 1, P2_BF16 = 2 };
 // barrier indices (8 bytes each)
 enum {
     V_STG_FULL = 0, V_STG_EMPTY = V2_MAX_STG, V_A_FULL = 2 * V2_MAX_STG, V_A_EMPTY = V_A_FULL + 16, V_ACC_FULL = V_A_EMPTY + 16,
-    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_DONE = V_B_PEER + V2_MAX_UNITS, V_STG_READY = V_DONE + 1, V_B_EMPTY = V_STG_READY + V2_MAX_STG, V_INFO = V_B_EMPTY + 8, V_KFULL = V_INFO + 32, V_KEMPTY = V_KFULL + 24, V_NBARS = V_KEMPTY + 24
+    V_ACC_EMPTY = V_ACC_FULL + 2, V_B_FULL = V_ACC_EMPTY + 2, V_B_PEER = V_B_FULL + V2_MAX_UNITS, V_DONE = V_B_PEER + V2_MAX_UNITS, V_STG_READY = V_DONE + 1, V_B_EMPTY = V_STG_READY + V2_MAX_STG, V_INFO = V_B_EMPTY + 8, V_KFULL = V_INFO + 32, V_KEMPTY = V_KFULL + 24,
+    V_P_READY = V_KEMPTY + 24, V_D2_FULL = V_P_READY + 1, V_FB_FULL = V_D2_FULL + 1, V_FB_PEER = V_FB_FULL + 1,   // MODE 4 (filterbank product)
+    V_NBARS = V_FB_PEER + 1
 };
 constexpr int V2_MAX_A_SLOTS = 16;
 constexpr int W_LOAD = 0, W_MMA = 1, W_BASIS = 2, W_MMA2 = 3, W_EPI0 = 4, W_CONV0 = 8;
@@ -277,6 +279,67 @@ __device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uin
     }
 }
 
+// MODE 4, the conventional front end: the accumulators hold R | I of the N/2 + 1 DFT
+// bins of this thread's frame.  (1) power per bin, split into a bf16 "hi" and a bf16 "mid" part (P = hi + mid to ~2^-17) and written
+// back IN PLACE over R as the A operand of a second tensor-core product: the 16 bins of a block become 8 columns of hi pairs and 8
+// columns of mid pairs -- K-step s of that product reads columns [16 s, 16 s + 8) and [16 s + 8, 16 s + 16); (2) hand-off to the
+// issuer warp, which multiplies by the triangular filterbank (bf16 hi + mid slabs in shared memory; hi.hi + mid.hi + hi.mid) into
+// the columns of I, no longer needed; (3) log10(max(., 1e-10)) of the Mel energies, stored like a log-Mel row.
+__device__ __forceinline__ void epi_fbank(const K2Params &p, uint32_t t_r, uint32_t t_i, float *optr, long long cstride, bool valid,
+                                          int lane, uint32_t p_ready_remote, uint32_t d2_full_bar, uint32_t d2_parity, uint32_t acc_empty_bar) {
+    const float kLog10_2 = 0.30102999566398120f;
+    for (int c0 = 0; c0 < p.nb; c0 += 16) {
+        uint32_t vr[16], vi[16], w[16];
+        tmem_ld16(t_r + (uint32_t)c0, vr);
+        tmem_ld16(t_i + (uint32_t)c0, vi);
+        tmem_wait_ld();
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const float r0 = __uint_as_float(vr[2 * j]), i0 = __uint_as_float(vi[2 * j]);
+            const float r1 = __uint_as_float(vr[2 * j + 1]), i1 = __uint_as_float(vi[2 * j + 1]);
+            const float p0 = fmaf(r0, r0, i0 * i0), p1 = fmaf(r1, r1, i1 * i1);            // |X[k]|^2 (scaled by the operand scales)
+            const __nv_bfloat162 h = __floats2bfloat162_rn(p0, p1);
+            const float2 hf = __bfloat1622float2(h);
+            const __nv_bfloat162 m = __floats2bfloat162_rn(p0 - hf.x, p1 - hf.y);
+            w[j] = *reinterpret_cast<const uint32_t *>(&h);                                 // K elements (2 j, 2 j + 1): low half first
+            w[8 + j] = *reinterpret_cast<const uint32_t *>(&m);
+        }
+        tmem_st16(t_r + (uint32_t)c0, w);
+    }
+    tmem_wait_st();
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive_remote(p_ready_remote);
+    mbar_wait(d2_full_bar, d2_parity);
+    tc_fence_after();
+    const bool vec4 = cstride == 1 && ((reinterpret_cast<uintptr_t>(optr) & 15) == 0);   // warp-uniform (rows are n_ch * 4 bytes apart)
+    for (int c0 = 0; c0 < p.fb_nb; c0 += 16) {
+        uint32_t d[16];
+        tmem_ld16(t_i + (uint32_t)c0, d);
+        tmem_wait_ld();
+        float v[16];
+#pragma unroll
+        for (int c = 0; c < 16; ++c) v[c] = fmaxf(fmaf(lg2_ftz(__uint_as_float(d[c])), kLog10_2, p.out_log10_offset), -10.f);
+        const int nrem = p.fb_mels - c0;
+        float *o = optr + (long long)c0 * cstride;
+        if (nrem >= 16 && vec4) {
+            if (valid) {
+#pragma unroll
+                for (int c = 0; c < 16; c += 4) *reinterpret_cast<float4 *>(o + c) = make_float4(v[c], v[c + 1], v[c + 2], v[c + 3]);
+            }
+        } else {
+#pragma unroll
+            for (int c = 0; c < 16; ++c) {
+                if (valid && c < nrem) *o = v[c];
+                o += cstride;
+            }
+        }
+    }
+    tc_fence_before();
+    __syncwarp();
+    if (lane == 0) mbar_arrive_remote(acc_empty_bar);
+}
+
 // Address of output element `idx` (elements of 4 bytes, or of 2 bytes with a 16-bit MELT_OPT_OUTPUT_DTYPE).
 __device__ __forceinline__ float *out_at(const K2Params &p, long long idx) {
     return p.out_dtype == 0 ? p.out + idx : reinterpret_cast<float *>(reinterpret_cast<unsigned short *>(p.out) + idx);
@@ -368,7 +431,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
     // stage, log-Mel) the epilogue warps and the converter warps together; MODE 2 (log-Mel) there are no epilogue warps -- they
     // form a third converter group and every converter warp drains a third of the bins of the previous tile; MODE 3 (log-Mel):
     // four drain warps AND three converter groups, 640 threads (launch_one says which is used when).
-    constexpr bool SHARE = MODE != 0 && MODE != 3;
+    constexpr bool SHARE = MODE == 1 || MODE == 2;
+    constexpr bool FB = MODE == 4;                                        // conventional front end: filterbank product after the power (see epi_fbank)
+    static_assert(!FB || (STREAM && !DIRECT && !RAGGED && PREC == P2_COMP), "MODE 4: dense batches, streamed basis, compensated operands");
     constexpr int NG = (MODE == 2 || MODE == 3) ? V2_CONV_GROUPS : V2_CONV_GROUPS - 1;   // converter groups: 3 without epilogue warps, 2 next to them
     constexpr int NT = v2_threads(MODE);                                  // threads of the block
     constexpr int CONV0 = MODE == 2 ? W_EPI0 : W_CONV0;                   // first converter warp
@@ -438,6 +503,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
         for (int i = t64; i < n_b; i += 64) { mbar_init(BAR(V_B_FULL + i), 1u); mbar_init(BAR(V_B_PEER + i), 1u); }
         if (t64 < 8) mbar_init(BAR(V_B_EMPTY + t64), 2u);                                // both issuers release a slab
         if (t64 == 8) mbar_init(BAR(V_DONE), 2u);                                        // both MMA issuers
+        if (FB && t64 == 9) mbar_init(BAR(V_P_READY), 8u);                               // the four epilogue warps of both CTAs
+        if (FB && t64 >= 10 && t64 < 13) mbar_init(BAR(V_D2_FULL + (t64 - 10)), 1u);     // D2_FULL, FB_FULL, FB_PEER
         fence_barrier_init();
     }
     if (p.n_mfcc > 0)
@@ -757,6 +824,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
             } else {
                 // long windows: the K-step slabs of every tile stream from L2 through a ring of b_slots slabs; the issuers
                 // release a slab (multicast tcgen05.commit to both CTAs) when its MMAs have completed
+                if constexpr (FB) {   // the filterbank image of this CTA (its half of the filter rows): resident for the whole launch
+                    const uint32_t fb_bytes = 2u * (uint32_t)p.fb_units * p.fb_kind_bytes;
+                    if (elect_one()) {
+                        mbar_arrive_expect_tx(BAR(V_FB_FULL), fb_bytes);
+                        bulk_g2s(sbase + p.off_fb, p.fb_img + (size_t)rank * fb_bytes, fb_bytes, BAR(V_FB_FULL));
+                    }
+                    __syncwarp();
+                }
                 int slot = 0;
                 uint32_t ph = 0;
                 for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
@@ -783,6 +858,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
         // with three busy converter / epilogue warps could not keep up with.
         if (STREAM && rank == 1 && warp == W_MMA && first_tile < n_tiles) {
             // streamed basis: this (otherwise idle) warp of the peer CTA tells the leader when a slab of the peer half has landed
+            if constexpr (FB) {   // and, once, when the peer half of the filterbank image has
+                mbar_wait(BAR(V_FB_FULL), 0);
+                if (lane == 0) mbar_arrive_remote(mapa_cluster(BAR(V_FB_PEER), 0));
+                __syncwarp();
+            }
             int slot = 0;
             uint32_t ph = 0;
             for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
@@ -812,6 +892,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
             int aslot = 0, stage = 0;
             uint32_t aph = 0, sph = 0;
             bool basis_pending = true;
+            bool fb_pending = true;   // MODE 4
+            uint32_t pph = 0;         // MODE 4: phase of P_READY
             constexpr bool b_res = !STREAM;
             const int b_slots = p.b_slots;
             int bslot = 0;          // streamed basis: ring slot of the next K-step's slab (resident basis: slot = K-step)
@@ -886,6 +968,32 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                     if (++aslot == a_slots) { aslot = 0; aph ^= 1u; }
                 }
                 basis_pending = false;
+                if constexpr (FB) {
+                    if (which == 0) {
+                        // the filterbank product of this tile (issuer R only): A = the power the epilogue warps of both CTAs wrote over R
+                        // (bf16 hi | mid column groups), B = the filterbank slabs, D2 = the columns of I (single accumulator stage)
+                        if (fb_pending) { mbar_wait(BAR(V_FB_FULL), 0); mbar_wait_cluster(BAR(V_FB_PEER), 0); fb_pending = false; }
+                        mbar_wait(BAR(V_P_READY), pph);
+                        pph ^= 1u;
+                        tc_fence_after();
+                        if (elect_one()) {
+                            const uint32_t idesc2 = umma_idesc(UMMA_BF16, (uint32_t)p.fb_nb, 256u);
+                            const uint32_t fb0 = sbase + p.off_fb;
+                            const uint64_t fd_hi = umma_smem_desc_kmajor_noswz(fb0, 128, 256);
+                            const uint64_t fd_mid = umma_smem_desc_kmajor_noswz(fb0 + p.fb_kind_bytes, 128, 256);
+                            const uint64_t fstep = (uint64_t)((2u * p.fb_kind_bytes) >> 4);
+                            const uint32_t d2 = tmem_base + (uint32_t)p.nb;
+                            for (int s2 = 0; s2 < p.fb_units; ++s2) {
+                                const uint32_t a_hi = tmem_base + 16u * (uint32_t)s2;
+                                umma2_ts_f16(d2, a_hi, fd_hi + (uint64_t)s2 * fstep, idesc2, s2 > 0);     // hi . hi
+                                umma2_ts_f16(d2, a_hi + 8, fd_hi + (uint64_t)s2 * fstep, idesc2, 1);      // mid . hi
+                                umma2_ts_f16(d2, a_hi, fd_mid + (uint64_t)s2 * fstep, idesc2, 1);         // hi . mid
+                            }
+                            tc_commit2(BAR(V_D2_FULL), 3);
+                        }
+                        __syncwarp();
+                    }
+                }
                 if (++stage == acc_stages) { stage = 0; sph ^= 1u; }
             }
             // Nobody waits for the last operand-slot releases (tcgen05.commit arrivals, multicast to both CTAs).  They must not
@@ -957,7 +1065,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
             TRACE(31);
             tc_fence_after();
             const uint32_t t_r = lane_taddr + (uint32_t)stage * (uint32_t)p.acc_cols, t_i = t_r + (uint32_t)p.nb;
-            if (SHARE || MODE == 3) {
+            if constexpr (FB) {
+                epi_fbank(p, t_r, t_i, optr, cstride, valid, lane, mapa_cluster(BAR(V_P_READY), 0), BAR(V_D2_FULL), (uint32_t)((tl - 1) & 1),
+                          acc_empty_remote + (uint32_t)stage * 8u);
+            } else if (SHARE || MODE == 3) {
                 // single accumulator stage, log-Mel: this warp drains every third 16-bin block, the two converter warps of the
                 // lane quarter the others (MODE 3: plain log-Mel, this warp drains every block)
                 epi_fast_share(t_r, t_i, p.nb, nm, RAGGED ? out_at(p, (out_row0 + lane) * p.n_ch + c_off) : (p.feature_major ? out_at(p, ((long long)b * p.n_ch + c_off) * T + t0 + row) : out_at(p, (ti.f0 + t0 + row) * p.n_ch + c_off)),

@@ -40,7 +40,9 @@ static void free_device(melt_plan *p) {
     cudaFree(p->d_tab);
     cudaFree(p->d_dct);
     cudaFree(p->d_bimg2);
+    cudaFree(p->d_fbimg);
     p->d_bimg2 = nullptr;
+    p->d_fbimg = nullptr;
     p->v2_ok = false;
     p->d_bimg = nullptr;
     p->d_tab = nullptr;
@@ -70,7 +72,7 @@ int plan_build_device(melt_plan *p) {
     const double centre = 0.5 * (double)c2;
 
     // ---- tiling of the contraction and of the Mel bins
-    k.n_fft = N; k.hop = H; k.n_mels = M; k.n_mfcc = p->n_mfcc; k.n_ch = p->n_mfcc > 0 ? p->n_mfcc : M;
+    k.n_fft = N; k.hop = H; k.n_mels = M; k.n_mfcc = p->n_mfcc; k.n_ch = p->fb_mels > 0 ? p->fb_mels : (p->n_mfcc > 0 ? p->n_mfcc : M);   // (conventional plan: M DFT bins in, fb_mels filters out)
     k.kstep = operand_kstep(kind);
     k.units = (k.kf + k.kstep - 1) / k.kstep;
     k.nk = comp ? 4 : 2;
@@ -276,6 +278,8 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
     const bool out16 = p->out_dtype != MELT_DTYPE_F32;
     if (out16 && (p->n_mfcc > 0 || p->output != MELT_OUTPUT_LOG || tap))
         return fail(MELT_ERR_UNSUPPORTED, "16-bit output: log-Mel output (n_mfcc == 0, MELT_OUTPUT_LOG, no tap) only");
+    if (p->fb_mels > 0 && (offsets || tap || !p->v2_ok))
+        return fail(MELT_ERR_UNSUPPORTED, "conventional (STFT + Mel filterbank) plan: dense batches through melt_forward / melt_forward_host only");
     const bool whisper = p->output == MELT_OUTPUT_LOG_WHISPER;
     if (whisper && (offsets || tap)) return fail(MELT_ERR_UNSUPPORTED, "Whisper-normalised output: dense batches without tap only");
     if (n_clips < 0) return fail(MELT_ERR_INVALID_ARG, "negative clip count");
@@ -381,8 +385,10 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
 
 using namespace melt;
 
-extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window, int n_mels, double fmin, double fmax,
-                                       int mel_scale, int n_mfcc) {
+// fb_mels = 0: the MelT / MFCCT plan of the paper.  fb_mels > 0 (melt_plan_create_stft_mel): the conventional front end -- the
+// projection runs on the N/2 + 1 DFT bins (n_mels = their number) and a triangular filterbank of fb_mels filters follows the power.
+static melt_plan *create_impl(double fs, int n_fft, int hop, int window, int n_mels, double fmin, double fmax,
+                              int mel_scale, int n_mfcc, int fb_mels) {
     if (!(fs > 0.0) || !std::isfinite(fs)) { set_error("fs must be positive"); return nullptr; }
     if (n_fft < 2 || n_fft > 65536) { set_error("n_fft=%d out of range [2, 65536]", n_fft); return nullptr; }
     if (hop < 1 || hop > 65535) { set_error("hop=%d out of range [1, 65535]", hop); return nullptr; }
@@ -407,6 +413,7 @@ extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window
     p->mel_scale = mel_scale; p->n_mfcc = n_mfcc;
     p->layout = MELT_LAYOUT_FRAME_MAJOR; p->precision = MELT_PREC_COMPENSATED; p->drop_last = 0; p->pad = MELT_PAD_NONE;
     p->in_scale_log2 = 12; p->output = MELT_OUTPUT_LOG; p->input_ready = 0; p->out_dtype = MELT_DTYPE_F32; p->eps_exp10 = -10; p->used.store(false); p->device = dev; p->sm_count = prop.multiProcessorCount;
+    p->fb_mels = fb_mels; p->d_fbimg = nullptr;
     p->d_bimg = nullptr; p->d_bimg2 = nullptr; p->v2_ok = false; p->v2_sigma = 0; p->d_tab = nullptr; p->d_dct = nullptr;
     p->pool = nullptr; p->copy_in = nullptr; p->copy_out = nullptr;
     memset(&p->kp, 0, sizeof(p->kp));
@@ -430,6 +437,21 @@ extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window
     p->centres.resize(n_mels);
     const double mlo = hz_to_mel(fmin), mhi = hz_to_mel(fmax);
     for (int m = 0; m < n_mels; ++m) p->centres[m] = mel_to_hz(mlo + (double)(m + 1) * (mhi - mlo) / (double)(n_mels + 1));
+    if (fb_mels > 0) {
+        // conventional front end: analysis frequencies = the DFT bins k fs / N, k = 0 .. N/2, then
+        // F[m][k] = max(0, min((f_k - e_m) / (e_{m+1} - e_m), (e_{m+2} - f_k) / (e_{m+2} - e_{m+1}))) with the M + 2 edges e uniform
+        // in HTK mel between fmin and fmax (their interior points are the MelT centres); peak 1, no normalisation
+        for (int k = 0; k < n_mels; ++k) p->centres[k] = (double)k * fs / (double)n_fft;
+        std::vector<double> e((size_t)fb_mels + 2);
+        for (int i = 0; i < fb_mels + 2; ++i) e[i] = mel_to_hz(mlo + (double)i * (mhi - mlo) / (double)(fb_mels + 1));
+        p->fb.assign((size_t)fb_mels * n_mels, 0.0);
+        for (int m = 0; m < fb_mels; ++m)
+            for (int k = 0; k < n_mels; ++k) {
+                const double f = p->centres[k];
+                const double up = (f - e[m]) / (e[m + 1] - e[m]), down = (e[m + 2] - f) / (e[m + 2] - e[m + 1]);
+                p->fb[(size_t)m * n_mels + k] = std::max(0.0, std::min(up, down));
+            }
+    }
     p->win.resize(n_fft);
     for (int n = 0; n < n_fft; ++n) {
         if (window == MELT_WINDOW_HANN_PERIODIC) p->win[n] = 0.5 - 0.5 * std::cos(2.0 * kPi * n / n_fft);
@@ -437,7 +459,24 @@ extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window
         else p->win[n] = 1.0;
     }
     if (plan_build_device(p) != MELT_OK) { melt_plan_destroy(p); return nullptr; }
+    if (fb_mels > 0 && !p->v2_ok) {
+        set_error("melt_plan_create_stft_mel: geometry not covered (needs hop %% 4 == 0, an aligned fold and n_fft / 2 + 1 <= 224 bins: n_fft=%d hop=%d)", n_fft, hop);
+        melt_plan_destroy(p);
+        return nullptr;
+    }
     return p;
+}
+
+extern "C" melt_plan *melt_plan_create(double fs, int n_fft, int hop, int window, int n_mels, double fmin, double fmax,
+                                       int mel_scale, int n_mfcc) {
+    return create_impl(fs, n_fft, hop, window, n_mels, fmin, fmax, mel_scale, n_mfcc, 0);
+}
+
+extern "C" melt_plan *melt_plan_create_stft_mel(double fs, int n_fft, int hop, int window, int n_mels, double fmin, double fmax) {
+    if (n_mels < 1 || n_mels > 128) { set_error("n_mels=%d out of range [1, 128] for the conventional front end", n_mels); return nullptr; }
+    if (n_fft < 2 || (n_fft & 1) || n_fft / 2 + 1 > 224) { set_error("melt_plan_create_stft_mel: n_fft=%d must be even with n_fft / 2 + 1 <= 224 bins", n_fft); return nullptr; }
+    if (!(fmin >= 0.0) || !(fmax > fmin)) { set_error("need 0 <= fmin < fmax"); return nullptr; }
+    return create_impl(fs, n_fft, hop, window, n_fft / 2 + 1, fmin, fmax, MELT_MEL_HTK, 0, n_mels);
 }
 
 extern "C" void melt_plan_destroy(melt_plan *p) {
@@ -452,6 +491,9 @@ extern "C" void melt_plan_destroy(melt_plan *p) {
 extern "C" int melt_plan_set_option(melt_plan *p, int key, int value) {
     if (!p) return fail(MELT_ERR_INVALID_ARG, "plan is NULL");
     if (p->used.load()) return fail(MELT_ERR_INVALID_ARG, "plan is immutable after its first forward call");
+    if (p->fb_mels > 0 && ((key == MELT_OPT_PRECISION && value != MELT_PREC_COMPENSATED) || (key == MELT_OPT_OUTPUT && value != MELT_OUTPUT_LOG) ||
+                           (key == MELT_OPT_OUTPUT_DTYPE && value != MELT_DTYPE_F32)))
+        return fail(MELT_ERR_UNSUPPORTED, "conventional (STFT + Mel filterbank) plan: compensated precision, log10 output, fp32 only");
     switch (key) {
         case MELT_OPT_LAYOUT:
             if (value < 0 || value > 1) return fail(MELT_ERR_INVALID_ARG, "bad layout %d", value);
@@ -631,6 +673,7 @@ extern "C" int melt_forward_ragged_noalloc(const melt_plan *p, const float *x, c
     if (!offsets) return fail(MELT_ERR_INVALID_ARG, "offsets is NULL");
     int rc = validate_common(p, x, out_any);
     if (rc) return rc;
+    if (p->fb_mels > 0) return fail(MELT_ERR_UNSUPPORTED, "conventional (STFT + Mel filterbank) plan: dense batches only");
     float *out = static_cast<float *>(out_any);
     const bool out16 = p->out_dtype != MELT_DTYPE_F32;
     if (out16 && (p->n_mfcc > 0 || p->output != MELT_OUTPUT_LOG))

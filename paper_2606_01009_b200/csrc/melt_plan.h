@@ -105,6 +105,11 @@ struct K2Params {
     int direct;                // very long windows: K-step staging (the loader stages two runs of kstep + 4 samples per frame and K-step)
     int b_resident, b_slots;   // basis half resident in shared memory (b_slots = units), or streamed through a ring of b_slots K-step slabs
     const float *dct;      // [n_mels][dct_pitch]
+    // ---- conventional front end (melt_plan_create_stft_mel; MODE 4 of the kernel): the nb "bins" are the DFT bins 0 .. N/2, and a
+    //      second tensor-core product with the triangular Mel filterbank follows their power.  fb_mels = 0: not in use.
+    int fb_mels, fb_nb, fb_units;      // Mel filters, padded to a multiple of 16 (N of the second MMA), K-steps of 16 bins (= nb / 16)
+    uint32_t fb_kind_bytes, off_fb;    // bytes of one K-step slab of one operand kind in this CTA (fb_nb / 2 rows x 32 B); where the image sits
+    const uint8_t *fb_img;             // [2 ranks][fb_units][hi, mid][fb_nb / 2 rows][16 bins] bf16, no-swizzle K-major slabs
     // ---- per-unit shared-memory byte offsets (relative to the first sample of the thread's frame)
     short tab[V2_MAX_UNITS][V2_TAB];
     // ---- implicit im2col by the tensor-map engine: 3-D map over the raw signal, dims (sample-in-row: pitch words,
@@ -123,6 +128,9 @@ struct melt_plan {
     double fs, fmin, fmax;
     int n_fft, hop, window, n_mels, mel_scale, n_mfcc;
     int layout, precision, drop_last, pad, in_scale_log2, output, input_ready, out_dtype, eps_exp10;
+    int fb_mels;                       // > 0: conventional STFT + Mel filterbank plan (n_mels = n_fft / 2 + 1 DFT bins, fb_mels filters)
+    std::vector<double> fb;            // its filterbank F[m][k], fb_mels x n_mels, fp64
+    uint8_t *d_fbimg;
     mutable std::atomic<bool> used;    // set by the first forward call: options are frozen from then on
     int device, sm_count;
     std::vector<double> centres, win;
@@ -146,6 +154,7 @@ int launch_forward(const melt_plan *p, const KParams &kp, cudaStream_t stream);
 int plan_build_v2(melt_plan *p);   // fills p->k2 / p->v2_ok (never fails the plan: v1 remains the general path)
 bool v2_accepts(const melt_plan *p, const float *x, long long len);
 int launch_forward2(const melt_plan *p, const K2Params &kp, cudaStream_t stream);
+int launch_forward2_fb(const K2Params &kp, int grid, int sigma, cudaStream_t stream);   // MODE 4 instantiations (melt_forward2_fb.cu)
 int launch_reflect_pad(const float *x, float *xp, int batch, long long len, int pad, long long plen, cudaStream_t stream);
 int v2_encode_tmap(K2Params &kp);
 int v2_encode_tmap_ragged(K2Params &kp);   // 2-D map over the packed buffer (any start sample, rows of `hop` samples)   // fills kp.tmap / kp.tma_rows for this call's (x, len, batch); never fails the call
