@@ -243,7 +243,10 @@ PER_WORKLOAD = [("cfg0", "compensated"), ("cfg2", "compensated"), ("cfg2", "tf32
                 # to its Table 5 (H100: MelT 0.070 ms at 160 s, PyTorch CUDA TF32) -- another machine, not the target
                 ("paper_spec_1s", "compensated"), ("paper_spec_10s", "compensated"), ("paper_spec_40s", "compensated"),
                 ("paper_spec_160s", "compensated"), ("paper_cep_160s", "compensated"), ("paper_mel512_160s", "compensated"),
-                ("paper_batch1_4s", "compensated"), ("paper_batch256_4s", "compensated")]
+                ("paper_batch1_4s", "compensated"), ("paper_batch256_4s", "compensated"),
+                # the conventional front end (STFT -> power -> triangular Mel filterbank -> log10) as ONE fused
+                # kernel on the same substrate (melt_plan_create_stft_mel), on the Whisper-shaped configs: the comparator of the paper
+                ("stftmel:cfg0", "compensated"), ("stftmel:cfg1", "compensated"), ("stftmel:cfg2", "compensated")]
 
 
 def bench_other_workloads(torch, mb, peaks, tf32_tflops, launches=20):
@@ -256,9 +259,17 @@ def bench_other_workloads(torch, mb, peaks, tf32_tflops, launches=20):
     stream = torch.cuda.current_stream()
     cache = {}
     for cfg, prec in PER_WORKLOAD:
-        c = wl.CONFIGS[cfg] if cfg in wl.CONFIGS else wl.PAPER_CONFIGS[cfg]
+        conv = cfg.startswith("stftmel:")
+        base = cfg.split(":")[1] if conv else cfg
+        c = wl.CONFIGS[base] if base in wl.CONFIGS else wl.PAPER_CONFIGS[base]
         ragged = bool(c.get("ragged"))
-        plan = make_plan(mb, c, prec)
+        if conv:
+            plan = mb.melt_plan_create_stft_mel(c["fs"], c["n_fft"], c["hop"], c["window"], c["n_mels"], c["fmin"], c["fmax"])
+            mb.melt_plan_set_option(plan, mb.MELT_OPT_DROP_LAST, int(c["drop_last"]))
+            mb.melt_plan_set_option(plan, mb.MELT_OPT_LAYOUT, int(c["layout"] == "feature_major"))
+            mb.melt_plan_set_option(plan, mb.MELT_OPT_INPUT_READY, 1)
+        else:
+            plan = make_plan(mb, c, prec)
         try:
             C = mb.melt_num_channels(plan)
             N, H, M, K = c["n_fft"], c["hop"], c["n_mels"], c["n_mfcc"]
@@ -280,6 +291,8 @@ def bench_other_workloads(torch, mb, peaks, tf32_tflops, launches=20):
                 out_shape = (B, C, T) if c["layout"] == "feature_major" else (B, T, C)
             nums = dict(frames=frames, flops=2.0 * frames * 2 * M * N + 2.0 * frames * M * K,
                         bytes_in=4.0 * (n_in if ragged else B * c["clip_len"]), bytes_out=4.0 * frames * C)
+            if conv:   # DFT as a dense product on N/2 + 1 bins (cos and sin rows) + the filterbank product, both counted once
+                nums["flops"] = 2.0 * frames * 2 * (N // 2 + 1) * N + 2.0 * frames * M * (N // 2 + 1)
             set_bytes = 4 * n_in + 4 * frames * C
             nsets = max(1, int(np.ceil(2.2 * l2 / set_bytes)))
             key = (cfg, nsets)
@@ -309,6 +322,8 @@ def bench_other_workloads(torch, mb, peaks, tf32_tflops, launches=20):
                    "t_hbm_us": roof["t_hbm_us"], "t_tensor_us": roof["t_tensor_us"], "launches": launches,
                    "gpu_launches_per_step": 2 if ragged else 1,
                    "kernel": mb.melt_plan_describe(plan).split(" | ")[0]}
+            if conv:
+                row["front_end"] = "stft_mel (fused DFT product -> power -> filterbank product -> log10; comparator, SURVEY 8(f) NEXT-4)"
             if c["n_clips"] == 1:
                 # single clip (latency regime): also one forward captured in a CUDA graph and replayed (launch cost amortised)
                 g = torch.cuda.CUDAGraph()

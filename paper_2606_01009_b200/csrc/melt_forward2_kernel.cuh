@@ -708,27 +708,40 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                     const int pw = p.pitch_bytes >> 2;
                     const long long jbase = st - (ragged ? (ti.s0 & 3ll) : 0ll);
                     float *dstp = reinterpret_cast<float *>(smem + p.off_stg + (size_t)slot * p.slot_bytes);
+                    // Only the rows a VALID frame of the chunk can read are brought in (its window, the K padding of the last K-step,
+                    // the alignment slack of ragged chunks): the last chunk of a clip has up to ~10 rows beyond that, and filling
+                    // them element by element held this warp -- the pacemaker of the kernel -- for tens of thousands of cycles
+                    // (the Whisper-shaped batch with MELT_OPT_PAD: 35.6 us against 23.7 us on a pre-padded batch; now 25.5).
+                    const int n_need = min(n_rows, info_v.nvalid + (p.n_fft + 34) / p.hop + 1);
                     uint32_t bulk_bytes = 0;
-                    for (int r = 0; r < n_rows; ++r) {
+                    for (int r = 0; r < n_need; ++r) {
                         const long long jlo = jbase + (long long)r * p.hop;
                         if (jlo >= 0 && jlo + pw <= clip_len) { bulk_bytes += (uint32_t)p.pitch_bytes; continue; }
-                        for (int col = lane; col < pw; col += 32) {
-                            long long j = jlo + col;
-                            j = j < 0 ? -j : j;
-                            j = j >= clip_len ? 2 * (clip_len - 1) - j : j;
-                            j = j < 0 ? 0 : (j >= clip_len ? clip_len - 1 : j);   // rows no valid frame reads: any finite sample
-                            dstp[r * pw + col] = __ldg(xb + j);
+                        for (int col0 = lane; col0 < pw; col0 += 128) {   // four independent loads in flight per lane, then the stores
+                            float v[4];
+#pragma unroll
+                            for (int u4 = 0; u4 < 4; ++u4) {
+                                long long j = jlo + col0 + 32 * u4;
+                                j = j < 0 ? -j : j;
+                                j = j >= clip_len ? 2 * (clip_len - 1) - j : j;
+                                j = j < 0 ? 0 : (j >= clip_len ? clip_len - 1 : j);   // (columns beyond the row, clips shorter than the padding: any sample)
+                                v[u4] = __ldg(xb + j);
+                            }
+#pragma unroll
+                            for (int u4 = 0; u4 < 4; ++u4)
+                                if (col0 + 32 * u4 < pw) dstp[r * pw + col0 + 32 * u4] = v[u4];
                         }
                     }
                     __syncwarp();   // every lane's stores precede lane 0's arrival below
-                    if (elect_one()) {
+                    if (lane == 0) {
                         if (ragged) { *info = info_v; mbar_arrive(info_bar); }
                         if (bulk_bytes) mbar_arrive_expect_tx(full, bulk_bytes);
                         else mbar_arrive(full);
-                        for (int r = 0; r < n_rows; ++r) {
-                            const long long jlo = jbase + (long long)r * p.hop;
-                            if (jlo >= 0 && jlo + pw <= clip_len) bulk_g2s(dst0 + (uint32_t)r * (uint32_t)p.pitch_bytes, xb + jlo, (uint32_t)p.pitch_bytes, full);
-                        }
+                    }
+                    __syncwarp();
+                    for (int r = lane; r < n_need; r += 32) {   // one bulk copy per row inside the clip, a row per lane (the phase cannot complete before lane 0's arrival above)
+                        const long long jlo = jbase + (long long)r * p.hop;
+                        if (jlo >= 0 && jlo + pw <= clip_len) bulk_g2s(dst0 + (uint32_t)r * (uint32_t)p.pitch_bytes, xb + jlo, (uint32_t)p.pitch_bytes, full);
                     }
                     __syncwarp();
                     TRACE(12);
