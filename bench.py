@@ -160,9 +160,15 @@ def torch_context(cfg, c, x_dev, steps=20):
     return out
 
 
+FRONT_END = "melt"   # --front-end: "melt" (the paper's method, the default) or "stft_mel" (the fused conventional comparator, NEXT-4)
+
+
 def make_plan(mb, c, precision, input_ready=True):
-    plan = mb.melt_plan_create(*wl.plan_args(c))
-    mb.melt_plan_set_option(plan, mb.MELT_OPT_PRECISION, PREC_NAMES[precision])
+    if FRONT_END == "stft_mel":
+        plan = mb.melt_plan_create_stft_mel(c["fs"], c["n_fft"], c["hop"], c["window"], c["n_mels"], c["fmin"], c["fmax"])
+    else:
+        plan = mb.melt_plan_create(*wl.plan_args(c))
+        mb.melt_plan_set_option(plan, mb.MELT_OPT_PRECISION, PREC_NAMES[precision])
     mb.melt_plan_set_option(plan, mb.MELT_OPT_DROP_LAST, int(c["drop_last"]))
     mb.melt_plan_set_option(plan, mb.MELT_OPT_LAYOUT, int(c["layout"] == "feature_major"))
     # the inputs are resident in HBM long before the timed region: consecutive forwards may read x while the previous kernel
@@ -393,6 +399,16 @@ def time_oracle(cfg, n_clips_sample, reps):
     kw = dict(fs=c["fs"], n_fft=c["n_fft"], hop=c["hop"], window_kind=c["window"], n_mels=c["n_mels"], fmin=c["fmin"],
               fmax=c["fmax"], n_mfcc=c["n_mfcc"], drop_last=c["drop_last"], want=("L", "C"))
     frames = 0
+    if FRONT_END == "stft_mel":        # the conventional front end's own oracle (numpy fp64; the FFT runs on one core)
+        from oracle import stft_mel_oracle as so
+        skw = dict(fs=c["fs"], n_fft=c["n_fft"], hop=c["hop"], window_kind=c["window"], n_mels=c["n_mels"], fmin=c["fmin"],
+                   fmax=c["fmax"], drop_last=c["drop_last"], want=("L",))
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            for xc in d["x"]:
+                frames += so.forward(xc, **skw)["L"].shape[0]
+        dt = time.perf_counter() - t0
+        return frames / dt, dt, 1, frames
     if d.get("offsets") is not None:   # ragged: clips packed back to back
         off = d["offsets"]
         clips = [d["x"][off[i]:off[i + 1]] for i in range(len(off) - 1)]
@@ -413,19 +429,22 @@ def run_reference(args):
         return
     cfg = args.workload
     c = wl.CONFIGS[cfg]
+    global FRONT_END
+    FRONT_END = args.front_end
     for _ in range(max(1, args.warmup)):
         fps0, _, _, fr0 = time_oracle(cfg, 1, 1)
     # bounded sample: as many clips per step (<= --cpu-clips) as keep the whole K-step run near one minute
     sample_clips = max(1, min(args.cpu_clips, int(60.0 * fps0 / (max(1, args.steps) * max(1, fr0)))))
     fps, dt, cores, frames = time_oracle(cfg, sample_clips, args.steps)
-    sample = "%d of %d clips of %s per step (%d frames), fp64 direct sums, OpenMP over frames" % (
-        sample_clips, c["n_clips"], cfg, frames // max(1, args.steps))
+    sample = "%d of %d clips of %s per step (%d frames), %s" % (
+        sample_clips, c["n_clips"], cfg, frames // max(1, args.steps),
+        "fp64 direct sums, OpenMP over frames" if FRONT_END == "melt" else "conventional front end: fp64 numpy rfft -> power -> filterbank product -> log10")
     line = {
         "impl": "reference", "metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "audio_s_per_s": fps * c["hop"] / c["fs"],
-        "config": {"workload": cfg, "sample": sample, "n_fft": c["n_fft"], "hop": c["hop"], "n_mels": c["n_mels"]},
+        "config": {"workload": cfg if FRONT_END == "melt" else "stftmel:" + cfg, "sample": sample, "n_fft": c["n_fft"], "hop": c["hop"], "n_mels": c["n_mels"]},
         "cpu_baseline": {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": fps, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }
@@ -440,6 +459,9 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="cfg1", choices=list(wl.CONFIGS))
     ap.add_argument("--precision", default="compensated", choices=list(PREC_NAMES))
+    ap.add_argument("--front-end", default="melt", choices=["melt", "stft_mel"],
+                    help="stft_mel: time the fused conventional STFT + Mel filterbank kernel (melt_plan_create_stft_mel) on the workload instead "
+                         "of MelT (dense log-Mel configs, compensated precision; --impl cuda only)")
     ap.add_argument("--clips", type=int, default=0, help="clips per GPU (default: the config's)")
     ap.add_argument("--buffer-sets", type=int, default=0, help="rotating input/output sets (default: enough to exceed 2x L2)")
     ap.add_argument("--cpu-clips", type=int, default=8, help="clips in the oracle sample")
@@ -475,6 +497,13 @@ def main():
     n_clips = args.clips or c["n_clips"]
     ragged = bool(c.get("ragged"))
     nums = None if ragged else workload_numbers(cfg, n_clips)
+    global FRONT_END
+    FRONT_END = args.front_end
+    if FRONT_END == "stft_mel":
+        if ragged or c["n_mfcc"] or args.precision != "compensated":
+            raise SystemExit("--front-end stft_mel: dense log-Mel configs, compensated precision")
+        nb_ = c["n_fft"] // 2 + 1   # DFT product on N/2 + 1 bins (cos and sin rows) + filterbank product, each counted once
+        nums["flops"] = 2.0 * nums["frames"] * 2 * nb_ * c["n_fft"] + 2.0 * nums["frames"] * c["n_mels"] * nb_
     peaks = load_peaks()
 
     # ---- plan
@@ -644,7 +673,7 @@ def main():
                  "tensor_peak_dtype": dtype, "tf32_tflops_measured": tf32_cublas, "tf32_tflops_peak_used": tf32_tflops,
                  "algorithmic_bytes": nums["bytes_in"] + nums["bytes_out"], "algorithmic_flops": nums["flops"],
                  "frac_vs_tf32_roofline": max(roof["t_hbm_us"] * 1e-6, nums["flops"] / (tf32_tflops * 1e12)) / (kernel_ms * 1e-3)})
-    prof = os.path.join(ROOT, "profiles", "traffic_%s_%s.json" % (cfg, args.precision))
+    prof = os.path.join(ROOT, "profiles", "traffic_%s%s_%s.json" % ("stftmel_" if FRONT_END == "stft_mel" else "", cfg, args.precision))
     if os.path.exists(prof):
         with open(prof) as fh:
             roof["traffic"] = json.load(fh).get("dram_bytes_per_launch")
@@ -675,7 +704,7 @@ def main():
         "metric": METRIC, "value": value, "unit": "frames/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": dtype,
         "data": "synthetic", "audio_s_per_s": value * c["hop"] / c["fs"],
-        "config": {"workload": cfg, "clips_per_gpu": B, "clip_samples": int(L), "frames_per_step_per_gpu": nums["frames"],
+        "config": {"workload": cfg if FRONT_END == "melt" else "stftmel:" + cfg, "clips_per_gpu": B, "clip_samples": int(L), "frames_per_step_per_gpu": nums["frames"],
                    "n_fft": c["n_fft"], "hop": c["hop"], "n_mels": c["n_mels"], "n_mfcc": c["n_mfcc"], "layout": c["layout"],
                    "precision": args.precision, "parallelism": "dp%d (independent shards, no collective)" % world,
                    "l2_policy": "rotating %d input/output buffer sets, %.0f MB total > 2x L2 (%.0f MB)" % (
