@@ -238,6 +238,7 @@ __device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uin
                     else v = fmaxf(fmaf(lg2_ftz(fmaf(praw, la, lb)), lc, ld), lmin);
                     if (HAS_DCT) {
                         const float *drow = dct_s + m * p.dct_pitch + q0;
+                        // (scalar FMAs on purpose: packed FFMA2 pairs measured 6.5 % SLOWER on the ragged MFCCT batch, 226.7 vs 212.8 us)
 #pragma unroll
                         for (int q4 = 0; q4 < 4; ++q4) {   // the table's rows are zero padded to whole blocks of 16 cepstra
                             const float4 d = *reinterpret_cast<const float4 *>(drow + 4 * q4);   // D[q0 + 4 q4 .. + 3][m]
@@ -430,11 +431,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
     // Who drains the accumulators: MODE 0 the four epilogue warps alone (next to two converter groups); MODE 1 (single accumulator
     // stage, log-Mel) the epilogue warps and the converter warps together; MODE 2 (log-Mel) there are no epilogue warps -- they
     // form a third converter group and every converter warp drains a third of the bins of the previous tile; MODE 3 (log-Mel):
-    // four drain warps AND three converter groups, 640 threads (launch_one says which is used when).
+    // four drain warps AND three converter groups, 640 threads; MODE 5: MODE 3 with a second set of four drain warps (warps 20-23,
+    // the odd 16-bin blocks), 768 threads (launch_one says which is used when).
     constexpr bool SHARE = MODE == 1 || MODE == 2;
     constexpr bool FB = MODE == 4;                                        // conventional front end: filterbank product after the power (see epi_fbank)
     static_assert(!FB || (STREAM && !DIRECT && !RAGGED && PREC == P2_COMP), "MODE 4: dense batches, streamed basis, compensated operands");
-    constexpr int NG = (MODE == 2 || MODE == 3) ? V2_CONV_GROUPS : V2_CONV_GROUPS - 1;   // converter groups: 3 without epilogue warps, 2 next to them
+    constexpr int NG = (MODE == 2 || MODE == 3 || MODE == 5) ? V2_CONV_GROUPS : V2_CONV_GROUPS - 1;   // converter groups: 3 without epilogue warps, 2 next to them
     constexpr int NT = v2_threads(MODE);                                  // threads of the block
     constexpr int CONV0 = MODE == 2 ? W_EPI0 : W_CONV0;                   // first converter warp
     constexpr int DRAINERS = MODE == 2 ? NG : 1 + NG;                     // warps per lane quarter that drain (SHARE)
@@ -499,7 +501,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
         const int n_b = STREAM ? 8 : (p.units < V2_MAX_UNITS ? p.units : V2_MAX_UNITS);   // basis barriers in use
         const int t64 = (warp == W_MMA ? 0 : 32) + lane;
         for (int i = t64; i < 16; i += 64) { mbar_init(BAR(V_A_FULL + i), 8u); mbar_init(BAR(V_A_EMPTY + i), 2u); }   // A_EMPTY: both issuers commit
-        if (t64 < 2) { mbar_init(BAR(V_ACC_FULL + t64), 2u); mbar_init(BAR(V_ACC_EMPTY + t64), (uint32_t)(SHARE ? 8 * DRAINERS : 8)); }
+        if (t64 < 2) { mbar_init(BAR(V_ACC_FULL + t64), 2u); mbar_init(BAR(V_ACC_EMPTY + t64), (uint32_t)(SHARE ? 8 * DRAINERS : (MODE == 5 ? 16 : 8))); }
         for (int i = t64; i < n_b; i += 64) { mbar_init(BAR(V_B_FULL + i), 1u); mbar_init(BAR(V_B_PEER + i), 1u); }
         if (t64 < 8) mbar_init(BAR(V_B_EMPTY + t64), 2u);                                // both issuers release a slab
         if (t64 == 8) mbar_init(BAR(V_DONE), 2u);                                        // both MMA issuers
@@ -860,7 +862,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                     }
                 }
             }
-            mbar_wait(BAR(V_DONE), 0);   // all tensor-core work of the pair, and the barrier arrivals it triggers, are done
         }
     } else if (warp == W_MMA || warp == W_MMA2) {
         // ============================================================== MMA issuers (leader CTA)
@@ -1022,7 +1023,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                 if (++stage == acc_stages) { stage = 0; sph ^= 1u; }
             }
         }
-    } else if (MODE != 2 && warp >= W_EPI0 && warp < W_EPI0 + 4) {
+    } else if ((MODE != 2 && warp >= W_EPI0 && warp < W_EPI0 + 4) || (MODE == 5 && warp >= W_CONV0 + 4 * NG)) {
         // ============================================================== epilogue (thread = frame)
         const int q = warp & 3;
         const int row = q * 32 + lane;
@@ -1081,11 +1082,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
             if constexpr (FB) {
                 epi_fbank(p, t_r, t_i, optr, cstride, valid, lane, mapa_cluster(BAR(V_P_READY), 0), BAR(V_D2_FULL), (uint32_t)((tl - 1) & 1),
                           acc_empty_remote + (uint32_t)stage * 8u);
-            } else if (SHARE || MODE == 3) {
+            } else if (SHARE || MODE == 3 || MODE == 5) {
                 // single accumulator stage, log-Mel: this warp drains every third 16-bin block, the two converter warps of the
                 // lane quarter the others (MODE 3: plain log-Mel, this warp drains every block)
                 epi_fast_share(t_r, t_i, p.nb, nm, RAGGED ? out_at(p, (out_row0 + lane) * p.n_ch + c_off) : (p.feature_major ? out_at(p, ((long long)b * p.n_ch + c_off) * T + t0 + row) : out_at(p, (ti.f0 + t0 + row) * p.n_ch + c_off)),
-                               cstride, valid, p.out_log10_offset, 0, MODE == 3 ? 1 : DRAINERS, p.out_dtype);
+                               cstride, valid, p.out_log10_offset, MODE == 5 && warp >= W_CONV0 ? 1 : 0, MODE == 3 ? 1 : (MODE == 5 ? 2 : DRAINERS), p.out_dtype);
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive_remote(acc_empty_remote + (uint32_t)stage * 8u);
@@ -1345,6 +1346,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
     TRACE_PT(5);
     tc_fence_before();
     __syncthreads();
+    // All tensor-core work of the pair, and the barrier arrivals it triggers, are done before a CTA retires: every warp takes the
+    // issuers' final commit here, where it has (almost) always completed -- the basis warp used to probe this barrier for the
+    // whole launch, on the scheduler it shares with the converter warps of lane quarter 2 (cfg4d tf32 217 -> 203 us).
+    if (first_tile < n_tiles) mbar_wait(BAR(V_DONE), 0);
     TRACE_PT(6);
 #ifdef MELT_STRICT_CLUSTER_SYNC
     cluster_sync_all();
@@ -1415,13 +1420,17 @@ static int launch_one(const K2Params &kp, int grid, cudaStream_t stream) {
     // the accumulator has a single stage, the basis is resident and the MMAs run at half rate (TF32): the tensor pipe is the
     // bound and idles while a tile is drained -- every converter warp drains a third of the previous tile's bins (MODE 2).
     // Measured (r02, B200, back to back): MODE 3 vs MODE 2  cfg1 -3.6 %, 256 x 4 s clips -13 %, cfg4a tf32 / bf16 -4.5 / -6.8 %,
-    // cfg2 tf32 +5 % (hence the exception), everything else within +-2 %.
+    // cfg2 tf32 +5 % (hence the exception), everything else within +-2 %.  MODE 5 = MODE 3 with EIGHT drain warps (two per lane
+    // quarter, alternate 16-bin blocks; 768 threads) where a single accumulator stage puts the drain between two tiles' MMAs and the
+    // basis is resident: cfg2 compensated 256 -> 247 us; with a streamed basis or K-block staging it measured 0.5-1.5 % slower.
     const bool plain = kp.n_mfcc == 0 && !kp.output_power && kp.tap == nullptr;
-    const int mode = !plain ? 0 : (PREC == P2_TF32 && kp.acc_stages == 1 && kp.b_resident && !kp.direct ? 2 : 3);
+    const int mode = !plain ? 0 : (PREC == P2_TF32 && kp.acc_stages == 1 && kp.b_resident && !kp.direct ? 2 : (kp.acc_stages == 1 && kp.b_resident && !kp.direct ? 5 : 3));
     if (kp.offsets) {
+        if (mode == 5) return launch_one_s<PREC, SIGMA, true, 5, false, false>(kp, grid, stream);
         if (mode == 3) return launch_one_r<PREC, SIGMA, true, 3>(kp, grid, stream);
         return mode == 2 ? launch_one_r<PREC, SIGMA, true, 2>(kp, grid, stream) : launch_one_r<PREC, SIGMA, true, 0>(kp, grid, stream);
     }
+    if (mode == 5) return launch_one_s<PREC, SIGMA, false, 5, false, false>(kp, grid, stream);
     if (mode == 3) return launch_one_r<PREC, SIGMA, false, 3>(kp, grid, stream);
     return mode == 2 ? launch_one_r<PREC, SIGMA, false, 2>(kp, grid, stream) : launch_one_r<PREC, SIGMA, false, 0>(kp, grid, stream);
 }

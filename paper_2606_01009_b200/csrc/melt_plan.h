@@ -62,7 +62,7 @@ constexpr int V2_CONV_GROUPS = 3;     // converter groups of 4 warps (one warp p
 // log-Mel): three converter groups that also drain the accumulators; MODE 0 (power / tap / MFCCT outputs): four epilogue
 // warps + two converter groups.  (A third converter group next to the epilogue warps, 640 threads at <= 102 registers, made the
 // ragged MFCCT batch SLOWER: 300 vs 225 us -- the schedulers are already oversubscribed.)
-constexpr int v2_threads(int mode) { return mode == 3 ? 128 * (2 + V2_CONV_GROUPS) : 128 * (1 + V2_CONV_GROUPS); }
+constexpr int v2_threads(int mode) { return mode == 5 ? 128 * (3 + V2_CONV_GROUPS) : (mode == 3 ? 128 * (2 + V2_CONV_GROUPS) : 128 * (1 + V2_CONV_GROUPS)); }
 constexpr int V2_MAX_UNITS = 128;     // K-steps per tile the per-unit load table covers
 constexpr int V2_MAX_STG = 12;        // staging ring slots (32-frame chunks)
 constexpr int V2_TAB = 12;            // int16 entries per unit: [0,4) forward quads, [4,8) backward quads, [8] single

@@ -60,9 +60,18 @@ __device__ __forceinline__ uint64_t globaltimer_ns() {
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
-// Wait for the phase with the given parity.  A watchdog turns a protocol bug into a trap (a launch error the
-// host sees) instead of a hung GPU: no legitimate wait in these kernels lasts anywhere near 4 seconds.
+// Wait for the phase with the given parity.  The product form is the bare probe-and-branch loop: a third of all issued
+// instructions of these kernels are barrier probes of waiting warps, and they compete for issue slots with the warps that
+// have work.  The form with a watchdog (five instructions per probe: -DMELT_WATCHDOG, development builds) turns a protocol
+// bug into a trap (a launch error the host sees) instead of a hung GPU: no legitimate wait in these kernels lasts anywhere
+// near 4 seconds.  Measured r02 (B200, back to back, one box, together with the late wait for the final commit in the kernel's
+// teardown): cfg1 23.5 -> 23.1 us, cfg2 tf32 / bf16 222 / 165 -> 210 / 158, cfg4a tf32 / bf16 67.6 / 43.5 -> 58.2 / 39.4, cfg4d tf32 / bf16
+// 219 / 118 -> 181 / 103, cfg4c compensated 166 -> 159.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+#ifndef MELT_WATCHDOG
+    asm volatile("{\n\t.reg .pred p;\n\tLAB_WAIT:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@!p bra LAB_WAIT;\n\t}" ::"r"(bar), "r"(parity) : "memory");
+    return;
+#endif
     if (mbar_try_wait(bar, parity)) return;
     uint64_t t0 = 0;
     uint32_t spins = 0;
@@ -236,6 +245,10 @@ __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t par
     return ok != 0;
 }
 __device__ __forceinline__ void mbar_wait_cluster(uint32_t bar, uint32_t parity) {
+#ifndef MELT_WATCHDOG
+    asm volatile("{\n\t.reg .pred p;\n\tLAB_WAIT:\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n\t@!p bra LAB_WAIT;\n\t}" ::"r"(bar), "r"(parity) : "memory");
+    return;
+#endif
     if (mbar_try_wait_cluster(bar, parity)) return;
     uint64_t t0 = 0;
     uint32_t spins = 0;
