@@ -305,7 +305,7 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
             rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, tile_prefix, 32, st);   // exclusive prefix of 32-frame chunks per clip
             K2Params k2 = p->k2;
             k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = 0; k2.frames_per_clip = 0;
-            k2.tiles_per_clip = 0; k2.n_tiles = -1;
+            k2.chunks_per_clip = 0; k2.n_tiles = -1;
             k2.offsets = offsets; k2.frame_offsets = out_frame_offsets; k2.tile_prefix = tile_prefix;
             k2.vpad = reflect ? p->n_fft / 2 : 0;
             k2.out_dtype = p->out_dtype;
@@ -356,11 +356,12 @@ static int forward_impl(const melt_plan *p, const float *x, const long long *off
             k2.vpad = reflect ? p->n_fft / 2 : 0;
             k2.input_ready = input_ready ? 1 : 0;
         }
-        const long long tpc2 = (T + 255) / 256;
-        if (tpc2 * n_clips * std::max(1, p->k2.passes) > 0x7fffffffLL) { if (scratch) cudaFreeAsync(scratch, st); return fail(MELT_ERR_UNSUPPORTED, "too many tiles"); }
+        const long long cpc2 = (T + 31) / 32;                          // 32-frame chunks per clip; a tile = 8 consecutive chunks of the batch
+        const long long nt2 = (cpc2 * n_clips + 7) / 8;
+        if (cpc2 * n_clips > 0x7fffffffLL || nt2 * std::max(1, p->k2.passes) > 0x7fffffffLL) { if (scratch) cudaFreeAsync(scratch, st); return fail(MELT_ERR_UNSUPPORTED, "too many tiles"); }
         k2.x = x; k2.out = out; k2.tap = tap; k2.n_clips = n_clips; k2.len = len; k2.frames_per_clip = T;
         k2.out_dtype = p->out_dtype;
-        k2.tiles_per_clip = (int)tpc2; k2.n_tiles = (int)(tpc2 * n_clips);
+        k2.chunks_per_clip = (int)std::max(1LL, cpc2); k2.n_tiles = (int)nt2;
         k2.offsets = nullptr; k2.frame_offsets = nullptr; k2.tile_prefix = nullptr;
         v2_encode_tmap(k2);
         if (!k2.direct || k2.tma_rows > 0) {   // (K-step staging needs its tensor map; without one the general kernel takes the batch)
@@ -697,7 +698,7 @@ extern "C" int melt_forward_ragged_noalloc(const melt_plan *p, const float *x, c
         rc = launch_ragged_scan(p, offsets, n_clips, out_frame_offsets, tile_prefix, 32, st);   // exclusive prefix of 32-frame chunks per clip
         K2Params k2 = p->k2;
         k2.x = x; k2.out = out; k2.tap = nullptr; k2.n_clips = n_clips; k2.len = 0; k2.frames_per_clip = 0;
-        k2.tiles_per_clip = 0; k2.n_tiles = -1;
+        k2.chunks_per_clip = 0; k2.n_tiles = -1;
         k2.offsets = offsets; k2.frame_offsets = out_frame_offsets; k2.tile_prefix = tile_prefix;
         k2.vpad = p->pad == MELT_PAD_REFLECT ? p->n_fft / 2 : 0;
         k2.out_dtype = p->out_dtype;

@@ -94,7 +94,7 @@ struct K2Params {
     float *out, *tap;
     int n_clips;
     long long len, frames_per_clip;
-    int tiles_per_clip, n_tiles;  // 256-frame tiles
+    int chunks_per_clip, n_tiles; // dense: 32-frame chunks per clip; tiles of 8 consecutive chunks of the batch (256 frames)
     // ---- batch (ragged: clips packed back to back; offsets != nullptr selects this form, frame-major output only)
     const long long *offsets;        // device sample offsets (n_clips + 1)
     const long long *frame_offsets;  // device frame offsets (n_clips + 1), written by the scan kernel
