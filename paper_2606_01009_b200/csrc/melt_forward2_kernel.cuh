@@ -346,44 +346,68 @@ __device__ __forceinline__ float *out_at(const K2Params &p, long long idx) {
     return p.out_dtype == 0 ? p.out + idx : reinterpret_cast<float *>(reinterpret_cast<unsigned short *>(p.out) + idx);
 }
 
-// Where a 256-frame tile lives: dense batches by division, ragged ones by binary search in the device-side tile prefix.
+// Where the 32-frame chunk of one lane quarter of a tile lives.
 struct Tile2 {
-    int clip, t0;      // clip index, first frame of the tile within the clip
+    int clip, t0;      // clip index, first frame of the chunk within the clip
     long long T;       // frames of the clip
     long long s0;      // index of the clip's first sample in x
     long long f0;      // index of the clip's first frame in the (packed or dense) frame order
     int pass;          // pass over the Mel bins (more than 128 bins: every tile is visited once per pass)
 };
-// Dense batches: a tile is 256 consecutive frames of one clip, found by division.  Ragged batches: the clips are cut into
-// 32-frame CHUNKS (the unit one converter / epilogue warp works on) and a tile is any 8 consecutive chunks of the packed
-// chunk order -- the four lane quarters of a CTA may belong to different clips, so the tail of a clip wastes at most 31 rows
-// instead of up to 255.  Only the loader looks chunks up (chunk_prefix, written by the scan kernel, is the exclusive prefix
-// of chunks per clip); it hands what the other warps need to them in shared memory (ChunkInfo).
+// The clips are cut into 32-frame CHUNKS (the unit one converter / epilogue warp works on) and a tile is any 8 consecutive chunks
+// of the packed chunk order -- the four lane quarters of a CTA may belong to different clips, so the tail of a clip wastes at most
+// 31 rows instead of up to 255.  Ragged batches: only the loader looks chunks up (chunk_prefix, written by the scan kernel, is the
+// exclusive prefix of chunks per clip); it hands what the other warps need to them in shared memory (ChunkInfo).  Dense batches:
+// every warp finds its chunk by arithmetic (ChunkCursor).
 struct ChunkInfo {
     long long row0;   // index of the chunk's first frame in the packed output
     int nvalid;       // frames of the chunk that exist (0 .. 32)
     int dlt;          // words by which the staged chunk sits further into its rows than the load table says (clip offset & 3)
 };
-template <bool RAGGED>
-__device__ __forceinline__ void get_tile2(const K2Params &p, int vtile, int rank, int q, Tile2 &ti) {
-    static_assert(!RAGGED, "ragged batches: the loader tracks the clip of every chunk itself");
-    // Dense batches: the chunk of lane quarter q of CTA `rank` in tile `vtile`.  The clips are cut into 32-frame chunks and a tile is
-    // any 8 consecutive chunks of the batch (chunks_per_clip per clip, clip after clip), as in a ragged batch: the tail of a clip
-    // wastes at most 31 rows instead of up to 255 -- 376 instead of 384 tiles on the Whisper-shaped batch, 216 instead of 256 on
-    // 64 x 858 frames -- and every warp finds its chunk by one division.  ti.t0 = first frame of THAT chunk within its clip.
-    int tile = vtile;
-    ti.pass = 0;
-    if (p.passes > 1) { tile = vtile / p.passes; ti.pass = vtile - tile * p.passes; }
-    const int g = tile * 8 + rank * 4 + q;
-    int b = g / p.chunks_per_clip;
-    int c = g - b * p.chunks_per_clip;
-    if (b >= p.n_clips) { b = 0; c = p.chunks_per_clip; }   // beyond the last chunk of the batch: t0 >= T, no frames
-    ti.clip = b;
-    ti.t0 = c * 32;
-    ti.T = p.frames_per_clip;
-    ti.s0 = (long long)b * p.len;
-    ti.f0 = (long long)b * p.frames_per_clip;
-}
+// Dense batches: the clips are cut into 32-frame chunks and a tile is any 8 consecutive chunks of the batch (chunks_per_clip per
+// clip, clip after clip), as in a ragged batch: the tail of a clip wastes at most 31 rows instead of up to 255 -- 376 instead of 384
+// tiles on the Whisper-shaped batch, 216 instead of 256 on 64 x 858 frames.  Chunk g = 8 tile + 4 rank + q is chunk g % chunks_per_clip
+// of clip g / chunks_per_clip; Tile2::t0 = first frame of THAT chunk within its clip.
+// The mapping without a division per tile: a CTA's visits are tile_step apart, so the chunk of a fixed lane quarter advances by
+// a fixed number of chunks from one visit to the next -- (adv_b clips, adv_c chunks) with one carry; with several passes over the
+// bins (a tile is visited once per pass, visit = tile * passes + pass) the pass advances too, and its carry moves one tile (8 chunks)
+// further.  (Four divisions per tile in the loader warp, the pacemaker of the kernel, cost 2-4 % on the workloads whose tile count
+// the packing does not change.)
+struct ChunkCursor {
+    int b, c, pass, adv_b, adv_c, adv_p, cpc, passes;
+    __device__ __forceinline__ void init(const K2Params &p, int first_visit, int visit_step, int rank, int q) {
+        cpc = p.chunks_per_clip;
+        passes = p.passes;
+        const int tile0 = first_visit / passes, dt = visit_step / passes;
+        pass = first_visit - tile0 * passes;
+        adv_p = visit_step - dt * passes;
+        const int g0 = tile0 * 8 + rank * 4 + q;
+        b = g0 / cpc;
+        c = g0 - b * cpc;
+        const int adv = 8 * dt;
+        adv_b = adv / cpc;
+        adv_c = adv - adv_b * cpc;
+    }
+    __device__ __forceinline__ void next() {
+        b += adv_b;
+        c += adv_c;
+        pass += adv_p;
+        if (pass >= passes) { pass -= passes; c += 8; }
+        while (c >= cpc) { c -= cpc; ++b; }
+    }
+    // the chunk dq lane quarters further on (dq < 4)
+    __device__ __forceinline__ void get(const K2Params &p, int dq, Tile2 &ti) const {
+        int bb = b, cc = c + dq;
+        while (cc >= cpc) { cc -= cpc; ++bb; }
+        if (bb >= p.n_clips) { bb = 0; cc = cpc; }   // beyond the last chunk of the batch: t0 >= T, no frames
+        ti.pass = pass;
+        ti.clip = bb;
+        ti.t0 = cc * 32;
+        ti.T = p.frames_per_clip;
+        ti.s0 = (long long)bb * p.len;
+        ti.f0 = (long long)bb * p.frames_per_clip;
+    }
+};
 
 // Ragged batches: a clip starts at any sample of the packed buffer, but the copy engines want 16-byte aligned sources, so a
 // chunk is fetched from the aligned sample below its start: frame sample n then sits dlt = (clip offset & 3) words further
@@ -566,9 +590,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
             const uint32_t ring0 = sbase + p.off_stg + (uint32_t)(lane * 2) * (uint32_t)p.kslot_bytes;
             const uint32_t half = (uint32_t)p.kslot_bytes >> 1;
             const int nblk = (p.units + 3) >> 2;
+            ChunkCursor cur;
+            cur.init(p, first_tile, tile_step, (int)rank, lane & 3);
             for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
                 Tile2 ti;
-                get_tile2<false>(p, tile, (int)rank, lane & 3, ti);
+                cur.get(p, 0, ti);
+                cur.next();
                 const int r0 = ti.t0;   // first frame of the quarter's chunk (rows beyond the clip are zero-filled)
                 for (int kb = 0; kb < nblk; ++kb) {
                     if (active) {
@@ -617,12 +644,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
         const int c0_pad = vr ? p.hop - vr : 0, r_pad = vq + (vr ? 1 : 0);
         long long rg_rclip = 0;
         int rg_cclip = 0;
+        ChunkCursor cur;   // dense: the chunk of lane quarter 0 of the current tile
+        if constexpr (!ragged) cur.init(p, first_tile, tile_step, (int)rank, 0);
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             for (int q = 0; q < 4; ++q) {
                 Tile2 ti;
                 long long row0;
                 if constexpr (!ragged) {
-                    get_tile2<false>(p, tile, (int)rank, q, ti);
+                    cur.get(p, q, ti);
                     row0 = (long long)ti.t0;
                 } else {
                     const int g = (p.passes > 1 ? tile / p.passes : tile) * 8 + (int)rank * 4 + q;   // chunk index in the packed chunk order
@@ -816,6 +845,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                 if (++cq == 4) { cq = 0; if (++ctp == P) { ctp = 0; cph ^= 1u; } }
             }
             ++tl;
+            if constexpr (!ragged) cur.next();
         }
         (void)cph;
         if (EARLY_LOADER) cluster_wait();   // the phase it arrived on at set-up, before the exit barrier below
@@ -1040,6 +1070,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
         // (plain log-Mel output never comes here: it runs without epilogue warps, MODE 2)
         bool dep_done = false;
         int tl = 0;   // tiles of this CTA so far
+        ChunkCursor cur;   // dense: this warp's chunk of the current tile
+        if constexpr (!RAGGED) cur.init(p, first_tile, tile_step, (int)rank, q);
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             // where this warp's 32 rows go: dense batches by division; ragged ones from the loader's chunk record (acquired through
             // the INFO barrier of this ring entry: this warp is its only waiter and waits for each of its phases once, in order)
@@ -1053,7 +1085,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                 ti.clip = 0; ti.t0 = 0; ti.T = 0; ti.s0 = 0; ti.f0 = 0;
                 ti.pass = p.passes > 1 ? tile % p.passes : 0;
             } else {
-                get_tile2<false>(p, tile, (int)rank, q, ti);
+                cur.get(p, 0, ti);
+                cur.next();
                 out_row0 = 0; nvalid32 = 0;
             }
             ++tl;
@@ -1123,6 +1156,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
         // SHARE (single accumulator stage, log-Mel): this warp also drains its share of the previous tile's accumulator --
         // after its second K-step of the next tile, so that the MMAs find operands waiting when the drain releases them.
         int pend_tile = -1, pend_tl = 0, dstage = 0;
+        ChunkCursor dcur;   // dense: this warp's chunk of the tile to drain next
+        if constexpr (!RAGGED) dcur.init(p, first_tile, tile_step, (int)rank, q);
         int tl = 0;   // tiles of this CTA so far
         // K-block staging (DIRECT): the two-slot ring of this lane quarter, fed by lane q of the loader warp; a row = 4 KS + 4 samples
         const int kidx = 2 * q;
@@ -1146,7 +1181,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                 dvalid = lane < ci.nvalid;                                                                       \
                 doptr = out_at(p, (ci.row0 + lane) * p.n_ch + dc_off);                                           \
             } else {                                                                                             \
-                get_tile2<false>(p, pend_tile, (int)rank, q, dt);                                                \
+                dcur.get(p, 0, dt);   /* tiles are drained in order */                                           \
+                dcur.next();                                                                                     \
                 const int drow = q * 32 + lane, dt0 = dt.t0 - q * 32;                                            \
                 dvalid = (long long)(dt0 + drow) < dt.T;                                                         \
                 dc_off = dt.pass * p.nb;                                                                         \
