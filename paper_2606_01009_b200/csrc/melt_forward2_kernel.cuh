@@ -1419,7 +1419,7 @@ static int launch_one_s(const K2Params &kp, int grid, cudaStream_t stream) {
         attr_done.fetch_or(bit, std::memory_order_release);
     }
     // Programmatic dependent launch: the CTAs of this grid are dispatched as soon as SMs of the previous kernel in the stream
-    // free up (its clusters finish at different times: 384 tiles on 74 pairs), instead of after its last CTA has retired and
+    // free up (its clusters finish at different times: 376 tiles on 74 pairs), instead of after its last CTA has retired and
     // a fresh launch has ramped up.  The kernel orders itself behind that kernel with griddepcontrol.wait: before its first read
     // of the caller's buffers by default, before its first global store only when the caller vouches for the input
     // (K2Params::input_ready, MELT_OPT_INPUT_READY).
