@@ -429,6 +429,11 @@ __global__ void __launch_bounds__(1024, 1) ragged_scan_kernel(const KParams p, c
     __shared__ long long carry_f;
     __shared__ int carry_t;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // Programmatic dependent launch (see launch_ragged_scan): this block may have been scheduled while the previous kernel of the
+    // stream is still running -- the forward kernel behind it may be scheduled now, and nothing is read or written before that
+    // previous kernel (which may produce `offsets`, or still read the arrays written below) has completed.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (tid == 0) { carry_f = 0; carry_t = 0; }
     __syncthreads();
     for (int base = 0; base < n_clips; base += 1024) {
@@ -472,8 +477,20 @@ __global__ void __launch_bounds__(1024, 1) ragged_scan_kernel(const KParams p, c
 }
 
 int launch_ragged_scan(const melt_plan *pl, const long long *offsets, int n_clips, long long *frame_offsets, int *tile_prefix, int tile_m, cudaStream_t stream) {
-    ragged_scan_kernel<<<1, 1024, 0, stream>>>(pl->kp, offsets, n_clips, frame_offsets, tile_prefix, tile_m);
-    MELT_CUDA(cudaGetLastError());
+    // launched like the forward kernels (programmatic stream serialisation): the block is scheduled as soon as an SM of the previous
+    // kernel frees up and orders itself behind that kernel with griddepcontrol.wait, instead of paying a full launch latency after
+    // the previous forward has drained -- and the forward kernel behind it is scheduled early in turn
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(1, 1, 1);
+    cfg.blockDim = dim3(1024, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    MELT_CUDA(cudaLaunchKernelEx(&cfg, ragged_scan_kernel, pl->kp, offsets, n_clips, frame_offsets, tile_prefix, tile_m));
     return MELT_OK;
 }
 
