@@ -787,18 +787,35 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                     continue;
                 }
                 if (ragged && !by_tma) {
-                    // the few chunks that reach beyond the packed buffer (end of the last clip), or rows of no valid frame:
-                    // plain bounds-checked loads by the whole warp (the bulk-copy engine needs 16-byte aligned sources)
+                    // The chunk that reaches beyond the packed buffer (the last one of the last clip; or a chunk without rows): hop-rows
+                    // that lie inside the buffer as one bulk copy each (s, hop and the pitch are multiples of 4 samples), the one or
+                    // two that straddle its end and those beyond it element by element, zeros past the end.  It is ONE chunk per
+                    // call, but the LAST one: read element by element as a whole (180 dependent iterations of a global load and a
+                    // shared store in this warp) it kept its CTA pair busy for ~20 us after every other pair had finished -- a
+                    // tenth of the speaker-style batch (trace: the ragged kernel's tiles were as fast as the dense kernel's).
                     const int pw = p.pitch_bytes >> 2;
-                    const int n_el = n_rows * pw;
                     float *dstp = reinterpret_cast<float *>(smem + p.off_stg + (size_t)slot * p.slot_bytes);
-                    for (int idx = lane; idx < n_el; idx += 32) {
-                        const int r = idx / pw;
-                        const long long g = s + (long long)r * p.hop + (idx - r * pw);
-                        dstp[idx] = g < total ? __ldg(p.x + g) : 0.f;
+                    uint32_t bulk_bytes = 0;
+                    for (int r = 0; r < n_rows; ++r) {
+                        const long long gl = s + (long long)r * p.hop;
+                        if (gl >= 0 && gl + pw <= total) { bulk_bytes += (uint32_t)p.pitch_bytes; continue; }
+                        for (int col = lane; col < pw; col += 32) {
+                            const long long g = gl + col;
+                            dstp[r * pw + col] = (g >= 0 && g < total) ? __ldg(p.x + g) : 0.f;
+                        }
+                    }
+                    __syncwarp();   // every lane's stores precede lane 0's arrival below
+                    if (lane == 0) {
+                        *info = info_v;
+                        mbar_arrive(info_bar);
+                        if (bulk_bytes) mbar_arrive_expect_tx(full, bulk_bytes);
+                        else mbar_arrive(full);
                     }
                     __syncwarp();
-                    if (lane == 0) { *info = info_v; mbar_arrive(info_bar); mbar_arrive(full); }
+                    for (int r = lane; r < n_rows; r += 32) {   // a row per lane (the phase cannot complete before lane 0's arrival above)
+                        const long long gl = s + (long long)r * p.hop;
+                        if (gl >= 0 && gl + pw <= total) bulk_g2s(dst0 + (uint32_t)r * (uint32_t)p.pitch_bytes, p.x + gl, (uint32_t)p.pitch_bytes, full);
+                    }
                     __syncwarp();
                     TRACE(12);
                     if (++slot == S) slot = 0;
