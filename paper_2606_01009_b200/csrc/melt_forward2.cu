@@ -64,7 +64,7 @@ int plan_build_v2(melt_plan *p) {
     k.unit_b_bytes = (uint32_t)k.nk * k.kind_bytes;
     k.dct_pitch = k1.dct_pitch;
     const uint32_t b_bytes = (uint32_t)k.units * k.unit_b_bytes;
-    const uint32_t dct_only = p->n_mfcc > 0 ? (uint32_t)(M * k.dct_pitch * 4) : 0;
+    const uint32_t dct_only = p->n_mfcc > 0 ? (uint32_t)(std::max(M, k.nb) * k.dct_pitch * 4) : 0;   // rows for the bins that pad the last block too (zero)
     // MFCCT, frame-major: 4 epilogue warps x 32 frames x n_mfcc floats behind the DCT table (cepstra transposed for coalesced stores)
     const uint32_t epi_bytes = (p->n_mfcc > 0 && p->layout == MELT_LAYOUT_FRAME_MAJOR) ? (uint32_t)(4 * 32 * p->n_mfcc * 4) : 0;
     const uint32_t fb_bytes = fbank ? (uint32_t)round_up2((int)(2u * (uint32_t)k.fb_units * k.fb_kind_bytes), 128) : 0;   // this CTA's half of the filterbank image

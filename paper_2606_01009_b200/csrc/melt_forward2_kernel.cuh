@@ -224,34 +224,48 @@ __device__ __forceinline__ void epi_generic(const K2Params &p, uint32_t t_r, uin
             tmem_ld16(t_r + (uint32_t)c0, vr);
             tmem_ld16(t_i + (uint32_t)c0, vi);
             tmem_wait_ld();
+            // The 16 values of the block first, all independent (power, one MUFU.LG2, FMA, max each), THEN the DCT / the stores: with
+            // the per-bin guard `m < nm` around everything, every bin was a branch target of its own and its latency chain (FMA ->
+            // LG2 -> FMA -> max -> 16 FMAs) ran alone -- the four epilogue warps took ~7000 of every ~8000 cycles of a tile of the
+            // speaker-style batch and the MMA issuers waited 3300 of them for an accumulator stage (r02 trace).  Bins beyond the
+            // plan's (the block is padded to 16) carry zero basis rows, hence finite values, and meet ZERO rows of the DCT table
+            // (cleared at set-up), so the DCT needs no guard; the stores keep theirs as a predicate.
+            const int nfull = nm - c0;   // bins of this block that exist (>= 16: all of them)
+            float v[16];
+            const bool is_power = p.output_power == 1;
 #pragma unroll
             for (int c = 0; c < 16; ++c) {
-                const int m = c0 + c;
-                if (m < nm) {
-                    const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
-                    const float praw = fmaf(r, r, im * im);                                          // Eq. (4)
-                    float v;
-                    // one formula for both log forms (two branches inside the unrolled bin loop cost the ragged MFCCT batch 35 %):
-                    //   contract form (Eq. 8, DESIGN R2): log10(max(S, 1e-10)) = max(lg2(1 * praw + 0) * log10(2) + offset, -10)
-                    //   printed form:                     ln(S + eps)          = max(lg2(scale * praw + eps) * ln(2) + 0, -inf)
-                    if (p.output_power == 1) v = praw * p.out_scale;
-                    else v = fmaxf(fmaf(lg2_ftz(fmaf(praw, la, lb)), lc, ld), lmin);
-                    if (HAS_DCT) {
-                        const float *drow = dct_s + m * p.dct_pitch + q0;
-                        // (scalar FMAs on purpose: packed FFMA2 pairs measured 6.5 % SLOWER on the ragged MFCCT batch, 226.7 vs 212.8 us)
+                const float r = __uint_as_float(vr[c]), im = __uint_as_float(vi[c]);
+                const float praw = fmaf(r, r, im * im);                                          // Eq. (4)
+                // one formula for both log forms (two branches inside the unrolled bin loop cost the ragged MFCCT batch 35 %):
+                //   contract form (Eq. 8, DESIGN R2): log10(max(S, 1e-10)) = max(lg2(1 * praw + 0) * log10(2) + offset, -10)
+                //   printed form:                     ln(S + eps)          = max(lg2(scale * praw + eps) * ln(2) + 0, -inf)
+                const float lv = fmaxf(fmaf(lg2_ftz(fmaf(praw, la, lb)), lc, ld), lmin);
+                v[c] = is_power ? praw * p.out_scale : lv;
+            }
+            if (HAS_DCT) {
+                if (q0 == 0 && tptr && valid) {
 #pragma unroll
-                        for (int q4 = 0; q4 < 4; ++q4) {   // the table's rows are zero padded to whole blocks of 16 cepstra
-                            const float4 d = *reinterpret_cast<const float4 *>(drow + 4 * q4);   // D[q0 + 4 q4 .. + 3][m]
-                            cacc[4 * q4 + 0] = fmaf(d.x, v, cacc[4 * q4 + 0]);
-                            cacc[4 * q4 + 1] = fmaf(d.y, v, cacc[4 * q4 + 1]);
-                            cacc[4 * q4 + 2] = fmaf(d.z, v, cacc[4 * q4 + 2]);
-                            cacc[4 * q4 + 3] = fmaf(d.w, v, cacc[4 * q4 + 3]);
-                        }
-                        if (q0 == 0 && tptr && valid) tptr[m * cstride] = v;
-                    } else if (valid) {
-                        optr[m * cstride] = v;
+                    for (int c = 0; c < 16; ++c)
+                        if (c < nfull) tptr[(c0 + c) * cstride] = v[c];
+                }
+                const float *drow = dct_s + c0 * p.dct_pitch + q0;
+                // (scalar FMAs on purpose: packed FFMA2 pairs measured 6.5 % SLOWER on the ragged MFCCT batch, 226.7 vs 212.8 us)
+#pragma unroll
+                for (int c = 0; c < 16; ++c) {
+#pragma unroll
+                    for (int q4 = 0; q4 < 4; ++q4) {   // the table's rows are zero padded to whole blocks of 16 cepstra
+                        const float4 d = *reinterpret_cast<const float4 *>(drow + c * p.dct_pitch + 4 * q4);   // D[q0 + 4 q4 .. + 3][c0 + c]
+                        cacc[4 * q4 + 0] = fmaf(d.x, v[c], cacc[4 * q4 + 0]);
+                        cacc[4 * q4 + 1] = fmaf(d.y, v[c], cacc[4 * q4 + 1]);
+                        cacc[4 * q4 + 2] = fmaf(d.z, v[c], cacc[4 * q4 + 2]);
+                        cacc[4 * q4 + 3] = fmaf(d.w, v[c], cacc[4 * q4 + 3]);
                     }
                 }
+            } else if (valid) {
+#pragma unroll
+                for (int c = 0; c < 16; ++c)
+                    if (c < nfull) optr[(c0 + c) * cstride] = v[c];
             }
         }
         if (!HAS_DCT || q0 + 16 >= K) {   // last pass over the accumulators: the MMAs of the tile after next may overwrite them
@@ -540,8 +554,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
         if (FB && t64 >= 10 && t64 < 13) mbar_init(BAR(V_D2_FULL + (t64 - 10)), 1u);     // D2_FULL, FB_FULL, FB_PEER
         fence_barrier_init();
     }
-    if (p.n_mfcc > 0)
-        for (int i = tid; i < p.n_mels * p.dct_pitch; i += NT) dct_s[i] = __ldg(p.dct + i);
+    if (p.n_mfcc > 0)   // the DCT table, with zero rows for the bins that pad the last 16-bin block (see epi_generic)
+        for (int i = tid; i < p.nb * p.dct_pitch; i += NT) dct_s[i] = i < p.n_mels * p.dct_pitch ? __ldg(p.dct + i) : 0.f;
     TRACE_PT(1);
     uint32_t tmem_base = 0;
     if (EARLY_LOADER && warp == W_LOAD) {
