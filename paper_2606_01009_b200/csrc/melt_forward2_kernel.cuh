@@ -382,6 +382,20 @@ struct ChunkInfo {
 // clip, clip after clip), as in a ragged batch: the tail of a clip wastes at most 31 rows instead of up to 255 -- 376 instead of 384
 // tiles on the Whisper-shaped batch, 216 instead of 256 on 64 x 858 frames.  Chunk g = 8 tile + 4 rank + q is chunk g % chunks_per_clip
 // of clip g / chunks_per_clip; Tile2::t0 = first frame of THAT chunk within its clip.
+// The order in which the loader issues the four chunks of a tile.  The staging ring holds less than two tiles, so the chunk issued LAST
+// only starts when a chunk of the current tile is released, and its converter warps wait for it at every tile boundary (~1000 cycles
+// in the r02 trace).  Dense batches give that wait to lane quarter 2 -- whose converter warps share their scheduler with no MMA issuer
+// and run a K-step ~230 cycles faster than those of quarters 1 and 3 -- instead of quarter 3, the slowest.  Ragged batches keep the
+// natural order (the loader's clip search only moves forward).
+#ifndef MELT_CHUNK_ORDER
+#define MELT_CHUNK_ORDER 0x2013   /* nibble qi: quarter issued qi-th = 3, 1, 0, 2 */
+#define MELT_CHUNK_POS 0x0312     /* nibble q: position of quarter q in that order */
+#endif
+template <bool RAGGED>
+__device__ __forceinline__ int chunk_order(int qi) { return RAGGED ? qi : (MELT_CHUNK_ORDER >> (4 * qi)) & 3; }
+template <bool RAGGED>
+__device__ __forceinline__ int chunk_pos(int q) { return RAGGED ? q : (MELT_CHUNK_POS >> (4 * q)) & 3; }
+
 // The mapping without a division per tile: a CTA's visits are tile_step apart, so the chunk of a fixed lane quarter advances by
 // a fixed number of chunks from one visit to the next -- (adv_b clips, adv_c chunks) with one carry; with several passes over the
 // bins (a tile is visited once per pass, visit = tile * passes + pass) the pass advances too, and its carry moves one tile (8 chunks)
@@ -661,7 +675,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
         ChunkCursor cur;   // dense: the chunk of lane quarter 0 of the current tile
         if constexpr (!ragged) cur.init(p, first_tile, tile_step, (int)rank, 0);
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
-            for (int q = 0; q < 4; ++q) {
+            for (int qi = 0; qi < 4; ++qi) {
+                const int q = chunk_order<ragged>(qi);   // the lane quarter whose chunk is issued qi-th
                 Tile2 ti;
                 long long row0;
                 if constexpr (!ragged) {
@@ -736,10 +751,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                 __syncwarp();
                 TRACE(10);
                 if (chunk_count >= S) {      // the slot's previous tenant, chunk c - S, has been read by every converter group
-                    mbar_wait(BAR(V_STG_EMPTY + eq + 4 * etp), eph);
+                    mbar_wait(BAR(V_STG_EMPTY + chunk_order<ragged>(eq) + 4 * etp), eph);
                     if (++eq == 4) { eq = 0; if (++etp == P) { etp = 0; eph ^= 1u; } }
                 }
-                const uint32_t full = BAR(V_STG_FULL + cq + 4 * ctp);
+                const uint32_t full = BAR(V_STG_FULL + q + 4 * ctp);
                 // ragged: the chunk's misalignment travels with it (read by the converters after their wait on `full`; the
                 // thread that writes it is the one that arrives on `full`, so the arrival publishes it)
                 ChunkInfo *const info = chunk_info + q + 4 * (tl & 7);
@@ -1179,7 +1194,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
         const uint32_t a_full_remote = mapa_cluster(BAR(V_A_FULL), 0);
         const uint32_t row_off = sbase + p.off_stg + (uint32_t)lane * (uint32_t)p.pitch_bytes;
         const float S_in = p.in_scale;
-        int sslot = q;                           // memory slot of this warp's chunk: (4 tl + q) mod S
+        int sslot = chunk_pos<RAGGED>(q);        // memory slot of this warp's chunk: (4 tl + its position in the loader's issue order) mod S
         int sbar = q;                            // its barriers: q + 4 (tl mod P) (see the loader)
         uint32_t sph = 0;
         int aslot = g % p.a_slots;               // ring position of unit counter ug = it * units + u, first u = g
