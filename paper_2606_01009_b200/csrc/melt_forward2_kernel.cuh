@@ -497,6 +497,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
     static_assert(!FB || (STREAM && !DIRECT && !RAGGED && PREC == P2_COMP), "MODE 4: dense batches, streamed basis, compensated operands");
     constexpr int NG = (MODE == 2 || MODE == 3 || MODE == 5) ? V2_CONV_GROUPS : V2_CONV_GROUPS - 1;   // converter groups: 3 without epilogue warps, 2 next to them
     constexpr int NT = v2_threads(MODE);                                  // threads of the block
+    // Dense batches: the four chunks of a CTA's FIRST tile are requested by its four epilogue / drain warps (idle until the first
+    // accumulator is full), one each and all at once, not one after the other by the loader warp, whose per-chunk bookkeeping (~700
+    // cycles) spread them over the first ~5000 cycles of every launch (r02 trace: first MMA 7300 cycles after the CTA's entry).
+    constexpr bool HELPED = !RAGGED && !DIRECT && MODE != 2;
     constexpr int CONV0 = MODE == 2 ? W_EPI0 : W_CONV0;                   // first converter warp
     constexpr int DRAINERS = MODE == 2 ? NG : 1 + NG;                     // warps per lane quarter that drain (SHARE)
     constexpr int DRAIN0 = MODE == 2 ? 0 : 1;                             // block index of converter group 0's share
@@ -577,7 +581,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
         asm volatile("bar.sync 1, %0;" ::"n"(NT - 96) : "memory");
         cluster_arrive_relaxed();
     } else {
-        if (EARLY_LOADER && tid >= 128) asm volatile("bar.arrive 1, %0;" ::"n"(NT - 96) : "memory");
+        if (EARLY_LOADER && tid >= 128) {
+            // (the warps that issue the first tile's copies wait like the loader: margins cleared, staging barriers set up)
+            if (HELPED && warp >= W_EPI0 && warp < W_EPI0 + 4) asm volatile("bar.sync 1, %0;" ::"n"(NT - 96) : "memory");
+            else asm volatile("bar.arrive 1, %0;" ::"n"(NT - 96) : "memory");
+        }
         TRACE_PT(2);
         tc_fence_before();
         asm volatile("bar.sync 2, %0;" ::"n"(SETUP_THREADS) : "memory");   // tensor memory allocated, barriers set up (this CTA)
@@ -732,6 +740,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
                 if (!ragged) {
                     if (p.vpad == 0) {
                         by_tma = n_rows > 0 && row0 + n_rows <= (long long)p.tma_rows;
+                        if (HELPED && tl == 0 && by_tma) {   // requested by the epilogue warp of this lane quarter (same predicate there)
+                            if (++slot == S) slot = 0;
+                            ++chunk_count;
+                            if (++cq == 4) { cq = 0; if (++ctp == P) { ctp = 0; cph ^= 1u; } }
+                            continue;
+                        }
                     } else {
                         c0 = c0_pad; c1 = (int)row0 - r_pad;    // st = c1 * hop + c0 (st >= 0)
                         by_tma = n_rows > 0 && st >= 0 && (long long)c1 + n_rows <= (long long)p.tma_rows;   // every row of the box inside the clip
@@ -1118,6 +1132,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(v2_threads(MODE), 1)
         int tl = 0;   // tiles of this CTA so far
         ChunkCursor cur;   // dense: this warp's chunk of the current tile
         if constexpr (!RAGGED) cur.init(p, first_tile, tile_step, (int)rank, q);
+        if constexpr (HELPED) {
+            // the chunk of this lane quarter of the CTA's first tile, if it is an ordinary one (one tensor-map box): see HELPED
+            if (warp < W_EPI0 + 4 && first_tile < n_tiles && p.vpad == 0) {
+                Tile2 ht;
+                cur.get(p, 0, ht);
+                if ((long long)ht.t0 < ht.T && ht.t0 + p.rows_per_chunk <= p.tma_rows) {
+                    if (lane == 0) {
+                        const uint32_t full = BAR(V_STG_FULL + q);   // tile phase 0
+                        mbar_arrive_expect_tx(full, (uint32_t)p.rows_per_chunk * (uint32_t)p.pitch_bytes);
+                        tma_load_3d(sbase + p.off_stg + (uint32_t)chunk_pos<RAGGED>(q) * (uint32_t)p.slot_bytes, p.tmap, 0, ht.t0, ht.clip, full);
+                    }
+                    __syncwarp();
+                }
+            }
+        }
         for (int tile = first_tile; tile < n_tiles; tile += tile_step) {
             // where this warp's 32 rows go: dense batches by division; ragged ones from the loader's chunk record (acquired through
             // the INFO barrier of this ring entry: this warp is its only waiter and waits for each of its phases once, in order)
